@@ -1,0 +1,201 @@
+/* soax.h -- C ABI of the B200-native SoAx hot path (arXiv 1710.03462, "SoAx: A generic C++ Structure of
+ * Arrays for handling particles in HPC codes").
+ *
+ * What the library is: per-particle streaming updates over heterogeneous particle records stored as a
+ * Structure of Arrays (one contiguous device array per field COMPONENT, PAPER.md:95-116 Listings 2-3 and
+ * PAPER.md:155 "three heap-allocated C++ arrays for x and v, respectively"), the AoS<->SoA transposition
+ * (PAPER.md:118), a double-precision energy reduction and PIC-style cell binning with a permutation of every
+ * field array, on one B200 (sm_100a).  Citations "PAPER.md:<line>" refer to the paper text;
+ * "Qn" to the readings listed in DESIGN.md.
+ *
+ * Conventions (all calls):
+ *   - plain C, no exceptions; every call returns an int status: SOAX_OK (0) or a negative soax_status;
+ *   - pointers named dev_* are DEVICE pointers, host_* are HOST pointers, everything else is host memory;
+ *   - the CALLER owns all device memory (PyTorch tensors in the harness); the library never calls cudaMalloc.
+ *     soax_alloc only carves a caller-provided slab into aligned per-component arrays;
+ *   - work is ENQUEUED on the caller's stream (`stream` = a cudaStream_t cast to void*, NULL = legacy default
+ *     stream) and no call synchronises, except where stated; scalar results go to device pointers;
+ *   - element counts are int64_t; permutations, counts and offsets are uint32_t device arrays (n < 2^32);
+ *   - floating point is IEEE-754 binary64/binary32, round to nearest even, no fast-math; every fused
+ *     multiply-add is explicit, so results are bit-reproducible.
+ */
+#ifndef SOAX_H
+#define SOAX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default) /* the library is built with -fvisibility=hidden: only this header is exported */
+#endif
+
+typedef enum {
+    SOAX_OK = 0,
+    SOAX_ERR_INVALID_ARG = -1,    /* null pointer, negative size, misaligned buffer, n > capacity ...           */
+    SOAX_ERR_UNKNOWN_LAYOUT = -2, /* the field list matches no compiled layout instantiation                    */
+    SOAX_ERR_UNSUPPORTED = -3,    /* the operation needs a field (or a field type / dimension) the layout lacks:
+                                     the run-time face of the paper's compile-time SFINAE check, PAPER.md:320   */
+    SOAX_ERR_ALLOC = -4,          /* slab or scratch too small, or host allocation of a handle failed          */
+    SOAX_ERR_CUDA = -5            /* a CUDA runtime call failed; see soax_last_cuda_error()                     */
+} soax_status;
+
+/* Element type of one field (id<int,1>, pos<double,3>, vel<double,3>, mass<float,1>). */
+typedef enum { SOAX_I32 = 0, SOAX_I64 = 1, SOAX_U8 = 2, SOAX_F32 = 3, SOAX_F64 = 4 } soax_dtype;
+
+/* One attribute of the particle record: the C face of SOAX_ATTRIBUTE(name, tag) plus its <type, dim> entry in
+ * the std::tuple typedef (Listing 5).  dim = 1 (scalar) or 3 (vector), or any positive
+ * count for the benchmark record's temp[SIZE] (Listing 4). */
+typedef struct {
+    const char* name;  /* "id", "pos", "vel", "acc", "mass", "charge", "flags", "temp" */
+    int32_t dtype;     /* a soax_dtype */
+    int32_t dim;
+} soax_field;
+
+typedef struct soax_layout soax_layout; /* opaque; owned by the registry, immutable, lives for the process  */
+typedef struct soax_container soax_t;            /* opaque container: layout + n + capacity + component pointers    */
+
+/* ---- layout registry (Listing 5; D7/D8 of the component inventory) ----------------------
+ * Layouts are COMPILE-TIME typelists (csrc/layout.hpp) whose kernels are generated from C++ templates; this
+ * call canonicalises a run-time field list (names, dtypes and dims, in declaration order) and returns the
+ * matching instantiation.  Built in: R1 {int32 id; double pos[3]; float vel[3]}, R2 {int64 id;
+ * double pos[3]; double vel[3]; double acc[3]; float mass; float charge; uint8 flags} (BASELINE.json config
+ * 4) and B6_S {float pos[3]; float vel[3]; float temp[S]} for S in {0, 8, 16, 32}.
+ * Errors: INVALID_ARG (null, nfields <= 0, bad dtype/dim), UNKNOWN_LAYOUT. */
+int soax_layout_define(const soax_field* fields, int32_t nfields, const soax_layout** out);
+
+/* Number of fields / of component arrays (sum of dims) of a layout; negative status on error. */
+int soax_layout_nfields(const soax_layout* layout);
+int soax_layout_ncomp(const soax_layout* layout);
+/* Describe component c (0 <= c < ncomp, declaration order, component-major): its field index, its index within
+ * the field and its soax_dtype.  Any out pointer may be NULL. */
+int soax_layout_comp(const soax_layout* layout, int32_t c, int32_t* field, int32_t* comp_in_field, int32_t* dtype);
+
+/* Array-of-Structures image of the layout (D1): record stride in bytes and the byte offset of
+ * every component.  packed != 0: declaration order, no padding (R1: stride 40, offsets 0 / 4,12,20 / 28,32,36 --
+ * BASELINE.json config 3, reading Q1); packed == 0: natural C alignment.  comp_offsets has ncomp entries. */
+int soax_layout_aos(const soax_layout* layout, int32_t packed, size_t* stride, size_t* comp_offsets);
+
+/* Bytes of device memory soax_alloc needs for `capacity` particles (each component array starts on a 256-byte
+ * boundary).  Returns 0 on error (null layout, capacity < 0). */
+size_t soax_slab_bytes(const soax_layout* layout, int64_t capacity);
+
+/* ---- container ("Soax<ArrayTypes> soax(42)", PAPER.md:110-116 allocate(n)) -----------------
+ * Carve `dev_slab` (caller-owned device memory, 256-byte aligned, >= soax_slab_bytes(layout, capacity)) into
+ * the per-component arrays and return a handle with n live particles.  The contents of the slab are not
+ * touched.  The handle is host memory; release it with soax_free (which never frees the slab).
+ * Errors: INVALID_ARG (null, n < 0, n > capacity, misaligned slab), ALLOC (slab too small). */
+int soax_alloc(const soax_layout* layout, int64_t n, int64_t capacity, void* dev_slab, size_t slab_bytes,
+               soax_t** out);
+int soax_free(soax_t* s);
+/* Live particle count; resize within capacity (PAPER.md:296 resize; no regrow, no data movement). */
+int64_t soax_size(const soax_t* s);
+int soax_resize(soax_t* s, int64_t n);
+/* Device pointer of one component array: field f, component c -- the paper's posArr(c).
+ * Errors: INVALID_ARG (bad field index), UNSUPPORTED (c outside the field's dimension). */
+int soax_field_ptr(const soax_t* s, int32_t field, int32_t comp, void** dev_ptr);
+
+/* Host <-> device transfer of whole component arrays (the end-to-end path: host buffers in, host buffers
+ * out).  host_comps has ncomp entries, one host array of n elements per component (NULL entries are skipped);
+ * copies are cudaMemcpyAsync on `stream` (truly asynchronous only from pinned host memory).  soax_upload sets
+ * the live count to n (n <= capacity). */
+int soax_upload(soax_t* s, const void* const* host_comps, int64_t n, void* stream);
+int soax_download(const soax_t* s, void* const* host_comps, int64_t n, void* stream);
+
+/* ---- a2..a4, a9: streaming integration steps (Eq. 1 "x += dt v") ------
+ * box = [0,1)^3 with periodic wrap  wrap(x) = x - floor(x), a result of exactly 1.0 mapped to 0.0 (Q3).
+ *   DRIFT                       pos_c = wrap(fma(dt, (double)vel_c, pos_c))                      (configs 1, 5)
+ *   SYMPLECTIC_EULER_HARMONIC   vel_c = fma_V((V)dt, (V)(-(k*(pos_c - center))), vel_c), V = type of vel,
+ *                               then DRIFT with the NEW vel (kick, then drift: Q2, Q4)           (configs 2, 3)
+ *   RK2_MIDPOINT_HARMONIC_MASKED  only for particles with (flags & flag_mask) != 0:               (config 4)
+ *                               w = k/(double)mass; a1 = -(w*(pos-center)); ph = wrap(fma(dt/2, vel, pos));
+ *                               vh = fma(dt/2, a1, vel); a2 = -(w*(ph-center)); pos = wrap(fma(dt, vh, pos));
+ *                               vel = fma(dt, a2, vel); acc = a2 (Q6, Q7, Q8); other particles: no change.
+ *   EULER_NOWRAP                pos_c = fma_P((P)dt, vel_c, pos_c), P = type of pos: Eq. 1 exactly as printed,
+ *                               no wrap (the paper's float benchmark)
+ * Needs fields pos[3] (and vel[3]; RK2 also acc[3] double, mass float, flags uint8): otherwise UNSUPPORTED.
+ * One full read-modify-write pass over memory per step and one kernel launch per step (Q14: no fusion in
+ * time, as in the paper's "loop many times ... and average"). */
+typedef enum {
+    SOAX_STEP_DRIFT = 0,
+    SOAX_STEP_SYMPLECTIC_EULER_HARMONIC = 1,
+    SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED = 2,
+    SOAX_STEP_EULER_NOWRAP = 3
+} soax_step_kind;
+
+typedef struct {
+    int32_t kind;      /* a soax_step_kind */
+    uint8_t flag_mask; /* RK2: particle is active iff (flags & flag_mask) != 0; config 4 uses 1 */
+    uint8_t pad_[3];
+    double dt;
+    double k;      /* spring constant (configs: 1) */
+    double center; /* centre of the harmonic well (configs: 0.5) */
+} soax_step_params;
+
+/* nsteps passes over the n live particles of `s`, in place.  Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+int soax_step(soax_t* s, const soax_step_params* params, int32_t nsteps, void* stream);
+
+/* a5: the same arithmetic on an Array of Structures (packed image of `layout`, see soax_layout_aos), kept as
+ * the in-library comparison baseline (thread per particle, strided access).  variant 0 = the
+ * paper-faithful kernel (one thread per record, direct strided field access); variant 1 = best effort
+ * (whole records staged through shared memory with coalesced 128-bit accesses).  dev_aos: n records,
+ * 16-byte aligned.  Kinds DRIFT and SYMPLECTIC_EULER_HARMONIC. */
+int soax_step_aos(const soax_layout* layout, void* dev_aos, int64_t n, const soax_step_params* params,
+                  int32_t nsteps, int32_t variant, void* stream);
+
+/* a6 / a7: bit copy of every field of every record between the packed AoS image and the component arrays
+ * ("a function copying the array data for one index to the Particle member variables", bulk
+ * form; PAPER.md:304 getElement).  dev_aos: n * stride bytes, 16-byte aligned.  aos_to_soa sets the live
+ * count of dst to n (n <= capacity). */
+int soax_aos_to_soa(soax_t* dst, const void* dev_aos, int64_t n, void* stream);
+int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream);
+
+/* ---- a8: energy reduction in double -----------------------------------------------------------------------
+ *   per particle  q = v0*v0; q = fma(v1,v1,q); q = fma(v2,v2,q)            (v_c = (double)vel_c)
+ *   [+ HARMONIC:  d_c = pos_c - center; q = fma(k*d_c, d_c, q), c = 0,1,2]
+ *   e_i = 0.5*q;  *dev_out = sum_i e_i  (double; fixed reduction tree: run-to-run deterministic)
+ * dev_scratch: >= soax_energy_scratch_bytes() bytes, 8-byte aligned.  dev_out: one double on the device. */
+typedef enum { SOAX_ENERGY_KINETIC = 0, SOAX_ENERGY_KINETIC_PLUS_HARMONIC = 1 } soax_energy_kind;
+size_t soax_energy_scratch_bytes(void);
+int soax_reduce_energy(const soax_t* s, int32_t kind, double k, double center, void* dev_scratch,
+                       size_t scratch_bytes, double* dev_out, void* stream);
+
+/* ---- a10..a14: PIC-style binning (BASELINE.json config 5) ------------------------------------
+ *   cell_i    = (i0*G + i1)*G + i2,  i_c = (int32)(pos_c * G)  (x slowest; pos in [0,1): Q11, Q16)
+ *   counts[c] = #{i : cell_i = c};  offsets = exclusive prefix sum of counts
+ *   perm      = indices 0..n-1 stably sorted by cell (gather map: perm[j] = source index of the particle that
+ *               ends in slot j; ties keep ascending index: Q12);  dst.f[j] = src.f[perm[j]] for EVERY component
+ * The permutation is unique and the result is deterministic for any particle distribution.
+ * grid_dim G: power of two, 1 <= G <= 64 (G^3 <= 2^18 cells).  src is read only; dst: same layout,
+ * capacity >= n, must not alias src; its live count becomes n.  dev_counts, dev_offsets: G^3 uint32 each;
+ * dev_perm: n uint32; any of the three may be NULL.  dev_scratch: >= soax_scratch_bytes(layout, n, G) bytes,
+ * 256-byte aligned.  Optional fusions (one call = config 5's whole pipeline): if drift_dt != 0 a DRIFT step
+ * with that dt is applied to src IN PLACE first, inside the same pass that computes the cell indices; if
+ * dev_kinetic != NULL it receives sum_i 0.5*|vel_i|^2 as in soax_reduce_energy(KINETIC).
+ * Errors: INVALID_ARG, UNSUPPORTED (no pos[3] double field, n >= 2^32), ALLOC (scratch too small), CUDA.
+ * Positions outside [0,1) are a precondition violation: their cell index is clamped into the grid. */
+size_t soax_scratch_bytes(const soax_layout* layout, int64_t n, int32_t grid_dim);
+int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
+                     uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
+                     size_t scratch_bytes, void* stream);
+
+/* ---- diagnostics ------------------------------------------------------------------------------------------ */
+const char* soax_strerror(int status);
+/* The cudaError_t (as int) of the last failed CUDA call made by this library on the calling thread, 0 if none. */
+int soax_last_cuda_error(void);
+/* Number of kernels this library has launched since load (or since the last soax_reset_launch_count). */
+int64_t soax_launch_count(void);
+void soax_reset_launch_count(void);
+/* Launch-shape knobs for benchmarking sweeps ("step_ppt", "step_block", "step_persist", ...); unknown keys
+ * return INVALID_ARG.  Not needed for normal use: defaults are the measured best. */
+int soax_tune(const char* key, int64_t value);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* SOAX_H */

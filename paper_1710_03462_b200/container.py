@@ -1,0 +1,153 @@
+"""Device plumbing around the C ABI: torch owns the device memory and the streams, the library does the work.
+
+`Soax` holds one torch uint8 slab carved by soax_alloc into per-component arrays and forwards
+every operation to the soax_* calls of binding.py.  Nothing here computes on particles.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+# layouts as (name, soax_dtype, dim) lists, declaration order (BASELINE.json config 4)
+R1 = (("id", B.SOAX_I32, 1), ("pos", B.SOAX_F64, 3), ("vel", B.SOAX_F32, 3))
+R2 = (("id", B.SOAX_I64, 1), ("pos", B.SOAX_F64, 3), ("vel", B.SOAX_F64, 3), ("acc", B.SOAX_F64, 3),
+      ("mass", B.SOAX_F32, 1), ("charge", B.SOAX_F32, 1), ("flags", B.SOAX_U8, 1))
+
+
+def B6(size_extra: int):
+    base = (("pos", B.SOAX_F32, 3), ("vel", B.SOAX_F32, 3))
+    return base if size_extra == 0 else base + (("temp", B.SOAX_F32, size_extra),)
+
+
+NP_DTYPE = {B.SOAX_I32: np.int32, B.SOAX_I64: np.int64, B.SOAX_U8: np.uint8, B.SOAX_F32: np.float32, B.SOAX_F64: np.float64}
+TORCH_DTYPE = {B.SOAX_I32: torch.int32, B.SOAX_I64: torch.int64, B.SOAX_U8: torch.uint8, B.SOAX_F32: torch.float32,
+               B.SOAX_F64: torch.float64}
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Soax:
+    """An SoA particle container on the current CUDA device (the paper's `Soax<ArrayTypes> soax(n)`)."""
+
+    def __init__(self, fields, n: int, capacity: int | None = None, device="cuda"):
+        self.fields = tuple(fields)
+        self.layout = B.soax_layout_define(self.fields)
+        self.capacity = n if capacity is None else capacity
+        self.slab_bytes = B.soax_slab_bytes(self.layout, self.capacity)
+        self.slab = torch.empty(self.slab_bytes, dtype=torch.uint8, device=device)
+        self.handle = B.soax_alloc(self.layout, n, self.capacity, self.slab.data_ptr(), self.slab_bytes)
+        self.ncomp = B.soax_layout_ncomp(self.layout)
+        self.comp_dtype = [B.soax_layout_comp(self.layout, c)[2] for c in range(self.ncomp)]
+        self._escratch = None
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h:
+            try:
+                B.soax_free(h)
+            except Exception:
+                pass
+
+    @property
+    def n(self) -> int:
+        return B.soax_size(self.handle)
+
+    # ---- views ---------------------------------------------------------------------------------------------
+    def field_index(self, name: str) -> int:
+        return [f[0] for f in self.fields].index(name)
+
+    def comp_view(self, field: str | int, comp: int = 0) -> torch.Tensor:
+        """torch view (no copy) of one component array: the paper's posArr(c)."""
+        f = self.field_index(field) if isinstance(field, str) else field
+        ptr = B.soax_field_ptr(self.handle, f, comp)
+        dt = self.fields[f][1]
+        off = ptr - self.slab.data_ptr()
+        return self.slab[off:off + self.n * B.DTYPE_SIZE[dt]].view(TORCH_DTYPE[dt])
+
+    # ---- host <-> device through the C ABI (end-to-end path) ---------------------------------------------------
+    def _host_ptrs(self, host: dict, writable: bool):
+        ptrs, keep = [], []
+        for name, dt, dim in self.fields:
+            a = host.get(name)
+            for c in range(dim):
+                if a is None:
+                    ptrs.append(None)
+                    continue
+                row = a[c]
+                if isinstance(row, torch.Tensor):
+                    assert row.is_contiguous() and row.dtype == TORCH_DTYPE[dt]
+                    ptrs.append(row.data_ptr())
+                else:
+                    assert row.flags["C_CONTIGUOUS"] and row.dtype == NP_DTYPE[dt] and (row.flags["WRITEABLE"] or not writable)
+                    ptrs.append(row.ctypes.data)
+                keep.append(row)
+        return ptrs, keep
+
+    def upload(self, host: dict, n: int | None = None) -> None:
+        """host: name -> (dim, N) numpy array or (pinned) torch CPU tensor, component-major."""
+        n = next(iter(host.values())).shape[1] if n is None else n
+        ptrs, keep = self._host_ptrs(host, writable=False)
+        B.soax_upload(self.handle, ptrs, n, _stream())
+        torch.cuda.current_stream().synchronize()      # pageable sources must outlive the copy
+        del keep
+
+    def download(self, into: dict | None = None) -> dict:
+        n = self.n
+        out = into if into is not None else {name: np.empty((dim, n), NP_DTYPE[dt]) for name, dt, dim in self.fields}
+        ptrs, keep = self._host_ptrs(out, writable=True)
+        B.soax_download(self.handle, ptrs, n, _stream())
+        torch.cuda.current_stream().synchronize()
+        del keep
+        return out
+
+    # ---- hot path ---------------------------------------------------------------------------------------------------
+    def step(self, kind: int, dt: float, nsteps: int = 1, k: float = 1.0, center: float = 0.5, flag_mask: int = 1) -> None:
+        B.soax_step(self.handle, B.step_params(kind, dt, k, center, flag_mask), nsteps, _stream())
+
+    def energy_async(self, kind: int, k: float = 1.0, center: float = 0.5, out: torch.Tensor | None = None) -> torch.Tensor:
+        if self._escratch is None:
+            self._escratch = torch.empty(B.soax_energy_scratch_bytes(), dtype=torch.uint8, device=self.slab.device)
+        out = torch.empty(1, dtype=torch.float64, device=self.slab.device) if out is None else out
+        B.soax_reduce_energy(self.handle, kind, k, center, self._escratch.data_ptr(), self._escratch.numel(),
+                             out.data_ptr(), _stream())
+        return out
+
+    def energy(self, kind: int, k: float = 1.0, center: float = 0.5) -> float:
+        return float(self.energy_async(kind, k, center).item())
+
+    def from_aos(self, aos: torch.Tensor, n: int) -> None:
+        B.soax_aos_to_soa(self.handle, aos.data_ptr(), n, _stream())
+
+    def to_aos(self, aos: torch.Tensor | None = None) -> torch.Tensor:
+        stride, _ = B.soax_layout_aos(self.layout, True)
+        n = self.n
+        aos = torch.empty(n * stride, dtype=torch.uint8, device=self.slab.device) if aos is None else aos
+        B.soax_soa_to_aos(self.handle, aos.data_ptr(), n, _stream())
+        return aos
+
+    def bin_permute(self, dst: "Soax", grid_dim: int, drift_dt: float = 0.0, want_kinetic: bool = False,
+                    scratch: torch.Tensor | None = None) -> dict:
+        """Returns device tensors: counts, offsets (uint32 as int32 views), perm, and kinetic (or None)."""
+        dev, n = self.slab.device, self.n
+        ncell = grid_dim ** 3
+        need = B.soax_scratch_bytes(self.layout, n, grid_dim)
+        if scratch is None:
+            scratch = torch.empty(need, dtype=torch.uint8, device=dev)
+        counts = torch.empty(ncell, dtype=torch.int32, device=dev)
+        offsets = torch.empty(ncell, dtype=torch.int32, device=dev)
+        perm = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+        kin = torch.empty(1, dtype=torch.float64, device=dev) if want_kinetic else None
+        B.soax_bin_permute(self.handle, dst.handle, grid_dim, drift_dt, counts.data_ptr(), offsets.data_ptr(),
+                           perm.data_ptr(), None if kin is None else kin.data_ptr(), scratch.data_ptr(), scratch.numel(),
+                           _stream())
+        return {"counts": counts, "offsets": offsets, "perm": perm[:n], "kinetic": kin, "scratch": scratch}
+
+
+def aos_step(fields, aos: torch.Tensor, n: int, kind: int, dt: float, nsteps: int = 1, variant: int = 0, k: float = 1.0,
+             center: float = 0.5) -> None:
+    layout = B.soax_layout_define(fields)
+    B.soax_step_aos(layout, aos.data_ptr(), n, B.step_params(kind, dt, k, center), nsteps, variant, _stream())

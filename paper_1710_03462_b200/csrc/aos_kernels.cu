@@ -1,0 +1,288 @@
+// aos_kernels.cu -- a5, a6, a7: everything that touches the Array-of-Structures image of a layout.
+//   * step_aos variant 0: the paper's AoS GPU kernel (K5): one thread per record, each field read
+//     and written in place with the stride of the record between neighbouring lanes (uncoalesced by design);
+//     it is the in-library baseline the SoA kernels are compared against (config 3).
+//   * step_aos variant 1: best effort on the same data: whole tiles of records are staged through shared memory
+//     with bulk asynchronous copies (TMA, UBLKCP), updated there, and written back in one piece.
+//   * aos_to_soa / soa_to_aos: the AoS side of a tile moves as ONE contiguous bulk copy global<->shared; the
+//     SoA side is read/written with fully coalesced per-component accesses.
+// The packed record (Q1) puts R1's doubles at offset 4 mod 8, so fields are accessed in pieces of the largest
+// power of two that divides both the stride and the field offset (4 bytes for R1, 1 byte for R2's 89-byte
+// record).
+#include "common.cuh"
+#include "ops.hpp"
+#include "tma.cuh"
+
+namespace soax {
+
+constexpr int cgcd(int a, int b) { return b == 0 ? a : cgcd(b, a % b); }
+
+// Load / store a T at an address whose alignment is only known to be A bytes (A a power of two <= 16).
+template <class T, int A>
+__device__ __forceinline__ T ld_piecewise(const unsigned char* p) {
+    if constexpr (A >= (int)sizeof(T)) {
+        return *reinterpret_cast<const T*>(p);
+    } else if constexpr (A >= 4) {
+        static_assert(sizeof(T) == 8, "only 8-byte types are split into words");
+        const uint32_t lo = *reinterpret_cast<const uint32_t*>(p), hi = *reinterpret_cast<const uint32_t*>(p + 4);
+        const unsigned long long u = ((unsigned long long)hi << 32) | lo;
+        T r;
+        memcpy(&r, &u, 8);
+        return r;
+    } else {
+        unsigned char b[sizeof(T)];
+#pragma unroll
+        for (int i = 0; i < (int)sizeof(T); ++i) b[i] = p[i];
+        T r;
+        memcpy(&r, b, sizeof(T));
+        return r;
+    }
+}
+template <class T, int A>
+__device__ __forceinline__ void st_piecewise(unsigned char* p, T v) {
+    if constexpr (A >= (int)sizeof(T)) {
+        *reinterpret_cast<T*>(p) = v;
+    } else if constexpr (A >= 4) {
+        unsigned long long u;
+        memcpy(&u, &v, 8);
+        *reinterpret_cast<uint32_t*>(p) = (uint32_t)u;
+        *reinterpret_cast<uint32_t*>(p + 4) = (uint32_t)(u >> 32);
+    } else {
+        unsigned char b[sizeof(T)];
+        memcpy(b, &v, sizeof(T));
+#pragma unroll
+        for (int i = 0; i < (int)sizeof(T); ++i) p[i] = b[i];
+    }
+}
+// alignment guaranteed for component C of a packed record whose array base is 16-byte aligned
+template <class L, int C>
+constexpr int comp_align() { return cgcd(16, cgcd(L::aos_stride, L::aos_offset(C))); }
+
+template <class L, class Tag>
+__device__ __forceinline__ typename L::template type_of<Tag> ld_field(const unsigned char* rec, int k) {
+    using T = typename L::template type_of<Tag>;
+    constexpr int c0 = L::template begin_of<Tag>;
+    constexpr int A = cgcd(16, cgcd(L::aos_stride, cgcd(L::aos_offset(c0), (int)sizeof(T))));
+    return ld_piecewise<T, A>(rec + L::aos_offset(c0) + k * (int)sizeof(T));
+}
+template <class L, class Tag>
+__device__ __forceinline__ void st_field(unsigned char* rec, int k, typename L::template type_of<Tag> v) {
+    using T = typename L::template type_of<Tag>;
+    constexpr int c0 = L::template begin_of<Tag>;
+    constexpr int A = cgcd(16, cgcd(L::aos_stride, cgcd(L::aos_offset(c0), (int)sizeof(T))));
+    st_piecewise<T, A>(rec + L::aos_offset(c0) + k * (int)sizeof(T), v);
+}
+
+// The update of ONE record held at `rec` (global or shared memory): same operation sequence as the SoA kernels.
+template <class L, int KIND>
+__device__ __forceinline__ void step_record(unsigned char* rec, double dt, double k, double ctr) {
+    using V = typename L::template type_of<vel_tag>;
+    const V dt_v = (V)dt;  // (float)dt rounds to nearest: dt_f of the contract
+    double x[3];
+    V v[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { x[d] = ld_field<L, pos_tag>(rec, d); v[d] = ld_field<L, vel_tag>(rec, d); }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        if constexpr (KIND == SOAX_STEP_SYMPLECTIC_EULER_HARMONIC) v[d] = kick1<V>(dt_v, k, ctr, x[d], v[d]);
+        x[d] = drift1<V>(dt, v[d], x[d]);
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        if constexpr (KIND == SOAX_STEP_SYMPLECTIC_EULER_HARMONIC) st_field<L, vel_tag>(rec, d, v[d]);
+        st_field<L, pos_tag>(rec, d, x[d]);
+    }
+}
+
+// ---- a5 variant 0: thread per record, strided access -------------------------------------------
+template <class L, int KIND>
+__global__ void __launch_bounds__(1024) step_aos_direct_kernel(unsigned char* aos, int64_t n, double dt, double k, double ctr) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) step_record<L, KIND>(aos + i * L::aos_stride, dt, k, ctr);
+}
+
+// ---- tile staging shared by variant 1 and the transposes -------------------------------------------------------
+constexpr int kTile = 256;  // records per tile = threads per CTA; kTile * stride is a multiple of 16 bytes
+
+// copy A bytes (A a power of two <= 16) between addresses aligned to A
+template <int A>
+__device__ __forceinline__ void copy_piece(unsigned char* dst, const unsigned char* src) {
+    if constexpr (A == 16) *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(src);
+    else if constexpr (A == 8) *reinterpret_cast<uint2*>(dst) = *reinterpret_cast<const uint2*>(src);
+    else if constexpr (A == 4) *reinterpret_cast<uint32_t*>(dst) = *reinterpret_cast<const uint32_t*>(src);
+    else if constexpr (A == 2) *reinterpret_cast<uint16_t*>(dst) = *reinterpret_cast<const uint16_t*>(src);
+    else *dst = *src;
+}
+
+// bring records [t0, t0 + cnt) into shared memory: one bulk copy for a full tile, piecewise copies for the tail
+template <class L>
+__device__ __forceinline__ void tile_load(unsigned char* sm, const unsigned char* aos, int64_t t0, int cnt, uint64_t* bar,
+                                          uint32_t& phase) {
+    constexpr int S = L::aos_stride;
+    if (cnt == kTile) {
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(bar, kTile * S);
+            bulk_g2s(sm, aos + t0 * S, kTile * S, bar);
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+    } else {
+        constexpr int A = cgcd(16, S);  // tail: copy in pieces the record size allows
+        const unsigned char* g = aos + t0 * S;
+        for (int o = threadIdx.x * A; o < cnt * S; o += blockDim.x * A) copy_piece<A>(sm + o, g + o);
+        __syncthreads();
+    }
+}
+// write records [t0, t0 + cnt) back from shared memory; all threads must have finished writing `sm`
+template <class L>
+__device__ __forceinline__ void tile_store(unsigned char* aos, const unsigned char* sm, int64_t t0, int cnt) {
+    constexpr int S = L::aos_stride;
+    if (cnt == kTile) {
+        fence_async_smem();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            bulk_s2g(aos + t0 * S, sm, kTile * S);
+            bulk_commit();
+            bulk_wait_read();  // the buffer is reused by the next tile
+        }
+        __syncthreads();
+    } else {
+        __syncthreads();
+        constexpr int A = cgcd(16, S);
+        unsigned char* g = aos + t0 * S;
+        for (int o = threadIdx.x * A; o < cnt * S; o += blockDim.x * A) copy_piece<A>(g + o, sm + o);
+        __syncthreads();
+    }
+}
+
+// ---- a5 variant 1: records staged through shared memory --------------------------------------------------------
+template <class L, int KIND>
+__global__ void __launch_bounds__(kTile) step_aos_staged_kernel(unsigned char* aos, int64_t n, double dt, double k, double ctr) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    __shared__ uint64_t bar;
+    if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+    __syncthreads();
+    uint32_t phase = 0;
+    const int64_t ntiles = (n + kTile - 1) / kTile;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t t0 = t * kTile;
+        const int cnt = (int)(n - t0 < kTile ? n - t0 : kTile);
+        tile_load<L>(sm, aos, t0, cnt, &bar, phase);
+        if ((int)threadIdx.x < cnt) step_record<L, KIND>(sm + threadIdx.x * L::aos_stride, dt, k, ctr);
+        tile_store<L>(aos, sm, t0, cnt);
+    }
+}
+
+// ---- a6: AoS -> SoA ----------------------------------------------------------------------------------------------
+template <class L>
+__global__ void __launch_bounds__(kTile) aos_to_soa_kernel(Ptrs<L::ncomp> a, const unsigned char* aos, int64_t n) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    __shared__ uint64_t bar;
+    if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+    __syncthreads();
+    uint32_t phase = 0;
+    const int64_t ntiles = (n + kTile - 1) / kTile;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t t0 = t * kTile;
+        const int cnt = (int)(n - t0 < kTile ? n - t0 : kTile);
+        tile_load<L>(sm, aos, t0, cnt, &bar, phase);
+        if ((int)threadIdx.x < cnt) {
+            const unsigned char* rec = sm + threadIdx.x * L::aos_stride;
+            for_each_comp<L>([&](auto ci) {
+                constexpr int C = decltype(ci)::value;
+                using T = typename L::template comp_type<C>;
+                comp_ptr<L, C>(a)[t0 + threadIdx.x] = ld_piecewise<T, comp_align<L, C>()>(rec + L::aos_offset(C));
+            });
+        }
+        __syncthreads();  // everyone is done reading before the next bulk copy overwrites the tile
+    }
+}
+
+// ---- a7: SoA -> AoS ----------------------------------------------------------------------------------------------
+template <class L>
+__global__ void __launch_bounds__(kTile) soa_to_aos_kernel(Ptrs<L::ncomp> a, unsigned char* aos, int64_t n) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    const int64_t ntiles = (n + kTile - 1) / kTile;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int64_t t0 = t * kTile;
+        const int cnt = (int)(n - t0 < kTile ? n - t0 : kTile);
+        if ((int)threadIdx.x < cnt) {
+            unsigned char* rec = sm + threadIdx.x * L::aos_stride;
+            for_each_comp<L>([&](auto ci) {
+                constexpr int C = decltype(ci)::value;
+                using T = typename L::template comp_type<C>;
+                st_piecewise<T, comp_align<L, C>()>(rec + L::aos_offset(C), comp_ptr<L, C>(a)[t0 + threadIdx.x]);
+            });
+        }
+        tile_store<L>(aos, sm, t0, cnt);
+    }
+}
+
+// ---- host side -----------------------------------------------------------------------------------------------------
+template <class L>
+static unsigned tile_grid(int64_t n, int ctas_per_sm) {
+    const int64_t ntiles = (n + kTile - 1) / kTile;
+    const int64_t cap = (int64_t)kSMs * ctas_per_sm;
+    return (unsigned)(ntiles < cap ? (ntiles < 1 ? 1 : ntiles) : cap);
+}
+template <class L>
+constexpr int tile_ctas_per_sm() {
+    constexpr int bytes = kTile * L::aos_stride + 64;
+    constexpr int by_smem = (200 * 1024) / bytes;
+    return by_smem < 8 ? (by_smem < 1 ? 1 : by_smem) : 8;  // 2048 threads / 256
+}
+
+template <class L, int KIND>
+static int step_aos_kind(void* aos, int64_t n, const soax_step_params* p, int variant, cudaStream_t st) {
+    constexpr bool ok = L::template has_as<pos_tag, double, 3>() &&
+                        (L::template has_as<vel_tag, float, 3>() || L::template has_as<vel_tag, double, 3>());
+    if constexpr (!ok) {
+        return SOAX_ERR_UNSUPPORTED;
+    } else {
+        unsigned char* base = static_cast<unsigned char*>(aos);
+        if (variant == 0) {
+            const int block = g_tune.aos_block;
+            step_aos_direct_kernel<L, KIND><<<(unsigned)((n + block - 1) / block), block, 0, st>>>(base, n, p->dt, p->k, p->center);
+        } else if (variant == 1) {
+            constexpr int smem = kTile * L::aos_stride;
+            step_aos_staged_kernel<L, KIND><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(base, n, p->dt, p->k, p->center);
+        } else {
+            return SOAX_ERR_INVALID_ARG;
+        }
+        return launched();
+    }
+}
+
+template <class L>
+int step_aos_entry(void* aos, int64_t n, const soax_step_params* p, int variant, cudaStream_t st) {
+    if (n == 0) return SOAX_OK;
+    switch (p->kind) {
+        case SOAX_STEP_DRIFT: return step_aos_kind<L, SOAX_STEP_DRIFT>(aos, n, p, variant, st);
+        case SOAX_STEP_SYMPLECTIC_EULER_HARMONIC: return step_aos_kind<L, SOAX_STEP_SYMPLECTIC_EULER_HARMONIC>(aos, n, p, variant, st);
+        case SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED:
+        case SOAX_STEP_EULER_NOWRAP: return SOAX_ERR_UNSUPPORTED;
+        default: return SOAX_ERR_INVALID_ARG;
+    }
+}
+
+template <class L>
+int aos_to_soa_entry(void* const* comps, const void* aos, int64_t n, cudaStream_t st) {
+    constexpr int smem = kTile * L::aos_stride;
+    aos_to_soa_kernel<L><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
+    return launched();
+}
+template <class L>
+int soa_to_aos_entry(void* const* comps, void* aos, int64_t n, cudaStream_t st) {
+    constexpr int smem = kTile * L::aos_stride;
+    soa_to_aos_kernel<L><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
+    return launched();
+}
+
+#define X(L)                                                                                         \
+    template int step_aos_entry<L>(void*, int64_t, const soax_step_params*, int, cudaStream_t);      \
+    template int aos_to_soa_entry<L>(void* const*, const void*, int64_t, cudaStream_t);              \
+    template int soa_to_aos_entry<L>(void* const*, void*, int64_t, cudaStream_t);
+SOAX_FOR_EACH_LAYOUT(X)
+#undef X
+
+}  // namespace soax

@@ -1,0 +1,283 @@
+// api.cu -- the C ABI of include/soax.h: layout registry, container handles, argument checking, dispatch.
+// Every step of the hot path runs in the kernels of the sibling .cu files; nothing here computes on the host.
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+#include "ops.hpp"
+
+namespace soax {
+std::atomic<int64_t> g_launches{0};
+thread_local int g_last_cuda_error = 0;
+Tuning g_tune;
+}  // namespace soax
+
+using namespace soax;
+
+// ---- run-time descriptor of one compiled layout (generated from the typelist) -------------------------------
+struct soax_layout {
+    const char* name;
+    int nfields, ncomp;
+    const char* fname[kMaxComp];
+    int fdtype[kMaxComp], fdim[kMaxComp], fbegin[kMaxComp];
+    int cfield[kMaxComp], cdtype[kMaxComp], csize[kMaxComp];
+    int (*step)(void* const*, int64_t, const soax_step_params*, cudaStream_t);
+    int (*step_aos)(void*, int64_t, const soax_step_params*, int, cudaStream_t);
+    int (*aos_to_soa)(void* const*, const void*, int64_t, cudaStream_t);
+    int (*soa_to_aos)(void* const*, void*, int64_t, cudaStream_t);
+    int (*energy)(void* const*, int64_t, int, double, double, void*, double*, cudaStream_t);
+    int (*bin_permute)(const BinArgs&, cudaStream_t);
+    size_t (*bin_scratch)(int64_t, int);
+};
+
+struct soax_container {
+    const soax_layout* layout;
+    int64_t n, capacity;
+    void* comp[kMaxComp];
+};
+
+namespace {
+
+template <class L>
+soax_layout describe(const char* name) {
+    soax_layout d{};
+    d.name = name;
+    d.nfields = L::nfields;
+    d.ncomp = L::ncomp;
+    for (int f = 0; f < L::nfields; ++f) {
+        d.fname[f] = L::field_name(f);
+        d.fdtype[f] = L::field_dtype(f);
+        d.fdim[f] = L::field_dim(f);
+        d.fbegin[f] = L::field_begin(f);
+    }
+    for (int c = 0; c < L::ncomp; ++c) {
+        d.cfield[c] = L::comp_field(c);
+        d.cdtype[c] = L::comp_dtype(c);
+        d.csize[c] = L::comp_size(c);
+    }
+    d.step = &step_entry<L>;
+    d.step_aos = &step_aos_entry<L>;
+    d.aos_to_soa = &aos_to_soa_entry<L>;
+    d.soa_to_aos = &soa_to_aos_entry<L>;
+    d.energy = &energy_entry<L>;
+    d.bin_permute = &bin_permute_entry<L>;
+    d.bin_scratch = &bin_scratch_bytes<L>;
+    return d;
+}
+
+const soax_layout* registry(int* count) {
+#define X(L) describe<L>(#L),
+    static const soax_layout table[] = {SOAX_FOR_EACH_LAYOUT(X)};
+#undef X
+    *count = (int)(sizeof(table) / sizeof(table[0]));
+    return table;
+}
+
+size_t carve(const soax_layout* l, int64_t cap, void* slab, void** comps) {
+    size_t off = 0;
+    for (int c = 0; c < l->ncomp; ++c) {
+        if (comps) comps[c] = static_cast<char*>(slab) + off;
+        off += align_up((size_t)cap * (size_t)l->csize[c], kAlign);
+    }
+    return off > 0 ? off : kAlign;
+}
+
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int ilog2_exact(int g) {
+    for (int b = 0; b <= 6; ++b) if ((1 << b) == g) return b;
+    return -1;
+}
+
+}  // namespace
+
+extern "C" {
+
+int soax_layout_define(const soax_field* fields, int32_t nfields, const soax_layout** out) {
+    if (!fields || !out || nfields <= 0 || nfields > kMaxComp) return SOAX_ERR_INVALID_ARG;
+    for (int f = 0; f < nfields; ++f)
+        if (!fields[f].name || fields[f].dim <= 0 || dtype_size(fields[f].dtype) == 0) return SOAX_ERR_INVALID_ARG;
+    int count = 0;
+    const soax_layout* table = registry(&count);
+    for (int i = 0; i < count; ++i) {
+        const soax_layout& l = table[i];
+        if (l.nfields != nfields) continue;
+        bool same = true;
+        for (int f = 0; f < nfields && same; ++f)
+            same = std::strcmp(l.fname[f], fields[f].name) == 0 && l.fdtype[f] == fields[f].dtype && l.fdim[f] == fields[f].dim;
+        if (same) { *out = &l; return SOAX_OK; }
+    }
+    return SOAX_ERR_UNKNOWN_LAYOUT;
+}
+
+int soax_layout_nfields(const soax_layout* l) { return l ? l->nfields : SOAX_ERR_INVALID_ARG; }
+int soax_layout_ncomp(const soax_layout* l) { return l ? l->ncomp : SOAX_ERR_INVALID_ARG; }
+
+int soax_layout_comp(const soax_layout* l, int32_t c, int32_t* field, int32_t* comp_in_field, int32_t* dtype) {
+    if (!l || c < 0 || c >= l->ncomp) return SOAX_ERR_INVALID_ARG;
+    if (field) *field = l->cfield[c];
+    if (comp_in_field) *comp_in_field = c - l->fbegin[l->cfield[c]];
+    if (dtype) *dtype = l->cdtype[c];
+    return SOAX_OK;
+}
+
+int soax_layout_aos(const soax_layout* l, int32_t packed, size_t* stride, size_t* comp_offsets) {
+    if (!l) return SOAX_ERR_INVALID_ARG;
+    size_t off = 0, maxal = 1;
+    for (int c = 0; c < l->ncomp; ++c) {
+        const size_t sz = (size_t)l->csize[c];
+        if (!packed) { off = align_up(off, sz); if (sz > maxal) maxal = sz; }
+        if (comp_offsets) comp_offsets[c] = off;
+        off += sz;
+    }
+    if (!packed) off = align_up(off, maxal);
+    if (stride) *stride = off;
+    return SOAX_OK;
+}
+
+size_t soax_slab_bytes(const soax_layout* l, int64_t capacity) {
+    if (!l || capacity < 0) return 0;
+    return carve(l, capacity, nullptr, nullptr);
+}
+
+int soax_alloc(const soax_layout* l, int64_t n, int64_t capacity, void* dev_slab, size_t slab_bytes, soax_t** out) {
+    if (!l || !out || n < 0 || capacity < n || !dev_slab || !aligned(dev_slab, kAlign)) return SOAX_ERR_INVALID_ARG;
+    if (slab_bytes < carve(l, capacity, nullptr, nullptr)) return SOAX_ERR_ALLOC;
+    soax_container* s = new (std::nothrow) soax_container();
+    if (!s) return SOAX_ERR_ALLOC;
+    s->layout = l;
+    s->n = n;
+    s->capacity = capacity;
+    carve(l, capacity, dev_slab, s->comp);
+    *out = s;
+    return SOAX_OK;
+}
+
+int soax_free(soax_t* s) {
+    if (!s) return SOAX_ERR_INVALID_ARG;
+    delete s;
+    return SOAX_OK;
+}
+
+int64_t soax_size(const soax_t* s) { return s ? s->n : (int64_t)SOAX_ERR_INVALID_ARG; }
+
+int soax_resize(soax_t* s, int64_t n) {
+    if (!s || n < 0 || n > s->capacity) return SOAX_ERR_INVALID_ARG;
+    s->n = n;
+    return SOAX_OK;
+}
+
+int soax_field_ptr(const soax_t* s, int32_t field, int32_t comp, void** dev_ptr) {
+    if (!s || !dev_ptr || field < 0 || field >= s->layout->nfields) return SOAX_ERR_INVALID_ARG;
+    if (comp < 0 || comp >= s->layout->fdim[field]) return SOAX_ERR_UNSUPPORTED;  // pos(42) on a 3-vector
+    *dev_ptr = s->comp[s->layout->fbegin[field] + comp];
+    return SOAX_OK;
+}
+
+int soax_upload(soax_t* s, const void* const* host_comps, int64_t n, void* stream) {
+    if (!s || !host_comps || n < 0 || n > s->capacity) return SOAX_ERR_INVALID_ARG;
+    for (int c = 0; c < s->layout->ncomp; ++c)
+        if (host_comps[c] && n > 0)
+            SOAX_CUDA(cudaMemcpyAsync(s->comp[c], host_comps[c], (size_t)n * s->layout->csize[c], cudaMemcpyHostToDevice,
+                                      (cudaStream_t)stream));
+    s->n = n;
+    return SOAX_OK;
+}
+
+int soax_download(const soax_t* s, void* const* host_comps, int64_t n, void* stream) {
+    if (!s || !host_comps || n < 0 || n > s->n) return SOAX_ERR_INVALID_ARG;
+    for (int c = 0; c < s->layout->ncomp; ++c)
+        if (host_comps[c] && n > 0)
+            SOAX_CUDA(cudaMemcpyAsync(host_comps[c], s->comp[c], (size_t)n * s->layout->csize[c], cudaMemcpyDeviceToHost,
+                                      (cudaStream_t)stream));
+    return SOAX_OK;
+}
+
+int soax_step(soax_t* s, const soax_step_params* p, int32_t nsteps, void* stream) {
+    if (!s || !p || nsteps < 0) return SOAX_ERR_INVALID_ARG;
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(s->layout->step(s->comp, s->n, p, (cudaStream_t)stream));
+    return SOAX_OK;
+}
+
+int soax_step_aos(const soax_layout* l, void* dev_aos, int64_t n, const soax_step_params* p, int32_t nsteps,
+                  int32_t variant, void* stream) {
+    if (!l || !p || nsteps < 0 || n < 0 || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(l->step_aos(dev_aos, n, p, variant, (cudaStream_t)stream));
+    return SOAX_OK;
+}
+
+int soax_aos_to_soa(soax_t* dst, const void* dev_aos, int64_t n, void* stream) {
+    if (!dst || n < 0 || n > dst->capacity || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    dst->n = n;
+    return n == 0 ? SOAX_OK : dst->layout->aos_to_soa(dst->comp, dev_aos, n, (cudaStream_t)stream);
+}
+
+int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream) {
+    if (!src || n < 0 || n > src->n || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    return n == 0 ? SOAX_OK : src->layout->soa_to_aos(const_cast<void* const*>(src->comp), dev_aos, n, (cudaStream_t)stream);
+}
+
+size_t soax_energy_scratch_bytes(void) { return kEnergyScratchBytes; }
+
+int soax_reduce_energy(const soax_t* s, int32_t kind, double k, double center, void* dev_scratch, size_t scratch_bytes,
+                       double* dev_out, void* stream) {
+    if (!s || !dev_scratch || !dev_out || !aligned(dev_scratch, 8) || !aligned(dev_out, 8)) return SOAX_ERR_INVALID_ARG;
+    if (scratch_bytes < kEnergyScratchBytes) return SOAX_ERR_ALLOC;
+    return s->layout->energy(const_cast<void* const*>(s->comp), s->n, kind, k, center, dev_scratch, dev_out,
+                             (cudaStream_t)stream);
+}
+
+size_t soax_scratch_bytes(const soax_layout* l, int64_t n, int32_t grid_dim) {
+    if (!l || n < 0 || ilog2_exact(grid_dim) < 0) return 0;
+    return l->bin_scratch(n, ilog2_exact(grid_dim));
+}
+
+int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
+                     uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
+                     size_t scratch_bytes, void* stream) {
+    if (!src || !dst || src == dst || src->layout != dst->layout || !dev_scratch || !aligned(dev_scratch, kAlign))
+        return SOAX_ERR_INVALID_ARG;
+    const int log2g = ilog2_exact(grid_dim);
+    if (log2g < 0 || dst->capacity < src->n) return SOAX_ERR_INVALID_ARG;
+    for (int c = 0; c < src->layout->ncomp; ++c)
+        if (src->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
+    if (src->n >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
+    const size_t need = src->layout->bin_scratch(src->n, log2g);
+    if (need == 0) return SOAX_ERR_UNSUPPORTED;
+    if (scratch_bytes < need) return SOAX_ERR_ALLOC;
+    BinArgs a{src->comp, dst->comp, src->n, log2g, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
+              dev_scratch, scratch_bytes};
+    dst->n = src->n;
+    return src->layout->bin_permute(a, (cudaStream_t)stream);
+}
+
+const char* soax_strerror(int status) {
+    switch (status) {
+        case SOAX_OK: return "ok";
+        case SOAX_ERR_INVALID_ARG: return "invalid argument";
+        case SOAX_ERR_UNKNOWN_LAYOUT: return "field list matches no compiled layout";
+        case SOAX_ERR_UNSUPPORTED: return "operation not supported by this layout (missing field, wrong type or dimension)";
+        case SOAX_ERR_ALLOC: return "buffer too small or host allocation failed";
+        case SOAX_ERR_CUDA: return "CUDA runtime error (see soax_last_cuda_error)";
+        default: return "unknown status";
+    }
+}
+
+int soax_last_cuda_error(void) { return g_last_cuda_error; }
+int64_t soax_launch_count(void) { return g_launches.load(); }
+void soax_reset_launch_count(void) { g_launches.store(0); }
+
+int soax_tune(const char* key, int64_t value) {
+    if (!key) return SOAX_ERR_INVALID_ARG;
+    const int v = (int)value;
+    if (!std::strcmp(key, "step_ppt")) { if (v != 1 && v != 2 && v != 4) return SOAX_ERR_INVALID_ARG; g_tune.step_ppt = v; }
+    else if (!std::strcmp(key, "step_block")) { if (v < 32 || v > 512 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.step_block = v; }
+    else if (!std::strcmp(key, "step_persist")) { if (v < 0 || v > 64) return SOAX_ERR_INVALID_ARG; g_tune.step_persist = v; }
+    else if (!std::strcmp(key, "aos_block")) { if (v < 32 || v > 1024 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.aos_block = v; }
+    else if (!std::strcmp(key, "bin_stage")) { if (v < 0 || v > 1) return SOAX_ERR_INVALID_ARG; g_tune.bin_stage = v; }
+    else return SOAX_ERR_INVALID_ARG;
+    return SOAX_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,367 @@
+// bin_kernels.cu -- a10..a14: PIC-style cell binning with a STABLE counting-sort permutation of every field
+// array (BASELINE.json config 5).
+//
+// Design: the 18-bit cell key is sorted by a two-pass least-significant-digit counting
+// sort with 9-bit digits (512 bins per pass), and the WHOLE RECORD travels with its key through both passes
+// together with its source index, so `perm` falls out as the carried index and no random gather of the field
+// arrays is ever made (a per-array gather would read one 32-byte sector per 4- or 8-byte item).  Each pass:
+//   tile_hist   per-tile digit histogram (tiles of kTileN consecutive particles)            4 B/particle read
+//   colscan_*   exclusive scan of the [tile][digit] table in digit-major order              (small)
+//   scatter     stable in-tile ranks (warp match + per-warp running counters), then every component array is
+//               moved src[i] -> dst[base[tile][digit] + rank]
+// Every step is a pure function of the data (no arrival-order atomics decide a position), so the result is the
+// unique stable permutation for ANY particle distribution, and bit-identical from run to run.
+// counts / offsets come from the sorted keys by boundary detection.
+#include "common.cuh"
+#include "ops.hpp"
+
+namespace soax {
+
+int sum_partials(const double* partial, int m, double* out, cudaStream_t st);  // reduce_kernels.cu
+
+constexpr int kRadixBits = 9;
+constexpr int kRadix = 1 << kRadixBits;        // 512 bins per pass
+constexpr int kSortThreads = 512;              // 16 warps
+constexpr int kItems = 8;                      // keys per thread
+constexpr int kTileN = kSortThreads * kItems;  // 4096 particles per tile
+constexpr int kWarps = kSortThreads / 32;
+constexpr int kScanRows = 64;                  // tiles per column-scan chunk
+
+// ---- pass 0: [drift +] cell index [+ kinetic energy], P = 4 particles per thread, fixed grid -------------------
+template <class L, bool DRIFT, bool KE, int P>
+__device__ __forceinline__ double cell_group(const Ptrs<L::ncomp>& a, int64_t i0, uint32_t* cell, double dt, double G,
+                                             int gmax, int log2g) {
+    using V = typename L::template type_of<vel_tag>;
+    Vec<double, P> x[3];
+    Vec<V, P> v[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) x[d] = ld_vec<double, P>(field_ptr<L, pos_tag>(a, d) + i0);
+    if constexpr (DRIFT || KE) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) v[d] = ld_vec<V, P>(field_ptr<L, vel_tag>(a, d) + i0);
+    }
+    if constexpr (DRIFT) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+#pragma unroll
+            for (int j = 0; j < P; ++j) x[d].v[j] = drift1<V>(dt, v[d].v[j], x[d].v[j]);
+            st_vec<double, P>(field_ptr<L, pos_tag>(a, d) + i0, x[d]);
+        }
+    }
+    Vec<uint32_t, P> c;
+    double e = 0.0;
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        c.v[j] = cell_of(x[0].v[j], x[1].v[j], x[2].v[j], G, gmax, log2g);
+        if constexpr (KE)
+            e += energy1<false>((double)v[0].v[j], (double)v[1].v[j], (double)v[2].v[j], 0.0, 0.0, 0.0, 0.0, 0.0);
+    }
+    st_vec<uint32_t, P>(cell + i0, c);
+    return e;
+}
+
+template <class L, bool DRIFT, bool KE>
+__global__ void __launch_bounds__(256) cell_kernel(Ptrs<L::ncomp> a, int64_t n, uint32_t* cell, double dt, int log2g,
+                                                   double* ke_partial) {
+    constexpr int P = 4;
+    __shared__ double sm[32];
+    const double G = (double)(1 << log2g);
+    const int gmax = (1 << log2g) - 1;
+    const int64_t ngroups = n / P;
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double e = 0.0;
+    for (int64_t g = tid; g < ngroups; g += stride) e += cell_group<L, DRIFT, KE, P>(a, g * P, cell, dt, G, gmax, log2g);
+    const int64_t t = ngroups * P + tid;
+    if (t < n) e += cell_group<L, DRIFT, KE, 1>(a, t, cell, dt, G, gmax, log2g);
+    if constexpr (KE) {
+        e = block_sum(e, sm);
+        if (threadIdx.x == 0) ke_partial[blockIdx.x] = e;
+    }
+}
+
+// ---- per-tile digit histogram -------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t* __restrict__ keys, int64_t n, int shift,
+                                                                 uint32_t* __restrict__ hist) {
+    __shared__ uint32_t h[kRadix];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t tile0 = (int64_t)blockIdx.x * kTileN;
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int64_t e = tile0 + k * kSortThreads + threadIdx.x;
+        if (e < n) atomicAdd(&h[(keys[e] >> shift) & (kRadix - 1)], 1u);
+    }
+    __syncthreads();
+    hist[(int64_t)blockIdx.x * kRadix + threadIdx.x] = h[threadIdx.x];
+}
+
+// ---- exclusive scan of hist[tile][digit] in (digit-major, tile-minor) order ----------------------------------------
+// phase 1: column sums of each chunk of kScanRows tiles
+__global__ void __launch_bounds__(kRadix) colscan_reduce_kernel(const uint32_t* __restrict__ hist, int ntiles,
+                                                                uint32_t* __restrict__ partial) {
+    const int r0 = blockIdx.x * kScanRows, r1 = min(r0 + kScanRows, ntiles);
+    uint32_t s = 0;
+    for (int r = r0; r < r1; ++r) s += hist[(int64_t)r * kRadix + threadIdx.x];
+    partial[(int64_t)blockIdx.x * kRadix + threadIdx.x] = s;
+}
+// exclusive scan of one value per thread over a CTA of kRadix threads
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t x, uint32_t* sm /* >= 32 */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += y;
+    }
+    if (lane == 31) sm[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = lane < (int)(blockDim.x >> 5) ? sm[lane] : 0, winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += y;
+        }
+        sm[lane] = winc - w;
+    }
+    __syncthreads();
+    return inc - x + sm[warp];
+}
+// phase 2 (one CTA): per digit, exclusive scan of the chunk sums over chunks; then exclusive scan of the digit
+// totals over digits -> dbase[digit]
+__global__ void __launch_bounds__(kRadix) colscan_top_kernel(uint32_t* __restrict__ partial, int nchunks,
+                                                             uint32_t* __restrict__ dbase) {
+    __shared__ uint32_t sm[32];
+    uint32_t run = 0;
+    for (int c = 0; c < nchunks; ++c) {
+        const uint32_t v = partial[(int64_t)c * kRadix + threadIdx.x];
+        partial[(int64_t)c * kRadix + threadIdx.x] = run;
+        run += v;
+    }
+    dbase[threadIdx.x] = block_excl_scan(run, sm);
+}
+// phase 3: hist[tile][digit] <- global offset of the first item of (digit, tile)
+__global__ void __launch_bounds__(kRadix) colscan_apply_kernel(uint32_t* __restrict__ hist, int ntiles,
+                                                               const uint32_t* __restrict__ partial,
+                                                               const uint32_t* __restrict__ dbase) {
+    const int r0 = blockIdx.x * kScanRows, r1 = min(r0 + kScanRows, ntiles);
+    uint32_t run = dbase[threadIdx.x] + partial[(int64_t)blockIdx.x * kRadix + threadIdx.x];
+    for (int r = r0; r < r1; ++r) {
+        const uint32_t v = hist[(int64_t)r * kRadix + threadIdx.x];
+        hist[(int64_t)r * kRadix + threadIdx.x] = run;
+        run += v;
+    }
+}
+
+// ---- stable scatter of one tile: keys, source indices and EVERY component array ------------------------------------
+template <class L>
+__global__ void __launch_bounds__(kSortThreads) scatter_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst,
+                                                               const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
+                                                               const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ idx_out,
+                                                               const uint32_t* __restrict__ base, int64_t n, int shift) {
+    __shared__ uint32_t wcnt[kWarps * kRadix];  // per-warp running digit counters, then per-warp global bases
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
+    __syncthreads();
+
+    // warp w owns the 32*kItems consecutive particles starting at tile0 + w*32*kItems; round k covers 32 of them
+    const int64_t e0 = (int64_t)blockIdx.x * kTileN + warp * (32 * kItems) + lane;
+    uint32_t key[kItems], dest[kItems];
+    uint32_t* mycnt = wcnt + warp * kRadix;
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int64_t e = e0 + k * 32;
+        const bool valid = e < n;
+        key[k] = valid ? key_in[e] : 0u;
+        const uint32_t d = (key[k] >> shift) & (kRadix - 1);
+        const uint32_t peers = __match_any_sync(0xffffffffu, valid ? d : (0x10000u | lane));
+        const uint32_t old = mycnt[d];
+        dest[k] = old + __popc(peers & lt);  // rank among the warp's earlier particles with this digit
+        __syncwarp();
+        if (valid && lane == 31 - __clz(peers)) mycnt[d] = old + __popc(peers);
+        __syncwarp();
+    }
+    __syncthreads();
+    // digit d (one thread each): turn the per-warp counts into global bases, warps in order
+    {
+        uint32_t run = base[(int64_t)blockIdx.x * kRadix + threadIdx.x];
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            const uint32_t c = wcnt[w * kRadix + threadIdx.x];
+            wcnt[w * kRadix + threadIdx.x] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) dest[k] += mycnt[(key[k] >> shift) & (kRadix - 1)];
+
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int64_t e = e0 + k * 32;
+        if (e < n) {
+            key_out[dest[k]] = key[k];
+            idx_out[dest[k]] = idx_in ? idx_in[e] : (uint32_t)e;
+        }
+    }
+    for_each_comp<L>([&](auto ci) {
+        constexpr int C = decltype(ci)::value;
+        using T = typename L::template comp_type<C>;
+        const T* s = comp_ptr<L, C>(src);
+        T* t = comp_ptr<L, C>(dst);
+        T val[kItems];
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int64_t e = e0 + k * 32;
+            if (e < n) val[k] = s[e];
+        }
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int64_t e = e0 + k * 32;
+            if (e < n) t[dest[k]] = val[k];
+        }
+    });
+}
+
+// ---- counts / offsets from the sorted keys --------------------------------------------------------------------------
+// off[c] = first sorted slot whose key is >= c, for c = 0..ncell (off[ncell] = n)
+__global__ void __launch_bounds__(256) boundaries_kernel(const uint32_t* __restrict__ sorted, int64_t n, uint32_t ncell,
+                                                         uint32_t* __restrict__ off) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+        const uint32_t cur = sorted[j];
+        const uint32_t first = j == 0 ? 0u : sorted[j - 1] + 1u;
+        for (uint32_t c = first; c <= cur; ++c) off[c] = (uint32_t)j;
+        if (j == n - 1)
+            for (uint32_t c = cur + 1; c <= ncell; ++c) off[c] = (uint32_t)n;
+    }
+}
+__global__ void __launch_bounds__(256) counts_kernel(const uint32_t* __restrict__ off, uint32_t ncell, uint32_t* counts,
+                                                     uint32_t* offsets) {
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < ncell) {
+        if (counts) counts[c] = off[c + 1] - off[c];
+        if (offsets) offsets[c] = off[c];
+    }
+}
+
+// ---- host side: scratch plan and the pipeline -------------------------------------------------------------------------
+template <class L>
+struct BinPlan {
+    size_t key0, key1, idx1, idx2, slab, hist, partial, dbase, off, ke, total;
+    int64_t ntiles, nchunks;
+    size_t comp_off[L::ncomp];
+    BinPlan(int64_t n, int log2g) {
+        ntiles = (n + kTileN - 1) / kTileN;
+        if (ntiles < 1) ntiles = 1;
+        nchunks = (ntiles + kScanRows - 1) / kScanRows;
+        const size_t ncell = (size_t)1 << (3 * log2g);
+        size_t o = 0;
+        auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1, kAlign); return at; };
+        key0 = take((size_t)n * 4);
+        key1 = take((size_t)n * 4);
+        idx1 = take((size_t)n * 4);
+        idx2 = take((size_t)n * 4);
+        slab = o;
+        for (int c = 0; c < L::ncomp; ++c) comp_off[c] = take((size_t)n * L::comp_size(c));
+        hist = take((size_t)ntiles * kRadix * 4);
+        partial = take((size_t)nchunks * kRadix * 4);
+        dbase = take(kRadix * 4);
+        off = take((ncell + 1) * 4);
+        ke = take(kEnergyScratchBytes);
+        total = o;
+    }
+};
+
+template <class L>
+size_t bin_scratch_bytes(int64_t n, int log2g) {
+    if constexpr (!L::template has_as<pos_tag, double, 3>()) return 0;
+    else return BinPlan<L>(n, log2g).total;
+}
+
+template <class L>
+int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
+    constexpr bool has_pos = L::template has_as<pos_tag, double, 3>();
+    constexpr bool has_vel = L::template has_as<vel_tag, float, 3>() || L::template has_as<vel_tag, double, 3>();
+    if constexpr (!has_pos) {
+        return SOAX_ERR_UNSUPPORTED;
+    } else {
+        const int64_t n = a.n;
+        const uint32_t ncell = 1u << (3 * a.log2g);
+        const bool drift = a.drift_dt != 0.0, ke = a.kinetic != nullptr;
+        if ((drift || ke) && !has_vel) return SOAX_ERR_UNSUPPORTED;
+        if (n == 0) {
+            if (a.counts) SOAX_CUDA(cudaMemsetAsync(a.counts, 0, (size_t)ncell * 4, st));
+            if (a.offsets) SOAX_CUDA(cudaMemsetAsync(a.offsets, 0, (size_t)ncell * 4, st));
+            if (ke) SOAX_CUDA(cudaMemsetAsync(a.kinetic, 0, sizeof(double), st));
+            return SOAX_OK;
+        }
+        const BinPlan<L> plan(n, a.log2g);
+        char* sc = static_cast<char*>(a.scratch);
+        uint32_t* key0 = reinterpret_cast<uint32_t*>(sc + plan.key0);
+        uint32_t* key1 = reinterpret_cast<uint32_t*>(sc + plan.key1);
+        uint32_t* idx1 = reinterpret_cast<uint32_t*>(sc + plan.idx1);
+        uint32_t* idx2 = a.perm ? a.perm : reinterpret_cast<uint32_t*>(sc + plan.idx2);
+        uint32_t* hist = reinterpret_cast<uint32_t*>(sc + plan.hist);
+        uint32_t* partial = reinterpret_cast<uint32_t*>(sc + plan.partial);
+        uint32_t* dbase = reinterpret_cast<uint32_t*>(sc + plan.dbase);
+        uint32_t* off = reinterpret_cast<uint32_t*>(sc + plan.off);
+        double* kep = reinterpret_cast<double*>(sc + plan.ke);
+        const Ptrs<L::ncomp> src = make_ptrs<L>(a.src), dst = make_ptrs<L>(a.dst);
+        Ptrs<L::ncomp> tmp;
+        for (int c = 0; c < L::ncomp; ++c) tmp.p[c] = sc + plan.comp_off[c];
+
+        // pass 0: [drift +] cell index [+ KE]
+        if constexpr (has_vel) {
+            if (drift && ke) cell_kernel<L, true, true><<<kEnergyBlocks, 256, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, kep);
+            else if (drift) cell_kernel<L, true, false><<<kEnergyBlocks, 256, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, kep);
+            else if (ke) cell_kernel<L, false, true><<<kEnergyBlocks, 256, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, kep);
+            else cell_kernel<L, false, false><<<kEnergyBlocks, 256, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, kep);
+        } else {
+            cell_kernel<L, false, false><<<kEnergyBlocks, 256, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, kep);
+        }
+        SOAX_TRY(launched());
+        if (ke) SOAX_TRY(sum_partials(kep, kEnergyBlocks, a.kinetic, st));
+
+        const int npass = 3 * a.log2g > kRadixBits ? 2 : 1;
+        const unsigned ntiles = (unsigned)plan.ntiles, nchunks = (unsigned)plan.nchunks;
+        for (int pass = 0; pass < npass; ++pass) {
+            const bool last = pass == npass - 1;
+            const uint32_t* kin = pass == 0 ? key0 : key1;
+            uint32_t* kout = pass == 0 ? key1 : key0;  // sorted keys end in key1 (1 pass) or key0 (2 passes)
+            const uint32_t* iin = pass == 0 ? nullptr : idx1;
+            uint32_t* iout = last ? idx2 : idx1;
+            const Ptrs<L::ncomp>& from = pass == 0 ? src : tmp;
+            const Ptrs<L::ncomp>& to = last ? dst : tmp;
+            const int shift = pass * kRadixBits;
+            tile_hist_kernel<<<ntiles, kSortThreads, 0, st>>>(kin, n, shift, hist);
+            SOAX_TRY(launched());
+            colscan_reduce_kernel<<<nchunks, kRadix, 0, st>>>(hist, (int)ntiles, partial);
+            SOAX_TRY(launched());
+            colscan_top_kernel<<<1, kRadix, 0, st>>>(partial, (int)nchunks, dbase);
+            SOAX_TRY(launched());
+            colscan_apply_kernel<<<nchunks, kRadix, 0, st>>>(hist, (int)ntiles, partial, dbase);
+            SOAX_TRY(launched());
+            scatter_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+            SOAX_TRY(launched());
+        }
+        if (a.counts || a.offsets) {
+            const uint32_t* sorted = npass == 1 ? key1 : key0;
+            boundaries_kernel<<<kSMs * 8, 256, 0, st>>>(sorted, n, ncell, off);
+            SOAX_TRY(launched());
+            counts_kernel<<<(ncell + 255) / 256, 256, 0, st>>>(off, ncell, a.counts, a.offsets);
+            SOAX_TRY(launched());
+        }
+        return SOAX_OK;
+    }
+}
+
+#define X(L)                                                               \
+    template int bin_permute_entry<L>(const BinArgs&, cudaStream_t);      \
+    template size_t bin_scratch_bytes<L>(int64_t, int);
+SOAX_FOR_EACH_LAYOUT(X)
+#undef X
+
+}  // namespace soax

@@ -1,0 +1,53 @@
+// ops.hpp -- per-layout entry points.  Each family lives in its own .cu, is a template over the layout and is
+// explicitly instantiated for every layout of SOAX_FOR_EACH_LAYOUT; registry.cu stores the instantiations'
+// addresses in the layout descriptor ("a field-descriptor and layout registry that generates per-layout CUDA
+// kernels from C++ templates").
+#pragma once
+#include <cuda_runtime.h>
+
+#include "layout.hpp"
+
+// The layouts compiled into the library.  Adding a layout = one line here (and a `using` in layout.hpp).
+#define SOAX_FOR_EACH_LAYOUT(X) X(R1) X(R2) X(B6<0>) X(B6<8>) X(B6<16>) X(B6<32>)
+
+namespace soax {
+
+// Launch-shape knobs (soax_tune).  Defaults are the measured best on B200 (profiles/).
+struct Tuning {
+    int step_ppt = 4;       // particles per thread in the SoA step kernels: 1, 2 or 4
+    int step_block = 256;   // threads per CTA
+    int step_persist = 0;   // 0: one CTA per tile of work; k > 0: persistent grid of k CTAs per SM
+    int aos_block = 256;
+    int xpose_tile = 512;   // records per transpose tile
+    int bin_stage = 1;      // 1: shared-memory staged (coalesced) scatter, 0: direct scatter
+};
+extern Tuning g_tune;
+
+template <class L> int step_entry(void* const* comps, int64_t n, const soax_step_params* p, cudaStream_t st);
+template <class L> int step_aos_entry(void* aos, int64_t n, const soax_step_params* p, int variant, cudaStream_t st);
+template <class L> int aos_to_soa_entry(void* const* comps, const void* aos, int64_t n, cudaStream_t st);
+template <class L> int soa_to_aos_entry(void* const* comps, void* aos, int64_t n, cudaStream_t st);
+template <class L> int energy_entry(void* const* comps, int64_t n, int kind, double k, double ctr, void* scratch,
+                                    double* out, cudaStream_t st);
+struct BinArgs {
+    void* const* src; void* const* dst; int64_t n; int log2g; double drift_dt;
+    uint32_t* counts; uint32_t* offsets; uint32_t* perm; double* kinetic;
+    void* scratch; size_t scratch_bytes;
+};
+template <class L> int bin_permute_entry(const BinArgs& a, cudaStream_t st);
+template <class L> size_t bin_scratch_bytes(int64_t n, int log2g);
+
+constexpr int kEnergyBlocks = 1184;  // 148 SMs x 8 CTAs: fixed, so the reduction tree is fixed
+constexpr size_t kEnergyScratchBytes = (size_t)kEnergyBlocks * sizeof(double);
+
+template <class L> inline Ptrs<L::ncomp> make_ptrs(void* const* comps) {
+    Ptrs<L::ncomp> a;
+    for (int c = 0; c < L::ncomp; ++c) a.p[c] = comps[c];
+    return a;
+}
+
+// byte size of the slab for `cap` particles: every component array starts on a 256-byte boundary
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace soax

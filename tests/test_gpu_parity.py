@@ -1,0 +1,334 @@
+"""GPU parity: the CUDA path (through the C ABI, libsoax.so) against the oracle, element by element, on the same
+seeded inputs.  Sizes span several tiles (4 particles/thread x 256 threads; 256-record transpose tiles; 4096-key
+sort tiles) plus a ragged tail.  Bars (BASELINE.json north_star): ids / counts / offsets / perm bit-exact; double
+positions within 1e-12 absolute (periodic distance); float velocities within 4 ulp; energy within 1e-10 relative.
+Because both sides run the same IEEE operation sequence (explicit fma, no contraction) the EXPECTATION is
+bit-equality, which the tests also assert where the arithmetic contract promises it.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1710_03462_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+DT = 1e-3
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_1710_03462_b200 import binding as B, container as Cn
+    B.lib()                                     # fail loudly if libsoax.so is missing: there is no fallback
+    return torch, B, Cn
+
+
+def bits(a):
+    a = np.ascontiguousarray(a)
+    return a.view({4: np.uint32, 8: np.uint64, 1: np.uint8}[a.dtype.itemsize])
+
+
+def pdist(a, b):
+    d = np.abs(np.asarray(a, np.float64) - np.asarray(b, np.float64))
+    return np.minimum(d, 1.0 - d)
+
+
+def ulp_dist32(a, b):
+    """distance in units in the last place between float32 arrays (sign-magnitude -> ordered integers)"""
+    def ordered(x):
+        i = np.ascontiguousarray(x).view(np.int32).astype(np.int64)
+        return np.where(i < 0, -(i & 0x7FFFFFFF), i)
+    return np.abs(ordered(a) - ordered(b))
+
+
+def check_r1(got, exp, expect_bits=True):
+    assert np.array_equal(got["id"], exp["id"])
+    assert pdist(got["pos"], exp["pos"]).max() <= 1e-12
+    assert ulp_dist32(got["vel"], exp["vel"]).max() <= 4
+    assert (got["pos"] >= 0).all() and (got["pos"] < 1).all()
+    if expect_bits:
+        assert np.array_equal(bits(got["pos"]), bits(exp["pos"])), "positions differ in some bit"
+        assert np.array_equal(bits(got["vel"]), bits(exp["vel"])), "velocities differ in some bit"
+
+
+def to_device(Cn, fields, host):
+    n = next(iter(host.values())).shape[1]
+    s = Cn.Soax(fields, n)
+    s.upload(host)
+    return s
+
+
+# ------------------------------------------------------------------------------------------ a2: drift (config 1)
+@pytest.mark.parametrize("n", [65536, 4099, 3, 1, 0])
+@pytest.mark.parametrize("ppt", [4, 2, 1])
+def test_drift_config1(gpu, n, ppt):
+    torch, B, Cn = gpu
+    B.soax_tune("step_ppt", ppt)
+    try:
+        host = inputs.make_r1(n, seed=0)
+        s = to_device(Cn, Cn.R1, host)
+        s.step(B.SOAX_STEP_DRIFT, DT, nsteps=10)
+        got = s.download()
+    finally:
+        B.soax_tune("step_ppt", 4)
+    exp = oracle.drift(host, DT, 10) if n else host
+    if n:
+        check_r1(got, exp)
+        assert np.array_equal(bits(got["vel"]), bits(host["vel"]))        # vel untouched
+
+
+def test_drift_face_crossings_and_special_values(gpu):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(1000, seed=5)
+    host["vel"] *= np.float32(400.0)                                  # |dt v| up to ~2: wraps, incl. the slow floor path
+    host["pos"][0, :8] = [0.0, 0.999, 0.001, 1.0 - 2.0 ** -53, 0.0, 0.5, 0.0, 2.0 ** -1074]
+    host["vel"][0, :8] = [-1e-17, 2.0, -2.0, 1e-20, -0.0, 3000.0, -2500.0, -1e-30]
+    s = to_device(Cn, Cn.R1, host)
+    s.step(B.SOAX_STEP_DRIFT, DT, nsteps=3)
+    check_r1(s.download(), oracle.drift(host, DT, 3))
+
+
+# ------------------------------------------------------------------------- a4 + a8: symplectic Euler (config 2)
+@pytest.mark.parametrize("n,nsteps", [(1 << 16, 100), (10007, 7)])
+def test_symplectic_euler_and_energy(gpu, n, nsteps):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(n, seed=0)
+    s = to_device(Cn, Cn.R1, host)
+    e0 = s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC)
+    s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=nsteps)
+    e1 = s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC)
+    ke1 = s.energy(B.SOAX_ENERGY_KINETIC)
+    got = s.download()
+    exp = oracle.symplectic_euler(host, DT, nsteps)
+    check_r1(got, exp)
+    o0 = oracle.energy(host, oracle.KINETIC_PLUS_HARMONIC)
+    o1 = oracle.energy(exp, oracle.KINETIC_PLUS_HARMONIC)
+    assert abs(e0 - o0) <= 1e-10 * abs(o0) and abs(e1 - o1) <= 1e-10 * abs(o1)
+    assert abs(ke1 - oracle.energy(exp, oracle.KINETIC)) <= 1e-10 * abs(ke1)
+    assert s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC) == e1          # run-to-run deterministic
+
+
+def test_symplectic_euler_general_k_and_center(gpu):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(5000, seed=3)
+    s = to_device(Cn, Cn.R1, host)
+    s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=5, k=2.5, center=0.25)
+    check_r1(s.download(), oracle.symplectic_euler(host, DT, 5, k=2.5, center=0.25))
+    e = s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, k=2.5, center=0.25)
+    o = oracle.energy(s.download(), oracle.KINETIC_PLUS_HARMONIC, k=2.5, center=0.25)
+    assert abs(e - o) <= 1e-10 * abs(o)
+
+
+def test_energy_hand_fixture_on_gpu(gpu):
+    torch, B, Cn = gpu
+    vel = np.array([[1, 2, 2], [0, 0, 0], [3, 4, 0], [-1, -1, -1]], np.float32).T.copy()
+    pos = np.array([[.5, .5, .5], [0, .5, .5], [.25, .75, .5], [.5, .5, 0]], np.float64).T.copy()
+    s = to_device(Cn, Cn.R1, {"id": np.arange(4, dtype=np.int32)[None], "pos": pos, "vel": vel})
+    assert s.energy(B.SOAX_ENERGY_KINETIC) == 18.5                      # tests/golden/energy_4particles.txt
+    assert s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC) == 18.8125
+
+
+# ------------------------------------------------------------------------------- a5, a6, a7: AoS (config 3)
+@pytest.mark.parametrize("n", [1 << 16, 70001, 255, 1])
+def test_aos_soa_transposes_byte_exact(gpu, n):
+    torch, B, Cn = gpu
+    rng = np.random.default_rng(n)
+    raw = rng.integers(0, 256, 40 * n, dtype=np.uint8)                # arbitrary bytes: NaN payloads, denormals, ...
+    aos = torch.from_numpy(raw).cuda()
+    s = Cn.Soax(Cn.R1, n)
+    s.from_aos(aos, n)
+    got = s.download()
+    exp = oracle.r1_aos_to_soa(raw)
+    for name in exp:
+        assert np.array_equal(bits(got[name]), bits(exp[name])), name
+    back = s.to_aos()
+    assert np.array_equal(back.cpu().numpy(), raw)                    # round trip is byte exact
+    assert np.array_equal(oracle.r1_soa_to_aos(exp), raw)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("n", [1 << 16, 7001])
+def test_aos_step_matches_oracle_and_soa_kernel(gpu, variant, n):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(n, seed=0)
+    raw = oracle.r1_soa_to_aos(host)
+    aos = torch.from_numpy(raw).cuda()
+    Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=20, variant=variant)
+    got = oracle.r1_aos_to_soa(aos.cpu().numpy())
+    check_r1(got, oracle.symplectic_euler(host, DT, 20))
+    # oracle-free cross-check: SoA kernel + SoA->AoS must reproduce the AoS kernel's bytes
+    s = to_device(Cn, Cn.R1, host)
+    s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=20)
+    assert torch.equal(s.to_aos(), aos)
+    aos2 = torch.from_numpy(raw).cuda()
+    Cn.aos_step(Cn.R1, aos2, n, B.SOAX_STEP_DRIFT, DT, nsteps=3, variant=variant)
+    check_r1(oracle.r1_aos_to_soa(aos2.cpu().numpy()), oracle.drift(host, DT, 3))
+
+
+def test_transposes_wide_record(gpu):
+    torch, B, Cn = gpu
+    n = 5003
+    host = inputs.make_r2(n, seed=2)
+    s = to_device(Cn, Cn.R2, host)
+    aos = s.to_aos()
+    stride, offs = B.soax_layout_aos(s.layout, True)
+    assert stride == 89
+    raw = aos.cpu().numpy().reshape(n, stride)
+    c = 0
+    for name, dt, dim in Cn.R2:
+        for k in range(dim):
+            sz = B.DTYPE_SIZE[dt]
+            col = np.ascontiguousarray(raw[:, offs[c]:offs[c] + sz]).view(Cn.NP_DTYPE[dt])[:, 0]
+            assert np.array_equal(bits(col), bits(host[name][k])), (name, k)
+            c += 1
+    t = Cn.Soax(Cn.R2, n)
+    t.from_aos(aos, n)
+    back = t.download()
+    for name in host:
+        assert np.array_equal(bits(back[name]), bits(host[name])), name
+
+
+# ----------------------------------------------------------------------------------------- a9: RK2 (config 4)
+@pytest.mark.parametrize("n,nsteps,mask", [(1 << 15, 20, 1), (4099, 3, 0x10), (257, 2, 0xFF)])
+def test_rk2_masked_wide_record(gpu, n, nsteps, mask):
+    torch, B, Cn = gpu
+    host = inputs.make_r2(n, seed=0)
+    if n == 4099:
+        host["vel"] *= 300.0                                          # wraps at the midpoint and at the end
+    s = to_device(Cn, Cn.R2, host)
+    s.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=nsteps, k=1.0, flag_mask=mask)
+    got = s.download()
+    exp = oracle.rk2_midpoint_masked(host, DT, nsteps, k=1.0, mask=mask)
+    assert pdist(got["pos"], exp["pos"]).max() <= 1e-12
+    assert np.abs(got["vel"] - exp["vel"]).max() <= 1e-12 and np.abs(got["acc"] - exp["acc"]).max() <= 1e-12
+    for name in host:                                                 # the contract promises bit equality
+        assert np.array_equal(bits(got[name]), bits(exp[name])), name
+    inactive = (host["flags"][0] & mask) == 0
+    for name in host:
+        assert np.array_equal(bits(got[name])[:, inactive], bits(host[name])[:, inactive]), name
+
+
+def test_rk2_acc_of_inactive_particles_is_preserved(gpu):
+    torch, B, Cn = gpu
+    host = inputs.make_r2(1001, seed=4)
+    host["acc"][:] = np.random.default_rng(0).normal(size=host["acc"].shape)   # not zero: must survive bit for bit
+    s = to_device(Cn, Cn.R2, host)
+    s.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=1)
+    got, exp = s.download(), oracle.rk2_midpoint_masked(host, DT, 1)
+    for name in host:
+        assert np.array_equal(bits(got[name]), bits(exp[name])), name
+
+
+def test_drift_wide_record(gpu):
+    torch, B, Cn = gpu
+    host = inputs.make_r2(3001, seed=6)
+    s = to_device(Cn, Cn.R2, host)
+    s.step(B.SOAX_STEP_DRIFT, DT, nsteps=4)
+    got, exp = s.download(), oracle.drift(host, DT, 4)
+    for name in host:
+        assert np.array_equal(bits(got[name]), bits(exp[name])), name
+
+
+# ------------------------------------------------------------------------------ a10..a14: binning (config 5)
+def run_bin(gpu, host, G, drift_dt=0.0, kinetic=False):
+    torch, B, Cn = gpu
+    n = host["id"].shape[1]
+    src, dst = to_device(Cn, Cn.R1, host), Cn.Soax(Cn.R1, n)
+    r = src.bin_permute(dst, G, drift_dt=drift_dt, want_kinetic=kinetic)
+    torch.cuda.synchronize()
+    out = {k: (v.cpu().numpy().view(np.uint32) if k in ("counts", "offsets", "perm") else v) for k, v in r.items()}
+    return src.download(), (dst.download() if n else None), out
+
+
+def check_bin(host_after_drift, sorted_soa, out, G):
+    exp = oracle.bin_r1(host_after_drift, G)
+    assert np.array_equal(out["counts"], exp["counts"])
+    assert np.array_equal(out["offsets"], exp["offsets"])
+    assert np.array_equal(out["perm"], exp["perm"])
+    want = oracle.permute_r1(host_after_drift, exp["perm"])
+    for name in want:
+        assert np.array_equal(bits(sorted_soa[name]), bits(want[name])), name
+    assert int(out["counts"].sum()) == host_after_drift["id"].shape[1]
+
+
+@pytest.mark.parametrize("n,G", [(100003, 64), (4096, 64), (4097, 8), (50000, 2), (31, 64), (1, 64), (70000, 1)])
+def test_bin_permute_matches_oracle(gpu, n, G):
+    host = inputs.make_r1(n, seed=7)
+    src_after, sorted_soa, out = run_bin(gpu, host, G)
+    for name in host:                                                 # no drift requested: src is read only
+        assert np.array_equal(bits(src_after[name]), bits(host[name]))
+    check_bin(host, sorted_soa, out, G)
+
+
+@pytest.mark.parametrize("case", ["one_cell", "sorted", "reverse", "two_cells_far"])
+def test_bin_permute_degenerate_distributions(gpu, case):
+    n, G = 20011, 64
+    host = inputs.make_r1(n, seed=9)
+    if case == "one_cell":
+        host["pos"][:] = 0.99 + 0.005 * host["pos"]                   # everything in the last cell
+    elif case in ("sorted", "reverse"):
+        order = np.argsort(oracle.bin_r1(host, G)["cell"], kind="stable")
+        host = inputs.take(host, order if case == "sorted" else order[::-1].copy())
+    else:
+        host["pos"][:, ::2] = 0.001
+        host["pos"][:, 1::2] = 0.999
+    src_after, sorted_soa, out = run_bin(gpu, host, G)
+    check_bin(host, sorted_soa, out, G)
+
+
+def test_bin_permute_fused_drift_and_kinetic_config5_shape(gpu):
+    torch, B, Cn = gpu
+    n, G = 1 << 17, 64
+    host = inputs.make_r1(n, seed=7)
+    src_after, sorted_soa, out = run_bin(gpu, host, G, drift_dt=DT, kinetic=True)
+    drifted = oracle.drift(host, DT, 1)
+    check_r1(src_after, drifted)                                      # the fused drift updated src in place
+    check_bin(drifted, sorted_soa, out, G)
+    ke = float(out["kinetic"].item())
+    oke = oracle.energy(drifted, oracle.KINETIC)
+    assert abs(ke - oke) <= 1e-10 * oke
+    assert np.array_equal(np.sort(sorted_soa["id"][0]), np.arange(n, dtype=np.int32))   # ids stay a permutation
+
+
+def test_bin_empty(gpu):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(0, seed=1)
+    _, _, out = run_bin(gpu, host, 4)
+    assert out["counts"].sum() == 0 and out["offsets"].sum() == 0
+
+
+# ----------------------------------------------------------------------- NEXT-1: the paper's float benchmark
+@pytest.mark.parametrize("size_extra", [0, 8, 32])
+def test_paper_float_benchmark_euler(gpu, size_extra):
+    torch, B, Cn = gpu
+    n = 10001
+    host = inputs.make_b6(n, seed=1)
+    full = dict(host)
+    if size_extra:
+        full["temp"] = np.zeros((size_extra, n), np.float32)
+    s = to_device(Cn, Cn.B6(size_extra), full)
+    s.step(B.SOAX_STEP_EULER_NOWRAP, 1e-3, nsteps=5)
+    got = s.download()
+    epos, evel = oracle.b6_euler(host["pos"], host["vel"], size_extra, np.float32(1e-3), 5)
+    assert np.array_equal(bits(got["pos"]), bits(epos)) and np.array_equal(bits(got["vel"]), bits(evel))
+
+
+# ------------------------------------------------------------------------------------------- error behaviour
+def test_error_codes(gpu):
+    torch, B, Cn = gpu
+    s = Cn.Soax(Cn.R1, 100)
+    with pytest.raises(B.SoaxError) as e:
+        B.soax_field_ptr(s.handle, 1, 3)                              # pos(42) on a 3-vector
+    assert e.value.status == B.SOAX_ERR_UNSUPPORTED
+    with pytest.raises(B.SoaxError) as e:
+        s.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT)          # R1 has no acc/mass/flags
+    assert e.value.status == B.SOAX_ERR_UNSUPPORTED
+    with pytest.raises(B.SoaxError) as e:
+        B.soax_resize(s.handle, 101)
+    assert e.value.status == B.SOAX_ERR_INVALID_ARG
+    b6 = Cn.Soax(Cn.B6(0), 10)
+    with pytest.raises(B.SoaxError) as e:
+        b6.bin_permute(Cn.Soax(Cn.B6(0), 10), 4, scratch=torch.empty(1 << 20, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == B.SOAX_ERR_UNSUPPORTED
