@@ -1,0 +1,413 @@
+"""bench.py -- particle-steps/s of the SoAx hot path on B200, with roofline, end-to-end and CPU-oracle figures.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl soax|reference] [--no-extras]
+
+Workload (BASELINE.json configs[1], "config 2"): N = 2^24 particles, record R1 {int32 id; double pos[3]; float vel[3]}
+stored as a Structure of Arrays, seed 0.  One bench "step" = one pass of config 2's whole path over the resident
+batch: energy (kinetic + harmonic, double) -> 100 symplectic-Euler steps (one kernel launch and one full memory
+pass each, Q14) -> energy.  value = particle-steps/s = ranks * N * 100 * K / time, inputs resident in HBM.
+N > 1 GPUs: weak scaling, every rank integrates its own 2^24-particle shard, no data-path collective.
+The working set (671 MB per rank) exceeds the 126 MB L2, so no flush is needed between iterations.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+LOG2N = 24
+NSTEPS = 100          # symplectic-Euler steps per bench step (config 2)
+DT = 1e-3
+STEP_BYTES = 72       # algorithmic bytes per particle per symplectic-Euler pass: 36 read + 36 written
+METRIC, UNIT = "particle-steps/s", "particle-steps/s"
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def committed_traffic():
+    """dram bytes per launch of the step kernel from the committed ncu --set full capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "step_kernel_traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f).get("dram_bytes_per_launch")
+    return None
+
+
+# ---------------------------------------------------------------------------------------------- clocks sampling
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(device_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def wait_first_sample(self, timeout: float = 5.0) -> None:
+        t0 = time.time()
+        while self.p is not None and os.path.getsize(self.f.name) == 0 and time.time() - t0 < timeout:
+            time.sleep(0.02)
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        for line in self.f:
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0])); mx.append(float(t[1])); pw.append(float(t[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), t[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------- the CPU oracle, timed
+def time_oracle(host, n_sample: int, nsteps: int) -> tuple[float, float]:
+    """particle-steps/s of the single-threaded oracle on the first n_sample particles; returns (rate, seconds)."""
+    import numpy as np
+    import oracle
+    from paper_1710_03462_b200 import inputs
+    sub = inputs.take(host, np.arange(n_sample))
+    aos = oracle.pack_r1(sub)                                    # packing is outside the timed loop
+    e = oracle.lib().soax_oracle_r1_energy
+    t0 = time.perf_counter()
+    e(aos.ctypes.data, aos.size, 1, 1.0, 0.5)
+    oracle.lib().soax_oracle_r1_symplectic_euler(aos.ctypes.data, aos.size, DT, 1.0, 0.5, nsteps)
+    e(aos.ctypes.data, aos.size, 1, 1.0, 0.5)
+    dt = time.perf_counter() - t0
+    return n_sample * nsteps / dt, dt
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle as it stands, on the host cores, each step a bounded sample of config 2."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1710_03462_b200 import inputs
+    n_sample = 1 << 18
+    host = inputs.make_r1(n_sample, seed=0)                      # counter-based: a prefix of the 2^24 set
+    for _ in range(args.warmup):
+        time_oracle(host, n_sample, NSTEPS)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time_oracle(host, n_sample, NSTEPS)
+    dt = time.perf_counter() - t0
+    value = n_sample * NSTEPS * args.steps / dt
+    sample = f"first 2^18 of the 2^24 particles x {NSTEPS} symplectic-Euler steps + 2 energy sums per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64+f32", "data": "synthetic",
+        "config": {"workload": "config2: R1 SoA symplectic-Euler harmonic, N=2^24, 100 steps + energy at step 0 and 100",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ------------------------------------------------------------------------------------------------- GPU helpers
+def ev_time_ms(torch, fn, iters: int, warmup: int = 3) -> float:
+    """average milliseconds of fn() over `iters` calls, CUDA events on the current stream, after warm-up"""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(iters):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / iters
+
+
+def device_fill(torch, s, seed: int) -> None:
+    """Seeded synthetic particles generated ON the device for the extra (non-headline) configs: same distributions
+    as inputs.py (id permutation, pos U[0,1)^3, vel N(0,1), mass U[0.5,2), charge +-1, flags uniform bytes)."""
+    g = torch.Generator(device="cuda")
+    g.manual_seed(seed)
+    n = s.n
+    names = [f[0] for f in s.fields]
+    iddt = s.comp_view("id").dtype
+    s.comp_view("id").copy_(torch.randperm(n, generator=g, device="cuda", dtype=torch.int64).to(iddt))
+    for c in range(3):
+        s.comp_view("pos", c).copy_(torch.rand(n, generator=g, device="cuda", dtype=torch.float64))
+        v = s.comp_view("vel", c)
+        v.copy_(torch.randn(n, generator=g, device="cuda", dtype=v.dtype))
+        if "acc" in names:
+            s.comp_view("acc", c).zero_()
+    if "mass" in names:
+        s.comp_view("mass").copy_(0.5 + 1.5 * torch.rand(n, generator=g, device="cuda", dtype=torch.float32)).clamp_(max=1.9999999)
+        s.comp_view("charge").copy_(torch.randint(0, 2, (n,), generator=g, device="cuda").float() * 2 - 1)
+        s.comp_view("flags").copy_(torch.randint(0, 256, (n,), generator=g, device="cuda", dtype=torch.uint8))
+
+
+def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5"), iters: int = 3) -> dict:
+    """The other section-8(a) rows, each timed alone with CUDA events (N=1, rank 0): reported beside the headline."""
+    ex = {}
+    n = s.n
+    gbs = lambda bytes_per_p, npart, ms: bytes_per_p * npart / ms / 1e6   # noqa: E731
+    if "energy" in which:
+        _extra_energy(torch, B, Cn, s, peak, ex, gbs)
+    if "config3" in which:
+        _extra_config3(torch, B, Cn, s, peak, ex, gbs, iters)
+    if "config1" in which:
+        _extra_config1(torch, B, Cn, ex)
+    if "config4" in which:
+        _extra_config4(torch, B, Cn, peak, ex, gbs, iters)
+    if "config5" in which:
+        _extra_config5(torch, B, Cn, peak, ex, gbs, iters)
+    return ex
+
+
+def _extra_energy(torch, B, Cn, s, peak, ex, gbs):
+    n = s.n
+    ms = ev_time_ms(torch, lambda: s.energy_async(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC), 20)
+    ex["energy_ke_pe"] = {"ms": ms, "GBps_algorithmic": gbs(36, n, ms), "frac_of_peak": gbs(36, n, ms) / peak}
+
+
+
+def _extra_config3(torch, B, Cn, s, peak, ex, gbs, iters):
+    # config 3: AoS baseline (paper-faithful and staged), transposes, SoA/AoS speed-up
+    n = s.n
+    ms_soa = ev_time_ms(torch, lambda: s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=NSTEPS), iters, 1) / NSTEPS
+    aos = s.to_aos()
+    ms_a2s = ev_time_ms(torch, lambda: s.from_aos(aos, n), 20)
+    ms_s2a = ev_time_ms(torch, lambda: s.to_aos(aos), 20)
+    ms_aos0 = ev_time_ms(torch, lambda: Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, NSTEPS, 0), iters, 1) / NSTEPS
+    ms_aos1 = ev_time_ms(torch, lambda: Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, NSTEPS, 1), iters, 1) / NSTEPS
+    ex["config3_aos_vs_soa"] = {
+        "n": n, "soa_step_ms": ms_soa, "aos_step_ms_thread_per_record": ms_aos0, "aos_step_ms_smem_staged": ms_aos1,
+        "soa_over_aos_speedup": ms_aos0 / ms_soa, "soa_over_staged_aos_speedup": ms_aos1 / ms_soa,
+        "aos_to_soa_ms": ms_a2s, "soa_to_aos_ms": ms_s2a,
+        "aos_to_soa_GBps": gbs(80, n, ms_a2s), "soa_to_aos_GBps": gbs(80, n, ms_s2a),
+        "aos_step_GBps_80B": gbs(80, n, ms_aos0), "staged_aos_step_GBps_80B": gbs(80, n, ms_aos1),
+        "transpose_break_even_steps": (ms_a2s + ms_s2a) / max(ms_aos0 - ms_soa, 1e-9)}
+
+
+def _extra_config1(torch, B, Cn, ex):
+    # config 1: 65536 particles, 10 drift steps (L2 resident, launch bound: no roofline claim)
+    s1 = Cn.Soax(Cn.R1, 65536)
+    device_fill(torch, s1, 0)
+    ms = ev_time_ms(torch, lambda: s1.step(B.SOAX_STEP_DRIFT, DT, nsteps=10), 20)
+    ex["config1_drift_l2_resident"] = {"n": 65536, "us_per_step": 1e3 * ms / 10, "particle_steps_per_s": 65536 * 10 / (ms * 1e-3)}
+
+
+def _extra_config4(torch, B, Cn, peak, ex, gbs, iters):
+    # config 4: wide record R2, N = 2^26, 20 masked RK2 steps
+    n4 = 1 << 26
+    s4 = Cn.Soax(Cn.R2, n4)
+    device_fill(torch, s4, 0)
+    ms = ev_time_ms(torch, lambda: s4.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=20, k=1.0, flag_mask=1), iters, 1) / 20
+    ex["config4_rk2_masked"] = {"n": n4, "ms_per_step": ms, "particle_steps_per_s": n4 / (ms * 1e-3),
+                                "GBps_63B_byte_granular": gbs(63, n4, ms), "GBps_117p5B_sector_granular": gbs(117.5, n4, ms),
+                                "frac_of_peak_117p5B": gbs(117.5, n4, ms) / peak}
+    del s4
+    torch.cuda.empty_cache()
+
+
+def _extra_config5(torch, B, Cn, peak, ex, gbs, iters):
+    # config 5: N = 2^27, fused drift + cell + KE, then the stable counting sort moving all 7 arrays
+    n5 = 1 << 27
+    s5, d5 = Cn.Soax(Cn.R1, n5), Cn.Soax(Cn.R1, n5)
+    device_fill(torch, s5, 7)
+    scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n5, 64), dtype=torch.uint8, device="cuda")
+    ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), iters, 1)
+    ms_d = ev_time_ms(torch, lambda: s5.step(B.SOAX_STEP_DRIFT, DT, nsteps=1), 5, 1)
+    ex["config5_bin_permute"] = {"n": n5, "grid": 64, "ms_total_drift_cell_ke_sort_permute": ms, "particles_per_s": n5 / (ms * 1e-3),
+                                 "drift_only_ms": ms_d, "drift_GBps_60B": gbs(60, n5, ms_d),
+                                 "GBps_ideal_148B": gbs(60 + 4 + 84, n5, ms), "scratch_GB": scratch.numel() / 1e9}
+
+
+# ------------------------------------------------------------------------------------------------- the SoAx arm
+def run_soax(args) -> None:
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_1710_03462_b200 import binding as B, container as Cn, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SoAx path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+
+    n = 1 << LOG2N
+    kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
+    if args.only_extras:                                          # profiling aid: one extra config alone, no headline
+        s = Cn.Soax(Cn.R1, n)
+        device_fill(torch, s, 0)
+        ex = run_extras(torch, B, Cn, s, measured_peak()[0], which=tuple(args.only_extras.split(",")), iters=max(1, args.steps))
+        print(json.dumps({"extras_only": ex, "gpu_launches": B.soax_launch_count()}))
+        return
+    host = inputs.make_r1(n, seed=rank)                           # weak scaling: each rank owns its own 2^24 shard
+    s = Cn.Soax(Cn.R1, n)
+    s.upload(host)
+    e_buf = torch.zeros(2, dtype=torch.float64, device="cuda")
+
+    def bench_step(ev=None):
+        s.energy_async(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, out=e_buf[0:1])
+        if ev:
+            ev[0].record()
+        s.step(kind, DT, nsteps=NSTEPS)
+        if ev:
+            ev[1].record()
+        s.energy_async(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, out=e_buf[1:2])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        bench_step()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.wait_first_sample()
+        for _ in range(2):                                        # keep the GPU under load while the sampler spins up
+            bench_step()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_a, t_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    l0 = B.soax_launch_count()
+    t_a.record()
+    for k in range(args.steps):
+        bench_step(evs[k])
+    t_b.record()
+    barrier()
+    launches = B.soax_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    ms = torch.tensor([t_a.elapsed_time(t_b)], dtype=torch.float64, device="cuda")
+    kern_ms = torch.tensor([sum(a.elapsed_time(b) for a, b in evs) / (NSTEPS * args.steps)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(kern_ms, op=dist.ReduceOp.MAX)
+    total_ms, kernel_ms = float(ms.item()), float(kern_ms.item())
+    value = world * n * NSTEPS * args.steps / (total_ms * 1e-3)
+    energies = [float(x) for x in e_buf.cpu()]
+
+    # ---- end to end through the C ABI with HOST buffers: upload -> energy, 100 steps, energy -> download ------------
+    pin = {k: torch.from_numpy(v).pin_memory() for k, v in host.items()}
+    out = {"pos": torch.empty((3, n), dtype=torch.float64).pin_memory(), "vel": torch.empty((3, n), dtype=torch.float32).pin_memory()}
+    e_host = torch.empty(2, dtype=torch.float64).pin_memory()
+    stream = torch.cuda.current_stream().cuda_stream
+    up_ptrs = [pin["id"][0].data_ptr()] + [pin["pos"][c].data_ptr() for c in range(3)] + [pin["vel"][c].data_ptr() for c in range(3)]
+    dn_ptrs = [None] + [out["pos"][c].data_ptr() for c in range(3)] + [out["vel"][c].data_ptr() for c in range(3)]
+
+    def e2e_step():
+        B.soax_upload(s.handle, up_ptrs, n, stream)
+        bench_step()
+        B.soax_download(s.handle, dn_ptrs, n, stream)
+        e_host.copy_(e_buf, non_blocking=True)
+        torch.cuda.current_stream().synchronize()              # the caller consumes the result of every step
+
+    for _ in range(max(1, min(args.warmup, 3))):
+        e2e_step()
+    barrier()
+    t_a.record()
+    for _ in range(args.steps):
+        e2e_step()
+    t_b.record()
+    barrier()
+    ms2 = torch.tensor([t_a.elapsed_time(t_b)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
+    e2e_value = world * n * NSTEPS * args.steps / (float(ms2.item()) * 1e-3)
+    e2e_check = bool(np.isfinite(out["pos"].numpy()).all())
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        achieved = STEP_BYTES * n / kernel_ms / 1e6              # GB/s: algorithmic bytes per launch / avg launch time
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64+f32", "data": "synthetic",
+            "config": {"workload": "config2: R1 {int32 id; double pos[3]; float vel[3]} SoA, N=2^24 per GPU, seed=rank, "
+                                   "per step: energy(KE+PE) + 100 symplectic-Euler harmonic steps (dt=1e-3, periodic wrap) + energy",
+                       "n_particles_per_gpu": n, "integration_steps_per_bench_step": NSTEPS, "parallelism": f"dp{world} (independent shards, no collective)",
+                       "l2": "working set 671 MB per GPU exceeds the 126 MB L2: no flush needed between iterations",
+                       "timing": "CUDA events on the launching stream, barrier + synchronize on both sides, max over ranks"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 40 * n, "d2h_bytes_per_step": 36 * n + 16,
+                    "ms_per_step": float(ms2.item()) / args.steps, "finite": e2e_check,
+                    "path": "soax_upload (7 pinned host arrays) -> soax_reduce_energy, 100 x soax_step, soax_reduce_energy -> soax_download (pos, vel) + energies"},
+            "roofline": {"bound": "hbm", "kernel": "step_soa_kernel<R1, SYMPLECTIC_EULER_HARMONIC, 4>", "achieved": achieved,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": committed_traffic(),
+                         "peak_source": peak_src, "algorithmic_bytes_per_launch": STEP_BYTES * n,
+                         "avg_launch_ms": kernel_ms, "frac_of_nominal_8TBps": achieved / 8000.0,
+                         "kernel_share_of_step": kernel_ms * NSTEPS * args.steps / total_ms},
+            "energy_step0_step100_last": energies,
+        }
+        if world == 1:
+            t0 = time.perf_counter()
+            n_sample = 1 << 21
+            rate, secs = time_oracle(host, n_sample, NSTEPS)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs,
+                                    "host_cores_available": os.cpu_count(),
+                                    "sample": f"first 2^21 of the 2^24 particles x {NSTEPS} symplectic-Euler steps + 2 energy sums, single thread"}
+            if not args.no_extras:
+                del pin, out
+                line["extras"] = run_extras(torch, B, Cn, s, peak)
+            line["host_seconds_outside_timed_regions"] = time.perf_counter() - t0
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["soax", "reference"], default="soax")
+    ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
+    ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5: run just those")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_soax(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -225,6 +225,127 @@ __global__ void __launch_bounds__(kSortThreads) scatter_kernel(Ptrs<L::ncomp> sr
     });
 }
 
+// ---- stable scatter, shared-memory staged: the tile is first sorted INSIDE shared memory, so that consecutive
+// threads then write consecutive slots of each bin's run and every run leaves the SM as a few full sectors
+// (the direct kernel above sends 32 different sectors per warp store).  One staging buffer (8 bytes per slot)
+// is reused for the key array, the index array and each component array in turn; it aliases the per-warp
+// counters, which are dead once every particle knows its slot.
+template <class T>
+__device__ __forceinline__ void stage_move(const T* __restrict__ s, T* __restrict__ t, unsigned char* buf, int64_t e0, int64_t n,
+                                           int cnt, const uint32_t (&lpos)[kItems], const uint32_t (&gdest)[kItems]) {
+    T* sm = reinterpret_cast<T*>(buf);
+    T val[kItems];
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int64_t e = e0 + k * 32;
+        if (e < n) val[k] = s[e];
+    }
+    __syncthreads();  // the previous array has been read out of the buffer
+#pragma unroll
+    for (int k = 0; k < kItems; ++k)
+        if (e0 + k * 32 < n) sm[lpos[k]] = val[k];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int j = threadIdx.x + k * kSortThreads;
+        if (j < cnt) t[gdest[k]] = sm[j];
+    }
+}
+
+template <class L>
+__global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst,
+                                                                      const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
+                                                                      const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ idx_out,
+                                                                      const uint32_t* __restrict__ base, int64_t n, int shift) {
+    __shared__ __align__(16) unsigned char buf[kWarps * kRadix * 4 > kTileN * 8 ? kWarps * kRadix * 4 : kTileN * 8];
+    __shared__ uint32_t delta[kRadix];  // global slot of a bin's first item minus its first slot inside the sorted tile
+    __shared__ uint32_t scan_sm[32];
+    uint32_t* wcnt = reinterpret_cast<uint32_t*>(buf);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
+    __syncthreads();
+
+    const int64_t tile0 = (int64_t)blockIdx.x * kTileN;
+    const int cnt = (int)(n - tile0 < kTileN ? n - tile0 : kTileN);
+    const int64_t e0 = tile0 + warp * (32 * kItems) + lane;
+    uint32_t key[kItems], lpos[kItems], gdest[kItems];
+    uint32_t* mycnt = wcnt + warp * kRadix;
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int64_t e = e0 + k * 32;
+        const bool valid = e < n;
+        key[k] = valid ? key_in[e] : 0u;
+        const uint32_t d = (key[k] >> shift) & (kRadix - 1);
+        const uint32_t peers = __match_any_sync(0xffffffffu, valid ? d : (0x10000u | lane));
+        const uint32_t old = mycnt[d];
+        lpos[k] = old + __popc(peers & lt);
+        __syncwarp();
+        if (valid && lane == 31 - __clz(peers)) mycnt[d] = old + __popc(peers);
+        __syncwarp();
+    }
+    __syncthreads();
+    {   // digit d = threadIdx.x: tile total -> first slot of the bin inside the sorted tile -> per-warp first slots
+        uint32_t total = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) total += wcnt[w * kRadix + threadIdx.x];
+        uint32_t run = block_excl_scan(total, scan_sm);
+        delta[threadIdx.x] = base[(int64_t)blockIdx.x * kRadix + threadIdx.x] - run;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            const uint32_t c = wcnt[w * kRadix + threadIdx.x];
+            wcnt[w * kRadix + threadIdx.x] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) lpos[k] += mycnt[(key[k] >> shift) & (kRadix - 1)];
+    __syncthreads();  // the counters are dead from here on: `buf` becomes the staging buffer
+
+    // keys first: the sorted keys tell every output slot j which bin (hence which global run) it belongs to
+    {
+        uint32_t* sm = reinterpret_cast<uint32_t*>(buf);
+#pragma unroll
+        for (int k = 0; k < kItems; ++k)
+            if (e0 + k * 32 < n) sm[lpos[k]] = key[k];
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int j = threadIdx.x + k * kSortThreads;
+            if (j < cnt) {
+                const uint32_t kj = sm[j];
+                gdest[k] = delta[(kj >> shift) & (kRadix - 1)] + (uint32_t)j;
+                key_out[gdest[k]] = kj;
+            }
+        }
+    }
+    // source indices (generated in the first pass, carried in the second): perm falls out of the last pass
+    {
+        uint32_t* sm = reinterpret_cast<uint32_t*>(buf);
+        uint32_t val[kItems];
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int64_t e = e0 + k * 32;
+            if (e < n) val[k] = idx_in ? idx_in[e] : (uint32_t)e;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kItems; ++k)
+            if (e0 + k * 32 < n) sm[lpos[k]] = val[k];
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int j = threadIdx.x + k * kSortThreads;
+            if (j < cnt) idx_out[gdest[k]] = sm[j];
+        }
+    }
+    for_each_comp<L>([&](auto ci) {
+        constexpr int C = decltype(ci)::value;
+        stage_move(comp_ptr<L, C>(src), comp_ptr<L, C>(dst), buf, e0, n, cnt, lpos, gdest);
+    });
+}
+
 // ---- counts / offsets from the sorted keys --------------------------------------------------------------------------
 // off[c] = first sorted slot whose key is >= c, for c = 0..ncell (off[ncell] = n)
 __global__ void __launch_bounds__(256) boundaries_kernel(const uint32_t* __restrict__ sorted, int64_t n, uint32_t ncell,
@@ -344,7 +465,10 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
             SOAX_TRY(launched());
             colscan_apply_kernel<<<nchunks, kRadix, 0, st>>>(hist, (int)ntiles, partial, dbase);
             SOAX_TRY(launched());
-            scatter_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+            if (g_tune.bin_stage)
+                scatter_staged_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+            else
+                scatter_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
             SOAX_TRY(launched());
         }
         if (a.counts || a.offsets) {
