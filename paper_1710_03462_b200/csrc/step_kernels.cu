@@ -128,6 +128,7 @@ constexpr bool step_supported() {
 
 template <class L, int KIND, int P>
 static int launch_step(const Ptrs<L::ncomp>& a, int64_t n, const StepK& c, cudaStream_t st) {
+    if (n == 0) return SOAX_OK;
     const int block = g_tune.step_block;
     const int64_t threads = (n / P > n % P ? n / P : n % P);
     int64_t blocks = (threads + block - 1) / block;
@@ -152,7 +153,6 @@ static int step_kind(const Ptrs<L::ncomp>& a, int64_t n, const StepK& c, cudaStr
 
 template <class L>
 int step_entry(void* const* comps, int64_t n, const soax_step_params* p, cudaStream_t st) {
-    if (n == 0) return SOAX_OK;
     const Ptrs<L::ncomp> a = make_ptrs<L>(comps);
     StepK c;
     c.dt = p->dt; c.k = p->k; c.ctr = p->center; c.hh = 0.5 * p->dt; c.dt_f = (float)p->dt; c.mask = p->flag_mask;
