@@ -252,6 +252,41 @@ def _extra_config5(torch, B, Cn, peak, ex, gbs, iters):
                                  "GBps_ideal_148B": gbs(60 + 4 + 84, n5, ms), "scratch_GB": scratch.numel() / 1e9}
 
 
+def run_tour(torch, B, Cn) -> None:
+    """Profiling aid (--tour): every kernel family of the library launched twice at its config's full size, nothing
+    timed.  `ncu --metrics ... python bench.py --tour` gives the per-kernel counters committed under profiles/."""
+    n = 1 << LOG2N
+    s = Cn.Soax(Cn.R1, n)
+    device_fill(torch, s, 0)
+    for _ in range(2):
+        s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=1)            # a4  (config 2)
+        s.energy_async(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC)                    # a8
+        s.step(B.SOAX_STEP_DRIFT, DT, nsteps=1)                                # a2
+    aos = s.to_aos()
+    for _ in range(2):
+        s.to_aos(aos)                                                          # a7  (config 3)
+        s.from_aos(aos, n)                                                     # a6
+        Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, 1, 0)   # a5 thread per record
+        Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, 1, 1)   # a5 staged
+    del s, aos
+    torch.cuda.empty_cache()
+    n4 = 1 << 26
+    s4 = Cn.Soax(Cn.R2, n4)
+    device_fill(torch, s4, 0)
+    for _ in range(2):
+        s4.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=1, k=1.0, flag_mask=1)   # a9  (config 4)
+    del s4
+    torch.cuda.empty_cache()
+    n5 = 1 << 27
+    s5, d5 = Cn.Soax(Cn.R1, n5), Cn.Soax(Cn.R1, n5)
+    device_fill(torch, s5, 7)
+    scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n5, 64), dtype=torch.uint8, device="cuda")
+    for _ in range(2):
+        s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch)   # a10-a14 (config 5)
+    torch.cuda.synchronize()
+    print(json.dumps({"tour": "done", "gpu_launches": B.soax_launch_count()}))
+
+
 # ------------------------------------------------------------------------------------------------- the SoAx arm
 def run_soax(args) -> None:
     import numpy as np
@@ -272,6 +307,9 @@ def run_soax(args) -> None:
 
     n = 1 << LOG2N
     kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
+    if args.tour:
+        run_tour(torch, B, Cn)
+        return
     if args.only_extras:                                          # profiling aid: one extra config alone, no headline
         s = Cn.Soax(Cn.R1, n)
         device_fill(torch, s, 0)
@@ -402,6 +440,7 @@ def main() -> None:
     ap.add_argument("--impl", choices=["soax", "reference"], default="soax")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5: run just those")
+    ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
