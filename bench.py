@@ -304,6 +304,9 @@ def run_soax(args) -> None:
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()
+    for kv in filter(None, args.tune.split(",")):
+        key, val = kv.split("=")
+        B.soax_tune(key, int(val))
 
     n = 1 << LOG2N
     kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
@@ -440,6 +443,7 @@ def main() -> None:
     ap.add_argument("--impl", choices=["soax", "reference"], default="soax")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5: run just those")
+    ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -14,6 +14,7 @@
 // counts / offsets come from the sorted keys by boundary detection.
 #include "common.cuh"
 #include "ops.hpp"
+#include "tma.cuh"
 
 namespace soax {
 
@@ -87,22 +88,38 @@ __global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t*
     h[threadIdx.x] = 0;
     __syncthreads();
     const int64_t tile0 = (int64_t)blockIdx.x * kTileN;
+    if (tile0 + kTileN <= n) {  // full tile: two 128-bit loads per thread (the histogram does not care about order)
+        const uint4* k4 = reinterpret_cast<const uint4*>(keys + tile0);
+        const uint4 a = k4[threadIdx.x], b = k4[threadIdx.x + kSortThreads];
+        const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) {
-        const int64_t e = tile0 + k * kSortThreads + threadIdx.x;
-        if (e < n) atomicAdd(&h[(keys[e] >> shift) & (kRadix - 1)], 1u);
+        for (int k = 0; k < 8; ++k) atomicAdd(&h[(w[k] >> shift) & (kRadix - 1)], 1u);
+    } else {
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const int64_t e = tile0 + k * kSortThreads + threadIdx.x;
+            if (e < n) atomicAdd(&h[(keys[e] >> shift) & (kRadix - 1)], 1u);
+        }
     }
     __syncthreads();
     hist[(int64_t)blockIdx.x * kRadix + threadIdx.x] = h[threadIdx.x];
 }
 
 // ---- exclusive scan of hist[tile][digit] in (digit-major, tile-minor) order ----------------------------------------
-// phase 1: column sums of each chunk of kScanRows tiles
+// phase 1: column sums of each chunk of kScanRows tiles.  Loads are issued in batches of 16 independent rows so
+// that the table streams at memory speed instead of one dependent round trip per row.
+constexpr int kScanBatch = 16;
 __global__ void __launch_bounds__(kRadix) colscan_reduce_kernel(const uint32_t* __restrict__ hist, int ntiles,
                                                                 uint32_t* __restrict__ partial) {
     const int r0 = blockIdx.x * kScanRows, r1 = min(r0 + kScanRows, ntiles);
     uint32_t s = 0;
-    for (int r = r0; r < r1; ++r) s += hist[(int64_t)r * kRadix + threadIdx.x];
+    for (int r = r0; r < r1; r += kScanBatch) {
+        uint32_t v[kScanBatch];
+#pragma unroll
+        for (int u = 0; u < kScanBatch; ++u) v[u] = r + u < r1 ? hist[(int64_t)(r + u) * kRadix + threadIdx.x] : 0u;
+#pragma unroll
+        for (int u = 0; u < kScanBatch; ++u) s += v[u];
+    }
     partial[(int64_t)blockIdx.x * kRadix + threadIdx.x] = s;
 }
 // exclusive scan of one value per thread over a CTA of kRadix threads
@@ -134,10 +151,15 @@ __global__ void __launch_bounds__(kRadix) colscan_top_kernel(uint32_t* __restric
                                                              uint32_t* __restrict__ dbase) {
     __shared__ uint32_t sm[32];
     uint32_t run = 0;
-    for (int c = 0; c < nchunks; ++c) {
-        const uint32_t v = partial[(int64_t)c * kRadix + threadIdx.x];
-        partial[(int64_t)c * kRadix + threadIdx.x] = run;
-        run += v;
+    for (int c = 0; c < nchunks; c += kScanBatch) {
+        uint32_t v[kScanBatch];
+#pragma unroll
+        for (int u = 0; u < kScanBatch; ++u) v[u] = c + u < nchunks ? partial[(int64_t)(c + u) * kRadix + threadIdx.x] : 0u;
+#pragma unroll
+        for (int u = 0; u < kScanBatch; ++u) {
+            if (c + u < nchunks) partial[(int64_t)(c + u) * kRadix + threadIdx.x] = run;
+            run += v[u];
+        }
     }
     dbase[threadIdx.x] = block_excl_scan(run, sm);
 }
@@ -147,10 +169,15 @@ __global__ void __launch_bounds__(kRadix) colscan_apply_kernel(uint32_t* __restr
                                                                const uint32_t* __restrict__ dbase) {
     const int r0 = blockIdx.x * kScanRows, r1 = min(r0 + kScanRows, ntiles);
     uint32_t run = dbase[threadIdx.x] + partial[(int64_t)blockIdx.x * kRadix + threadIdx.x];
-    for (int r = r0; r < r1; ++r) {
-        const uint32_t v = hist[(int64_t)r * kRadix + threadIdx.x];
-        hist[(int64_t)r * kRadix + threadIdx.x] = run;
-        run += v;
+    for (int r = r0; r < r1; r += kScanBatch) {
+        uint32_t v[kScanBatch];
+#pragma unroll
+        for (int u = 0; u < kScanBatch; ++u) v[u] = r + u < r1 ? hist[(int64_t)(r + u) * kRadix + threadIdx.x] : 0u;
+#pragma unroll
+        for (int u = 0; u < kScanBatch; ++u) {
+            if (r + u < r1) hist[(int64_t)(r + u) * kRadix + threadIdx.x] = run;
+            run += v[u];
+        }
     }
 }
 
@@ -346,6 +373,185 @@ __global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::nc
     });
 }
 
+// ---- stable scatter, TMA ring (default): every array of the tile (keys, carried source indices, each component
+// array) arrives in shared memory as ONE 1-D bulk asynchronous copy (cp.async.bulk -> UBLKCP) into a 3-stage
+// ring, so the loads of the next arrays are in flight while the current one is being written out; nothing passes
+// through registers on the way in.  The tile is never physically sorted in shared memory: after the ranking
+// every output slot j knows its source element inv[j] (the inverse of the in-tile stable permutation), reads
+// ring[inv[j]] and writes it to its global slot, consecutive threads writing consecutive slots of a bin's run.
+// 64 registers/thread and ~106 KB of shared memory let two CTAs share an SM: one ranks while the other streams.
+constexpr int kRingStages = 3;
+constexpr int kStageBytes = kTileN * 8;  // one array of the tile at 8 bytes per element
+constexpr int kRingSmem = kRingStages * kStageBytes + kTileN * 2 /*inv*/ + kRadix * 4 /*delta*/ + 32 * 4 /*scan*/ + 64 /*mbarriers*/;
+static_assert(kWarps * kRadix * 4 <= kStageBytes, "the per-warp counters alias ring stage 1");
+
+template <class L, bool HAS_IDX>
+__global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst,
+                                                                      const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
+                                                                      const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ idx_out,
+                                                                      const uint32_t* __restrict__ base, int64_t n, int shift) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* ring = smem;
+    uint16_t* inv = reinterpret_cast<uint16_t*>(smem + kRingStages * kStageBytes);
+    uint32_t* delta = reinterpret_cast<uint32_t*>(smem + kRingStages * kStageBytes + kTileN * 2);
+    uint32_t* scan_sm = delta + kRadix;
+    uint64_t* full = reinterpret_cast<uint64_t*>(scan_sm + 32);
+    uint32_t* wcnt = reinterpret_cast<uint32_t*>(ring + kStageBytes);  // aliases stage 1 until the ranking is done
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t tile0 = (int64_t)blockIdx.x * kTileN;
+    const int cnt = (int)(n - tile0 < kTileN ? n - tile0 : kTileN);
+    const bool bulk = cnt == kTileN;  // CTA-uniform: the ragged last tile is filled by ordinary loads instead
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kRingStages; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    // fill(stage, array): start bringing `cnt` elements of an array into a ring stage.  Called by ALL threads at
+    // CTA-uniform points, after a __syncthreads() that retired every reader of the stage.
+    auto fill = [&](int stage, const auto* g) {
+        using T = std::remove_cv_t<std::remove_pointer_t<decltype(g)>>;
+        unsigned char* sb = ring + stage * kStageBytes;
+        if (bulk) {
+            if (tid == 0) {
+                mbar_expect_tx(&full[stage], kTileN * (uint32_t)sizeof(T));
+                bulk_g2s(sb, g + tile0, kTileN * (uint32_t)sizeof(T), &full[stage]);
+            }
+        } else {
+            T* s = reinterpret_cast<T*>(sb);
+            for (int i = tid; i < cnt; i += kSortThreads) s[i] = g[tile0 + i];
+        }
+    };
+    // ready(stage, parity): the array requested by the matching fill() is in shared memory
+    auto ready = [&](int stage, uint32_t parity) {
+        if (bulk) mbar_wait(&full[stage], parity);
+        else __syncthreads();
+    };
+    for (int i = tid; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
+    const uint32_t my_base = base[(int64_t)blockIdx.x * kRadix + tid];  // issued now, consumed after the ranking
+    __syncthreads();  // barriers initialised, counters zeroed
+
+    // sequence of arrays moved by this CTA: 0 = keys, [1 = carried indices,] then the components; array a uses
+    // ring stage a % 3 for the (a / 3)-th time.  Stage 1 is the counters for now, so start with arrays 0 and 2.
+    constexpr int kFirstComp = HAS_IDX ? 2 : 1;
+    constexpr int kArrays = kFirstComp + L::ncomp;
+    auto fill_array = [&](auto ai) {  // ai: integral_constant<int, a>
+        constexpr int a = decltype(ai)::value;
+        if constexpr (a >= kArrays) {
+        } else if constexpr (a == 0) {
+            fill(0, key_in);
+        } else if constexpr (HAS_IDX && a == 1) {
+            fill(1, idx_in);
+        } else {
+            constexpr int C = a - kFirstComp;
+            fill(a % kRingStages, comp_ptr<L, C>(src));
+        }
+    };
+    fill_array(std::integral_constant<int, 0>{});
+    fill_array(std::integral_constant<int, 2>{});
+
+    // ---- ranking: warp w owns elements [256 w, 256 w + 256) of the tile, 8 rounds of 32 in element order -------
+    ready(0, 0);
+    const uint32_t* keybuf = reinterpret_cast<const uint32_t*>(ring);
+    const int e0 = warp * (32 * kItems) + lane;
+    uint32_t lpos[kItems];
+    uint32_t* mycnt = wcnt + warp * kRadix;
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t peers[kItems];
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {  // lanes holding the same digit, from kRadixBits ballots (no MATCH: its cost grows with the number of distinct values)
+        const int e = e0 + k * 32;
+        const bool valid = e < cnt;
+        const uint32_t d = valid ? (keybuf[e] >> shift) & (kRadix - 1) : 0u;
+        uint32_t m = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+        for (int b = 0; b < kRadixBits; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+            m &= bit ? bal : ~bal;
+        }
+        peers[k] = valid ? m : 0u;
+        lpos[k] = d;
+    }
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const uint32_t d = lpos[k];
+        const uint32_t old = mycnt[d];
+        lpos[k] = old + __popc(peers[k] & lt);
+        __syncwarp();
+        if (peers[k] != 0u && lane == 31 - __clz(peers[k])) mycnt[d] = old + __popc(peers[k]);
+        __syncwarp();
+    }
+    __syncthreads();
+    {   // digit d = tid: tile total -> first slot of the bin in tile-sorted order -> per-warp first slots
+        uint32_t total = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) total += wcnt[w * kRadix + tid];
+        uint32_t run = block_excl_scan(total, scan_sm);
+        delta[tid] = my_base - run;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            const uint32_t c = wcnt[w * kRadix + tid];
+            wcnt[w * kRadix + tid] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int e = e0 + k * 32;
+        if (e < cnt) inv[lpos[k] + mycnt[(keybuf[e] >> shift) & (kRadix - 1)]] = (uint16_t)e;
+    }
+    fence_async_smem();  // the counters (generic-proxy writes) are about to be overwritten by a bulk copy
+    __syncthreads();     // inv complete, counters dead: stage 1 joins the ring
+    fill_array(std::integral_constant<int, 1>{});
+
+    // ---- output slots: thread t owns slots t, t + 512, ... of the tile-sorted order --------------------------------
+    uint32_t gdest[kItems], srcp[kItems / 2];  // source elements packed two per register
+#pragma unroll
+    for (int k = 0; k < kItems; ++k) {
+        const int j = tid + k * kSortThreads;
+        uint32_t s = 0;
+        if (j < cnt) {
+            s = inv[j];
+            const uint32_t kj = keybuf[s];
+            gdest[k] = delta[(kj >> shift) & (kRadix - 1)] + (uint32_t)j;
+            key_out[gdest[k]] = kj;
+            if constexpr (!HAS_IDX) idx_out[gdest[k]] = (uint32_t)(tile0 + s);
+        }
+        if (k & 1) srcp[k >> 1] |= s << 16; else srcp[k >> 1] = s;
+    }
+    __syncthreads();  // the keys have been read: stage 0 is free
+    fill_array(std::integral_constant<int, 3>{});
+
+    auto move_array = [&](auto ai, const auto* /*type tag*/ tp, auto* gout) {
+        constexpr int a = decltype(ai)::value;
+        using T = std::remove_cv_t<std::remove_pointer_t<decltype(tp)>>;
+        ready(a % kRingStages, (a / kRingStages) & 1);
+        const T* sb = reinterpret_cast<const T*>(ring + (a % kRingStages) * kStageBytes);
+        T v[kItems];
+#pragma unroll
+        for (int k = 0; k < kItems; ++k) {
+            const uint32_t s = (srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
+            if (tid + k * kSortThreads < cnt) v[k] = sb[s];
+        }
+        // The stores come BEFORE the barrier on purpose: they consume the loaded values, so every shared-memory
+        // read of this stage has completed when its thread arrives.  A barrier alone does not order reads that are
+        // still in flight in the generic proxy against the bulk copy (async proxy) that refills the stage.
+#pragma unroll
+        for (int k = 0; k < kItems; ++k)
+            if (tid + k * kSortThreads < cnt) gout[gdest[k]] = v[k];
+        __syncthreads();  // the stage can take the array three places ahead
+        fill_array(std::integral_constant<int, a + kRingStages>{});
+    };
+    if constexpr (HAS_IDX) move_array(std::integral_constant<int, 1>{}, idx_in, idx_out);
+    for_each_comp<L>([&](auto ci) {
+        constexpr int C = decltype(ci)::value;
+        move_array(std::integral_constant<int, kFirstComp + C>{}, comp_ptr<L, C>(src), comp_ptr<L, C>(dst));
+    });
+}
+
 // ---- counts / offsets from the sorted keys --------------------------------------------------------------------------
 // off[c] = first sorted slot whose key is >= c, for c = 0..ncell (off[ncell] = n)
 __global__ void __launch_bounds__(256) boundaries_kernel(const uint32_t* __restrict__ sorted, int64_t n, uint32_t ncell,
@@ -446,6 +652,11 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
         SOAX_TRY(launched());
         if (ke) SOAX_TRY(sum_partials(kep, kEnergyBlocks, a.kinetic, st));
 
+        static const bool ring_ready = [] {
+            return cudaFuncSetAttribute(scatter_ring_kernel<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingSmem) == cudaSuccess &&
+                   cudaFuncSetAttribute(scatter_ring_kernel<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingSmem) == cudaSuccess;
+        }();
+        if (!ring_ready) return cuda_fail(cudaGetLastError());
         const int npass = 3 * a.log2g > kRadixBits ? 2 : 1;
         const unsigned ntiles = (unsigned)plan.ntiles, nchunks = (unsigned)plan.nchunks;
         for (int pass = 0; pass < npass; ++pass) {
@@ -465,7 +676,10 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
             SOAX_TRY(launched());
             colscan_apply_kernel<<<nchunks, kRadix, 0, st>>>(hist, (int)ntiles, partial, dbase);
             SOAX_TRY(launched());
-            if (g_tune.bin_stage)
+            if (g_tune.bin_stage == 2) {
+                if (pass == 0) scatter_ring_kernel<L, false><<<ntiles, kSortThreads, kRingSmem, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+                else scatter_ring_kernel<L, true><<<ntiles, kSortThreads, kRingSmem, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+            } else if (g_tune.bin_stage == 1)
                 scatter_staged_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
             else
                 scatter_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);

@@ -253,8 +253,16 @@ def check_bin(host_after_drift, sorted_soa, out, G):
     assert int(out["counts"].sum()) == host_after_drift["id"].shape[1]
 
 
-@pytest.mark.parametrize("n,G", [(100003, 64), (4096, 64), (4097, 8), (50000, 2), (31, 64), (1, 64), (70000, 1)])
-def test_bin_permute_matches_oracle(gpu, n, G):
+@pytest.fixture(params=[2, 1, 0], ids=["ring", "staged", "direct"])
+def bin_stage(request, gpu):
+    """every scatter variant of the counting sort (soax_tune bin_stage) must give the same unique result"""
+    gpu[1].soax_tune("bin_stage", request.param)
+    yield request.param
+    gpu[1].soax_tune("bin_stage", 2)
+
+
+@pytest.mark.parametrize("n,G", [(100003, 64), (4096, 64), (4097, 8), (50000, 2), (31, 64), (1, 64), (70000, 1), (8191, 64)])
+def test_bin_permute_matches_oracle(gpu, bin_stage, n, G):
     host = inputs.make_r1(n, seed=7)
     src_after, sorted_soa, out = run_bin(gpu, host, G)
     for name in host:                                                 # no drift requested: src is read only
@@ -263,7 +271,7 @@ def test_bin_permute_matches_oracle(gpu, n, G):
 
 
 @pytest.mark.parametrize("case", ["one_cell", "sorted", "reverse", "two_cells_far"])
-def test_bin_permute_degenerate_distributions(gpu, case):
+def test_bin_permute_degenerate_distributions(gpu, bin_stage, case):
     n, G = 20011, 64
     host = inputs.make_r1(n, seed=9)
     if case == "one_cell":
