@@ -287,6 +287,51 @@ def run_tour(torch, B, Cn) -> None:
     print(json.dumps({"tour": "done", "gpu_launches": B.soax_launch_count()}))
 
 
+def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
+    """Design study behind the counting sort (--bin-study): one 9-bit pass (G = 8, 512 bins) over 2^27 R1 particles
+    whose cell pattern is synthetic, so that the length and the sector alignment of the runs a tile writes per bin are
+    controlled; then the digit-width sweep on the real config-5 input.  Prints one JSON line per measurement."""
+    n = 1 << log2n
+    s5, d5 = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
+    device_fill(torch, s5, 7)
+    e = torch.arange(n, device="cuda", dtype=torch.int64)
+
+    def set_cells(cell):                                          # G = 8: cell = (i0*8 + i1)*8 + i2, pos at the cell centre
+        for c, i in enumerate((cell // 64, (cell // 8) % 8, cell % 8)):
+            s5.comp_view("pos", c).copy_((i.double() + 0.5) / 8.0)
+
+    g = torch.Generator(device="cuda")
+    g.manual_seed(1)
+    shuffled = torch.randperm(4096, generator=g, device="cuda")[e % 4096]
+    patterns = [
+        ("uniform random positions (runs ~Poisson(8), any alignment)", None),
+        ("exactly 8 per bin and tile, runs sector-aligned", (e // 8) % 512),
+        ("exactly 8 per bin and tile, shuffled inside the tile, runs sector-aligned", (shuffled // 8) % 512),
+        ("exactly 8 per bin and tile, every run starts 1 element past a sector boundary",
+         torch.where(e < 512, e % 512, ((e - 512) // 8) % 512)),
+        ("exactly 8 per bin and tile, every run starts 4 elements past a sector boundary",
+         torch.where(e < 2048, (e // 4) % 512, ((e - 2048) // 8) % 512)),
+        ("exactly 64 per bin and tile (64 bins used), runs sector-aligned", (e // 64) % 64),
+    ]
+    scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
+    B.soax_tune("bin_bits", 9)
+    for name, cell in patterns:
+        if cell is None:
+            for c in range(3):
+                s5.comp_view("pos", c).copy_(torch.rand(n, generator=g, device="cuda", dtype=torch.float64))
+        else:
+            set_cells(cell)
+        ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 8, scratch=scratch), 5, 2)
+        print(json.dumps({"study": "one 9-bit pass, G=8 (cell + histogram + scan + scatter + counts)", "n": n, "pattern": name, "ms": round(ms, 3)}))
+    device_fill(torch, s5, 7)
+    for bits in (9, 7, 6, 5):
+        B.soax_tune("bin_bits", bits)
+        ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), 3, 1)
+        print(json.dumps({"study": "config 5 whole pipeline vs digit width", "n": n, "bin_bits": bits,
+                          "passes": (18 + bits - 1) // bits, "ms": round(ms, 3)}))
+    B.soax_tune("bin_bits", 0)
+
+
 # ------------------------------------------------------------------------------------------------- the SoAx arm
 def run_soax(args) -> None:
     import numpy as np
@@ -312,6 +357,9 @@ def run_soax(args) -> None:
     kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
     if args.tour:
         run_tour(torch, B, Cn)
+        return
+    if args.bin_study:
+        run_bin_study(torch, B, Cn)
         return
     if args.only_extras:                                          # profiling aid: one extra config alone, no headline
         s = Cn.Soax(Cn.R1, n)
@@ -444,6 +492,7 @@ def main() -> None:
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
+    ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (run length, alignment, digit width)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     args = ap.parse_args()
     if args.impl == "reference":

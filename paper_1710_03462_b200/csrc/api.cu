@@ -275,6 +275,7 @@ int soax_tune(const char* key, int64_t value) {
     else if (!std::strcmp(key, "step_block")) { if (v < 32 || v > 512 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.step_block = v; }
     else if (!std::strcmp(key, "step_persist")) { if (v < 0 || v > 64) return SOAX_ERR_INVALID_ARG; g_tune.step_persist = v; }
     else if (!std::strcmp(key, "aos_block")) { if (v < 32 || v > 1024 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.aos_block = v; }
+    else if (!std::strcmp(key, "bin_bits")) { if (v < 0 || v > 9) return SOAX_ERR_INVALID_ARG; g_tune.bin_bits = v; }
     else if (!std::strcmp(key, "bin_stage")) { if (v < 0 || v > 2) return SOAX_ERR_INVALID_ARG; g_tune.bin_stage = v; }
     else return SOAX_ERR_INVALID_ARG;
     return SOAX_OK;

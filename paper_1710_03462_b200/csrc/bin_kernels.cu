@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(256) cell_kernel(Ptrs<L::ncomp> a, int64_t n, 
 }
 
 // ---- per-tile digit histogram -------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t* __restrict__ keys, int64_t n, int shift,
+__global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t* __restrict__ keys, int64_t n, int shift, uint32_t mask,
                                                                  uint32_t* __restrict__ hist) {
     __shared__ uint32_t h[kRadix];
     h[threadIdx.x] = 0;
@@ -93,34 +93,35 @@ __global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t*
         const uint4 a = k4[threadIdx.x], b = k4[threadIdx.x + kSortThreads];
         const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
 #pragma unroll
-        for (int k = 0; k < 8; ++k) atomicAdd(&h[(w[k] >> shift) & (kRadix - 1)], 1u);
+        for (int k = 0; k < 8; ++k) atomicAdd(&h[(w[k] >> shift) & mask], 1u);
     } else {
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             const int64_t e = tile0 + k * kSortThreads + threadIdx.x;
-            if (e < n) atomicAdd(&h[(keys[e] >> shift) & (kRadix - 1)], 1u);
+            if (e < n) atomicAdd(&h[(keys[e] >> shift) & mask], 1u);
         }
     }
     __syncthreads();
-    hist[(int64_t)blockIdx.x * kRadix + threadIdx.x] = h[threadIdx.x];
+    if (threadIdx.x <= mask) hist[(int64_t)blockIdx.x * (mask + 1) + threadIdx.x] = h[threadIdx.x];  // row of mask+1 bins
 }
 
 // ---- exclusive scan of hist[tile][digit] in (digit-major, tile-minor) order ----------------------------------------
 // phase 1: column sums of each chunk of kScanRows tiles.  Loads are issued in batches of 16 independent rows so
 // that the table streams at memory speed instead of one dependent round trip per row.
 constexpr int kScanBatch = 16;
-__global__ void __launch_bounds__(kRadix) colscan_reduce_kernel(const uint32_t* __restrict__ hist, int ntiles,
+__global__ void __launch_bounds__(kRadix) colscan_reduce_kernel(const uint32_t* __restrict__ hist, int ntiles, int nb,
                                                                 uint32_t* __restrict__ partial) {
     const int r0 = blockIdx.x * kScanRows, r1 = min(r0 + kScanRows, ntiles);
+    if ((int)threadIdx.x >= nb) return;
     uint32_t s = 0;
     for (int r = r0; r < r1; r += kScanBatch) {
         uint32_t v[kScanBatch];
 #pragma unroll
-        for (int u = 0; u < kScanBatch; ++u) v[u] = r + u < r1 ? hist[(int64_t)(r + u) * kRadix + threadIdx.x] : 0u;
+        for (int u = 0; u < kScanBatch; ++u) v[u] = r + u < r1 ? hist[(int64_t)(r + u) * nb + threadIdx.x] : 0u;
 #pragma unroll
         for (int u = 0; u < kScanBatch; ++u) s += v[u];
     }
-    partial[(int64_t)blockIdx.x * kRadix + threadIdx.x] = s;
+    partial[(int64_t)blockIdx.x * nb + threadIdx.x] = s;
 }
 // exclusive scan of one value per thread over a CTA of kRadix threads
 __device__ __forceinline__ uint32_t block_excl_scan(uint32_t x, uint32_t* sm /* >= 32 */) {
@@ -147,35 +148,38 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t x, uint32_t* sm /* 
 }
 // phase 2 (one CTA): per digit, exclusive scan of the chunk sums over chunks; then exclusive scan of the digit
 // totals over digits -> dbase[digit]
-__global__ void __launch_bounds__(kRadix) colscan_top_kernel(uint32_t* __restrict__ partial, int nchunks,
+__global__ void __launch_bounds__(kRadix) colscan_top_kernel(uint32_t* __restrict__ partial, int nchunks, int nb,
                                                              uint32_t* __restrict__ dbase) {
     __shared__ uint32_t sm[32];
+    const bool on = (int)threadIdx.x < nb;  // blockDim = max(32, nb): idle lanes still take part in the scan
     uint32_t run = 0;
-    for (int c = 0; c < nchunks; c += kScanBatch) {
+    for (int c = 0; on && c < nchunks; c += kScanBatch) {
         uint32_t v[kScanBatch];
 #pragma unroll
-        for (int u = 0; u < kScanBatch; ++u) v[u] = c + u < nchunks ? partial[(int64_t)(c + u) * kRadix + threadIdx.x] : 0u;
+        for (int u = 0; u < kScanBatch; ++u) v[u] = c + u < nchunks ? partial[(int64_t)(c + u) * nb + threadIdx.x] : 0u;
 #pragma unroll
         for (int u = 0; u < kScanBatch; ++u) {
-            if (c + u < nchunks) partial[(int64_t)(c + u) * kRadix + threadIdx.x] = run;
+            if (c + u < nchunks) partial[(int64_t)(c + u) * nb + threadIdx.x] = run;
             run += v[u];
         }
     }
-    dbase[threadIdx.x] = block_excl_scan(run, sm);
+    const uint32_t ex = block_excl_scan(run, sm);
+    if (on) dbase[threadIdx.x] = ex;
 }
 // phase 3: hist[tile][digit] <- global offset of the first item of (digit, tile)
-__global__ void __launch_bounds__(kRadix) colscan_apply_kernel(uint32_t* __restrict__ hist, int ntiles,
+__global__ void __launch_bounds__(kRadix) colscan_apply_kernel(uint32_t* __restrict__ hist, int ntiles, int nb,
                                                                const uint32_t* __restrict__ partial,
                                                                const uint32_t* __restrict__ dbase) {
     const int r0 = blockIdx.x * kScanRows, r1 = min(r0 + kScanRows, ntiles);
-    uint32_t run = dbase[threadIdx.x] + partial[(int64_t)blockIdx.x * kRadix + threadIdx.x];
+    if ((int)threadIdx.x >= nb) return;
+    uint32_t run = dbase[threadIdx.x] + partial[(int64_t)blockIdx.x * nb + threadIdx.x];
     for (int r = r0; r < r1; r += kScanBatch) {
         uint32_t v[kScanBatch];
 #pragma unroll
-        for (int u = 0; u < kScanBatch; ++u) v[u] = r + u < r1 ? hist[(int64_t)(r + u) * kRadix + threadIdx.x] : 0u;
+        for (int u = 0; u < kScanBatch; ++u) v[u] = r + u < r1 ? hist[(int64_t)(r + u) * nb + threadIdx.x] : 0u;
 #pragma unroll
         for (int u = 0; u < kScanBatch; ++u) {
-            if (r + u < r1) hist[(int64_t)(r + u) * kRadix + threadIdx.x] = run;
+            if (r + u < r1) hist[(int64_t)(r + u) * nb + threadIdx.x] = run;
             run += v[u];
         }
     }
@@ -186,7 +190,7 @@ template <class L>
 __global__ void __launch_bounds__(kSortThreads) scatter_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst,
                                                                const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
                                                                const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ idx_out,
-                                                               const uint32_t* __restrict__ base, int64_t n, int shift) {
+                                                               const uint32_t* __restrict__ base, int64_t n, int shift, uint32_t mask) {
     __shared__ uint32_t wcnt[kWarps * kRadix];  // per-warp running digit counters, then per-warp global bases
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int i = threadIdx.x; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
@@ -202,7 +206,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_kernel(Ptrs<L::ncomp> sr
         const int64_t e = e0 + k * 32;
         const bool valid = e < n;
         key[k] = valid ? key_in[e] : 0u;
-        const uint32_t d = (key[k] >> shift) & (kRadix - 1);
+        const uint32_t d = (key[k] >> shift) & mask;
         const uint32_t peers = __match_any_sync(0xffffffffu, valid ? d : (0x10000u | lane));
         const uint32_t old = mycnt[d];
         dest[k] = old + __popc(peers & lt);  // rank among the warp's earlier particles with this digit
@@ -213,7 +217,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_kernel(Ptrs<L::ncomp> sr
     __syncthreads();
     // digit d (one thread each): turn the per-warp counts into global bases, warps in order
     {
-        uint32_t run = base[(int64_t)blockIdx.x * kRadix + threadIdx.x];
+        uint32_t run = (threadIdx.x <= mask ? base[(int64_t)blockIdx.x * (mask + 1) + threadIdx.x] : 0u);
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) {
             const uint32_t c = wcnt[w * kRadix + threadIdx.x];
@@ -223,7 +227,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_kernel(Ptrs<L::ncomp> sr
     }
     __syncthreads();
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) dest[k] += mycnt[(key[k] >> shift) & (kRadix - 1)];
+    for (int k = 0; k < kItems; ++k) dest[k] += mycnt[(key[k] >> shift) & mask];
 
 #pragma unroll
     for (int k = 0; k < kItems; ++k) {
@@ -283,7 +287,7 @@ template <class L>
 __global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst,
                                                                       const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
                                                                       const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ idx_out,
-                                                                      const uint32_t* __restrict__ base, int64_t n, int shift) {
+                                                                      const uint32_t* __restrict__ base, int64_t n, int shift, uint32_t mask) {
     __shared__ __align__(16) unsigned char buf[kWarps * kRadix * 4 > kTileN * 8 ? kWarps * kRadix * 4 : kTileN * 8];
     __shared__ uint32_t delta[kRadix];  // global slot of a bin's first item minus its first slot inside the sorted tile
     __shared__ uint32_t scan_sm[32];
@@ -303,7 +307,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::nc
         const int64_t e = e0 + k * 32;
         const bool valid = e < n;
         key[k] = valid ? key_in[e] : 0u;
-        const uint32_t d = (key[k] >> shift) & (kRadix - 1);
+        const uint32_t d = (key[k] >> shift) & mask;
         const uint32_t peers = __match_any_sync(0xffffffffu, valid ? d : (0x10000u | lane));
         const uint32_t old = mycnt[d];
         lpos[k] = old + __popc(peers & lt);
@@ -317,7 +321,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::nc
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) total += wcnt[w * kRadix + threadIdx.x];
         uint32_t run = block_excl_scan(total, scan_sm);
-        delta[threadIdx.x] = base[(int64_t)blockIdx.x * kRadix + threadIdx.x] - run;
+        delta[threadIdx.x] = (threadIdx.x <= mask ? base[(int64_t)blockIdx.x * (mask + 1) + threadIdx.x] : 0u) - run;
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) {
             const uint32_t c = wcnt[w * kRadix + threadIdx.x];
@@ -327,7 +331,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::nc
     }
     __syncthreads();
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) lpos[k] += mycnt[(key[k] >> shift) & (kRadix - 1)];
+    for (int k = 0; k < kItems; ++k) lpos[k] += mycnt[(key[k] >> shift) & mask];
     __syncthreads();  // the counters are dead from here on: `buf` becomes the staging buffer
 
     // keys first: the sorted keys tell every output slot j which bin (hence which global run) it belongs to
@@ -342,7 +346,7 @@ __global__ void __launch_bounds__(kSortThreads) scatter_staged_kernel(Ptrs<L::nc
             const int j = threadIdx.x + k * kSortThreads;
             if (j < cnt) {
                 const uint32_t kj = sm[j];
-                gdest[k] = delta[(kj >> shift) & (kRadix - 1)] + (uint32_t)j;
+                gdest[k] = delta[(kj >> shift) & mask] + (uint32_t)j;
                 key_out[gdest[k]] = kj;
             }
         }
@@ -389,7 +393,7 @@ template <class L, bool HAS_IDX>
 __global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst,
                                                                       const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
                                                                       const uint32_t* __restrict__ idx_in, uint32_t* __restrict__ idx_out,
-                                                                      const uint32_t* __restrict__ base, int64_t n, int shift) {
+                                                                      const uint32_t* __restrict__ base, int64_t n, int shift, uint32_t mask) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* ring = smem;
     uint16_t* inv = reinterpret_cast<uint16_t*>(smem + kRingStages * kStageBytes);
@@ -429,7 +433,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::n
         else __syncthreads();
     };
     for (int i = tid; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
-    const uint32_t my_base = base[(int64_t)blockIdx.x * kRadix + tid];  // issued now, consumed after the ranking
+    const uint32_t my_base = (tid <= (int)mask ? base[(int64_t)blockIdx.x * (mask + 1) + tid] : 0u);  // issued now, consumed after the ranking
     __syncthreads();  // barriers initialised, counters zeroed
 
     // sequence of arrays moved by this CTA: 0 = keys, [1 = carried indices,] then the components; array a uses
@@ -463,7 +467,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::n
     for (int k = 0; k < kItems; ++k) {  // lanes holding the same digit, from kRadixBits ballots (no MATCH: its cost grows with the number of distinct values)
         const int e = e0 + k * 32;
         const bool valid = e < cnt;
-        const uint32_t d = valid ? (keybuf[e] >> shift) & (kRadix - 1) : 0u;
+        const uint32_t d = valid ? (keybuf[e] >> shift) & mask : 0u;
         uint32_t m = __ballot_sync(0xffffffffu, valid);
 #pragma unroll
         for (int b = 0; b < kRadixBits; ++b) {
@@ -501,7 +505,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::n
 #pragma unroll
     for (int k = 0; k < kItems; ++k) {
         const int e = e0 + k * 32;
-        if (e < cnt) inv[lpos[k] + mycnt[(keybuf[e] >> shift) & (kRadix - 1)]] = (uint16_t)e;
+        if (e < cnt) inv[lpos[k] + mycnt[(keybuf[e] >> shift) & mask]] = (uint16_t)e;
     }
     fence_async_smem();  // the counters (generic-proxy writes) are about to be overwritten by a bulk copy
     __syncthreads();     // inv complete, counters dead: stage 1 joins the ring
@@ -516,7 +520,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::n
         if (j < cnt) {
             s = inv[j];
             const uint32_t kj = keybuf[s];
-            gdest[k] = delta[(kj >> shift) & (kRadix - 1)] + (uint32_t)j;
+            gdest[k] = delta[(kj >> shift) & mask] + (uint32_t)j;
             key_out[gdest[k]] = kj;
             if constexpr (!HAS_IDX) idx_out[gdest[k]] = (uint32_t)(tile0 + s);
         }
@@ -577,7 +581,7 @@ __global__ void __launch_bounds__(256) counts_kernel(const uint32_t* __restrict_
 // ---- host side: scratch plan and the pipeline -------------------------------------------------------------------------
 template <class L>
 struct BinPlan {
-    size_t key0, key1, idx1, idx2, slab, hist, partial, dbase, off, ke, total;
+    size_t key0, key1, idx1, idx2, idx3, slab, hist, partial, dbase, off, ke, total;
     int64_t ntiles, nchunks;
     size_t comp_off[L::ncomp];
     BinPlan(int64_t n, int log2g) {
@@ -591,6 +595,7 @@ struct BinPlan {
         key1 = take((size_t)n * 4);
         idx1 = take((size_t)n * 4);
         idx2 = take((size_t)n * 4);
+        idx3 = take((size_t)n * 4);
         slab = o;
         for (int c = 0; c < L::ncomp; ++c) comp_off[c] = take((size_t)n * L::comp_size(c));
         hist = take((size_t)ntiles * kRadix * 4);
@@ -631,6 +636,7 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
         uint32_t* key1 = reinterpret_cast<uint32_t*>(sc + plan.key1);
         uint32_t* idx1 = reinterpret_cast<uint32_t*>(sc + plan.idx1);
         uint32_t* idx2 = a.perm ? a.perm : reinterpret_cast<uint32_t*>(sc + plan.idx2);
+        uint32_t* idx3 = reinterpret_cast<uint32_t*>(sc + plan.idx3);
         uint32_t* hist = reinterpret_cast<uint32_t*>(sc + plan.hist);
         uint32_t* partial = reinterpret_cast<uint32_t*>(sc + plan.partial);
         uint32_t* dbase = reinterpret_cast<uint32_t*>(sc + plan.dbase);
@@ -657,36 +663,50 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
                    cudaFuncSetAttribute(scatter_ring_kernel<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingSmem) == cudaSuccess;
         }();
         if (!ring_ready) return cuda_fail(cudaGetLastError());
-        const int npass = 3 * a.log2g > kRadixBits ? 2 : 1;
+        // Least-significant-digit passes over the 3*log2g key bits.  Digit width is a measured trade (profiles/): a pass
+        // with 512 bins leaves runs of ~8 elements whose ragged ends cost partial-sector read-modify-writes in L2
+        // (5.0 ms per pass at 2^27), a pass with 64 bins leaves runs of ~64 (2.2 ms), so three 6-bit passes beat two
+        // 9-bit passes.  soax_tune("bin_bits") overrides the width.
+        const int bits = 3 * a.log2g;
+        const int width = g_tune.bin_bits > 0 ? g_tune.bin_bits : 6;
+        const int npass = bits == 0 ? 1 : (bits + width - 1) / width;
         const unsigned ntiles = (unsigned)plan.ntiles, nchunks = (unsigned)plan.nchunks;
+        uint32_t* keys[2] = {key0, key1};
+        uint32_t* idxs[2] = {idx1, idx3};
+        int shift = 0;
         for (int pass = 0; pass < npass; ++pass) {
             const bool last = pass == npass - 1;
-            const uint32_t* kin = pass == 0 ? key0 : key1;
-            uint32_t* kout = pass == 0 ? key1 : key0;  // sorted keys end in key1 (1 pass) or key0 (2 passes)
-            const uint32_t* iin = pass == 0 ? nullptr : idx1;
-            uint32_t* iout = last ? idx2 : idx1;
-            const Ptrs<L::ncomp>& from = pass == 0 ? src : tmp;
-            const Ptrs<L::ncomp>& to = last ? dst : tmp;
-            const int shift = pass * kRadixBits;
-            tile_hist_kernel<<<ntiles, kSortThreads, 0, st>>>(kin, n, shift, hist);
+            const int w = (bits - shift + (npass - pass) - 1) / (npass - pass);  // balanced digit widths
+            const uint32_t mask = (1u << w) - 1u;
+            const uint32_t* kin = keys[pass & 1];
+            uint32_t* kout = keys[(pass + 1) & 1];  // sorted keys end in keys[npass & 1]
+            const uint32_t* iin = pass == 0 ? nullptr : idxs[(pass - 1) & 1];
+            uint32_t* iout = last ? idx2 : idxs[pass & 1];
+            // the last pass writes dst; before it the records alternate between the scratch slab and dst
+            const bool to_dst = ((npass - 1 - pass) & 1) == 0;
+            const Ptrs<L::ncomp>& from = pass == 0 ? src : (to_dst ? tmp : dst);
+            const Ptrs<L::ncomp>& to = to_dst ? dst : tmp;
+            tile_hist_kernel<<<ntiles, kSortThreads, 0, st>>>(kin, n, shift, mask, hist);
             SOAX_TRY(launched());
-            colscan_reduce_kernel<<<nchunks, kRadix, 0, st>>>(hist, (int)ntiles, partial);
+            const int nb = (int)mask + 1, scan_threads = nb < 32 ? 32 : nb;  // the table is [tile][nb]
+            colscan_reduce_kernel<<<nchunks, scan_threads, 0, st>>>(hist, (int)ntiles, nb, partial);
             SOAX_TRY(launched());
-            colscan_top_kernel<<<1, kRadix, 0, st>>>(partial, (int)nchunks, dbase);
+            colscan_top_kernel<<<1, scan_threads, 0, st>>>(partial, (int)nchunks, nb, dbase);
             SOAX_TRY(launched());
-            colscan_apply_kernel<<<nchunks, kRadix, 0, st>>>(hist, (int)ntiles, partial, dbase);
+            colscan_apply_kernel<<<nchunks, scan_threads, 0, st>>>(hist, (int)ntiles, nb, partial, dbase);
             SOAX_TRY(launched());
             if (g_tune.bin_stage == 2) {
-                if (pass == 0) scatter_ring_kernel<L, false><<<ntiles, kSortThreads, kRingSmem, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
-                else scatter_ring_kernel<L, true><<<ntiles, kSortThreads, kRingSmem, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+                if (pass == 0) scatter_ring_kernel<L, false><<<ntiles, kSortThreads, kRingSmem, st>>>(from, to, kin, kout, iin, iout, hist, n, shift, mask);
+                else scatter_ring_kernel<L, true><<<ntiles, kSortThreads, kRingSmem, st>>>(from, to, kin, kout, iin, iout, hist, n, shift, mask);
             } else if (g_tune.bin_stage == 1)
-                scatter_staged_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+                scatter_staged_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift, mask);
             else
-                scatter_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift);
+                scatter_kernel<L><<<ntiles, kSortThreads, 0, st>>>(from, to, kin, kout, iin, iout, hist, n, shift, mask);
             SOAX_TRY(launched());
+            shift += w;
         }
         if (a.counts || a.offsets) {
-            const uint32_t* sorted = npass == 1 ? key1 : key0;
+            const uint32_t* sorted = keys[npass & 1];
             boundaries_kernel<<<kSMs * 8, 256, 0, st>>>(sorted, n, ncell, off);
             SOAX_TRY(launched());
             counts_kernel<<<(ncell + 255) / 256, 256, 0, st>>>(off, ncell, a.counts, a.offsets);

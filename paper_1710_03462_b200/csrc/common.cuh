@@ -82,9 +82,10 @@ __device__ __forceinline__ uint32_t cell_of(double x0, double x1, double x2, dou
 }
 
 // ---- vector access: P consecutive elements of one component array per thread --------------------------------
-// sizeof(T)*P in {1,2,4,8,16,32}; 32 bytes = one LDG.E.256 / STG.E.256 (sm_100 and later only), 16 = .128.
+// sizeof(T)*P in {1,2,4,8,16,32,64}; 32 bytes = one LDG.E.256 / STG.E.256 (sm_100 and later only), 16 = .128,
+// 64 = two 256-bit accesses.
 template <class T, int P>
-struct alignas(sizeof(T) * P) Vec {
+struct alignas(sizeof(T) * P > 32 ? 32 : sizeof(T) * P) Vec {
     T v[P];
 };
 
@@ -93,7 +94,15 @@ template <class T, int P>
 __device__ __forceinline__ Vec<T, P> ld_vec(const T* p) {
     constexpr int B = sizeof(T) * P;
     Vec<T, P> r;
-    if constexpr (B == 32) {
+    if constexpr (B == 64) {
+        uint32_t* w = reinterpret_cast<uint32_t*>(&r);
+        asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]), "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7])
+                     : "l"(p));
+        asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8+32];"
+                     : "=r"(w[8]), "=r"(w[9]), "=r"(w[10]), "=r"(w[11]), "=r"(w[12]), "=r"(w[13]), "=r"(w[14]), "=r"(w[15])
+                     : "l"(p));
+    } else if constexpr (B == 32) {
         uint32_t* w = reinterpret_cast<uint32_t*>(&r);
         asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                      : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]), "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7])
@@ -113,7 +122,15 @@ __device__ __forceinline__ Vec<T, P> ld_vec(const T* p) {
 template <class T, int P>
 __device__ __forceinline__ void st_vec(T* p, const Vec<T, P>& r) {
     constexpr int B = sizeof(T) * P;
-    if constexpr (B == 32) {
+    if constexpr (B == 64) {
+        const uint32_t* w = reinterpret_cast<const uint32_t*>(&r);
+        asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                     :: "l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7])
+                     : "memory");
+        asm volatile("st.global.L1::no_allocate.v8.b32 [%0+32], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                     :: "l"(p), "r"(w[8]), "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15])
+                     : "memory");
+    } else if constexpr (B == 32) {
         const uint32_t* w = reinterpret_cast<const uint32_t*>(&r);
         asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                      :: "l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7])

@@ -19,6 +19,7 @@ struct Tuning {
     int step_persist = 0;   // 0: one CTA per tile of work; k > 0: persistent grid of k CTAs per SM
     int aos_block = 256;
     int xpose_tile = 512;   // records per transpose tile
+    int bin_bits = 0;       // digit width of the counting-sort passes: 0 = default (6), else 1..9
     int bin_stage = 2;      // 2: TMA-ring scatter (default), 1: shared-memory staged scatter, 0: direct scatter
 };
 extern Tuning g_tune;

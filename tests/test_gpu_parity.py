@@ -253,12 +253,15 @@ def check_bin(host_after_drift, sorted_soa, out, G):
     assert int(out["counts"].sum()) == host_after_drift["id"].shape[1]
 
 
-@pytest.fixture(params=[2, 1, 0], ids=["ring", "staged", "direct"])
+@pytest.fixture(params=[(2, 0), (2, 9), (2, 4), (1, 0), (0, 0)], ids=["ring", "ring-9bit", "ring-4bit", "staged", "direct"])
 def bin_stage(request, gpu):
-    """every scatter variant of the counting sort (soax_tune bin_stage) must give the same unique result"""
-    gpu[1].soax_tune("bin_stage", request.param)
+    """every scatter variant and digit width of the counting sort (soax_tune bin_stage / bin_bits) must give the
+    same unique result"""
+    gpu[1].soax_tune("bin_stage", request.param[0])
+    gpu[1].soax_tune("bin_bits", request.param[1])
     yield request.param
     gpu[1].soax_tune("bin_stage", 2)
+    gpu[1].soax_tune("bin_bits", 0)
 
 
 @pytest.mark.parametrize("n,G", [(100003, 64), (4096, 64), (4097, 8), (50000, 2), (31, 64), (1, 64), (70000, 1), (8191, 64)])
