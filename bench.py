@@ -332,8 +332,64 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
     B.soax_tune("bin_bits", 0)
 
 
+def run_paper_replica(torch, B, Cn, max_log2n: int = 27) -> None:
+    """NEXT-1 (--paper-replica): the paper's own experiment on B200 -- Eq. 1, x += dt v in float,
+    SoA of six float arrays against AoS of Particle<SIZE> = {float x[3]; float v[3]; float temp[SIZE]} (Listing 4),
+    execution time per particle and step against N (Fig. 8).  AoS kernel = one thread per record
+    (K5); `staged` = the TMA-staged best effort.  Prints one JSON line."""
+    sizes = (0, 8, 16, 32)
+    rows = []
+    for log2n in range(7, max_log2n + 1, 2):
+        n = 1 << log2n
+        reps = max(10, min(2000, (1 << 28) // n))                 # steps per timed call: ~2^28 particle-steps
+        row = {"n": n}
+        s = Cn.Soax(Cn.B6(0), n)
+        for c in range(3):
+            s.comp_view("pos", c).copy_(torch.rand(n, device="cuda"))
+            s.comp_view("vel", c).copy_(torch.randn(n, device="cuda"))
+        ms = ev_time_ms(torch, lambda: s.step(B.SOAX_STEP_EULER_NOWRAP, DT, nsteps=reps), 3, 1)
+        row["soa_ns_per_particle_step"] = ms * 1e6 / (reps * n)
+        del s
+        for S in sizes:
+            stride = 24 + 4 * S
+            aos = torch.rand(n * (6 + S), device="cuda", dtype=torch.float32).view(torch.uint8)
+            for variant, tag in ((0, f"aos{S}"), (1, f"aos{S}_staged")):
+                ms = ev_time_ms(torch, lambda: Cn.aos_step(Cn.B6(S), aos, n, B.SOAX_STEP_EULER_NOWRAP, DT, reps, variant), 3, 1)
+                row[f"{tag}_ns_per_particle_step"] = ms * 1e6 / (reps * n)
+            row[f"soa_over_aos{S}_speedup"] = row[f"aos{S}_ns_per_particle_step"] / row["soa_ns_per_particle_step"]
+            row[f"aos{S}_record_bytes"] = stride
+            del aos
+        row["footprint_MB"] = {"soa_and_aos0": n * 24 / 1e6, "aos32": n * 152 / 1e6, "l2_MB": 126}
+        rows.append(row)
+        torch.cuda.empty_cache()
+    big = rows[-1]
+    cross = [r["n"] for r in rows if r["soa_over_aos0_speedup"] > 1.0]
+    print(json.dumps({
+        "experiment": "paper replica (Fig. 8): float x += dt*v, SoA (6 float arrays) vs AoS Particle<SIZE>, ns per particle-step",
+        "paper_gpu_claims": {"hardware": "Tesla M2050 (Fermi), CUDA 7.0", "soa_over_aos0_large_n": "~2x", "soa_over_aos32_large_n": "~20x",
+                             "aos_faster_below_n": "~2000", "cite": "PAPER.md:231-241"},
+        "b200_large_n": {"n": big["n"], **{f"soa_over_aos{S}": big[f"soa_over_aos{S}_speedup"] for S in sizes},
+                         "algorithmic_bytes_per_particle_step": 36,   # Eq. 1: two loads and one store per component (PAPER.md:138)
+                         "soa_GBps": 36.0 / big["soa_ns_per_particle_step"],
+                         **{f"aos{S}_GBps_useful": 36.0 / big[f"aos{S}_ns_per_particle_step"] for S in sizes}},
+        "soa_faster_than_aos0_from_n": min(cross) if cross else None,
+        "rows": rows, "gpu_launches": B.soax_launch_count()}))
+
+
 # ------------------------------------------------------------------------------------------------- the SoAx arm
 def run_soax(args) -> None:
+    """Everything runs on a side stream (not the legacy default stream), so that soax_step can replay its captured
+    graph of nsteps launches; CUDA events are recorded on that same stream."""
+    import torch
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the SoAx path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        _run_soax(args)
+
+
+def _run_soax(args) -> None:
     import numpy as np
     import torch
     import torch.distributed as dist
@@ -360,6 +416,9 @@ def run_soax(args) -> None:
         return
     if args.bin_study:
         run_bin_study(torch, B, Cn)
+        return
+    if args.paper_replica:
+        run_paper_replica(torch, B, Cn)
         return
     if args.only_extras:                                          # profiling aid: one extra config alone, no headline
         s = Cn.Soax(Cn.R1, n)
@@ -492,6 +551,7 @@ def main() -> None:
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
+    ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
     ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (run length, alignment, digit width)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     args = ap.parse_args()

@@ -134,14 +134,19 @@ typedef struct {
     double center; /* centre of the harmonic well (configs: 0.5) */
 } soax_step_params;
 
-/* nsteps passes over the n live particles of `s`, in place.  Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+/* nsteps passes over the n live particles of `s`, in place.  Errors: INVALID_ARG, UNSUPPORTED, CUDA.
+ * With nsteps >= 2 on a capturable stream (any stream but the legacy default stream, not itself being captured)
+ * the nsteps launches are captured once into a CUDA graph kept with the container and replayed by later identical
+ * calls: the same kernels and passes, without a host round trip per step (what a launch-bound, L2-resident
+ * particle set such as config 1 needs).  On the legacy default stream the launches are issued one by one. */
 int soax_step(soax_t* s, const soax_step_params* params, int32_t nsteps, void* stream);
 
 /* a5: the same arithmetic on an Array of Structures (packed image of `layout`, see soax_layout_aos), kept as
  * the in-library comparison baseline (thread per particle, strided access).  variant 0 = the
  * paper-faithful kernel (one thread per record, direct strided field access); variant 1 = best effort
  * (whole records staged through shared memory with coalesced 128-bit accesses).  dev_aos: n records,
- * 16-byte aligned.  Kinds DRIFT and SYMPLECTIC_EULER_HARMONIC. */
+ * 16-byte aligned.  Kinds DRIFT, SYMPLECTIC_EULER_HARMONIC and EULER_NOWRAP (the last also on the paper's float
+ * record B6_S = Particle<SIZE>: the B200 re-run of Fig. 8). */
 int soax_step_aos(const soax_layout* layout, void* dev_aos, int64_t n, const soax_step_params* params,
                   int32_t nsteps, int32_t variant, void* stream);
 

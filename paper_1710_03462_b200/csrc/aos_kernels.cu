@@ -77,6 +77,19 @@ __device__ __forceinline__ void st_field(unsigned char* rec, int k, typename L::
 template <class L, int KIND>
 __device__ __forceinline__ void step_record(unsigned char* rec, double dt, double k, double ctr) {
     using V = typename L::template type_of<vel_tag>;
+    if constexpr (KIND == SOAX_STEP_EULER_NOWRAP) {
+        // Eq. 1 as printed on the paper's own record (Listing 4): x_c += dt v_c, one
+        // fma in the type of pos, no wrap; temp[SIZE] rides along untouched -- that is the whole point of Fig. 8.
+        using X = typename L::template type_of<pos_tag>;
+        const X dt_x = (X)dt;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const X x = ld_field<L, pos_tag>(rec, d);
+            const V v = ld_field<L, vel_tag>(rec, d);
+            st_field<L, pos_tag>(rec, d, fma_t(dt_x, (X)v, x));
+        }
+        return;
+    }
     const V dt_v = (V)dt;  // (float)dt rounds to nearest: dt_f of the contract
     double x[3];
     V v[3];
@@ -234,8 +247,11 @@ constexpr int tile_ctas_per_sm() {
 
 template <class L, int KIND>
 static int step_aos_kind(void* aos, int64_t n, const soax_step_params* p, int variant, cudaStream_t st) {
-    constexpr bool ok = L::template has_as<pos_tag, double, 3>() &&
-                        (L::template has_as<vel_tag, float, 3>() || L::template has_as<vel_tag, double, 3>());
+    constexpr bool wrapped = L::template has_as<pos_tag, double, 3>() &&
+                             (L::template has_as<vel_tag, float, 3>() || L::template has_as<vel_tag, double, 3>());
+    constexpr bool plain = (L::template has_as<pos_tag, double, 3>() || L::template has_as<pos_tag, float, 3>()) &&
+                           (L::template has_as<vel_tag, float, 3>() || L::template has_as<vel_tag, double, 3>());
+    constexpr bool ok = KIND == SOAX_STEP_EULER_NOWRAP ? plain : wrapped;
     if constexpr (!ok) {
         return SOAX_ERR_UNSUPPORTED;
     } else {
@@ -259,8 +275,8 @@ int step_aos_entry(void* aos, int64_t n, const soax_step_params* p, int variant,
     switch (p->kind) {
         case SOAX_STEP_DRIFT: return step_aos_kind<L, SOAX_STEP_DRIFT>(aos, n, p, variant, st);
         case SOAX_STEP_SYMPLECTIC_EULER_HARMONIC: return step_aos_kind<L, SOAX_STEP_SYMPLECTIC_EULER_HARMONIC>(aos, n, p, variant, st);
-        case SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED:
-        case SOAX_STEP_EULER_NOWRAP: return SOAX_ERR_UNSUPPORTED;
+        case SOAX_STEP_EULER_NOWRAP: return step_aos_kind<L, SOAX_STEP_EULER_NOWRAP>(aos, n, p, variant, st);
+        case SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED: return SOAX_ERR_UNSUPPORTED;
         default: return SOAX_ERR_INVALID_ARG;
     }
 }

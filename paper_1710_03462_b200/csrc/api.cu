@@ -31,10 +31,22 @@ struct soax_layout {
     size_t (*bin_scratch)(int64_t, int);
 };
 
+// A captured `nsteps`-launch step loop, kept with the container and replayed while the call is the same: small
+// (L2-resident) particle sets are launch-bound, and a graph replays its kernel nodes back to back without a host
+// round trip per step.  Still one kernel launch and one full memory pass per step (Q14).
+struct StepGraph {
+    cudaGraphExec_t exec = nullptr;
+    soax_step_params params{};
+    int32_t nsteps = 0;
+    int64_t n = 0;
+    Tuning tune{};
+};
+
 struct soax_container {
     const soax_layout* layout;
     int64_t n, capacity;
     void* comp[kMaxComp];
+    StepGraph graph;
 };
 
 namespace {
@@ -156,6 +168,7 @@ int soax_alloc(const soax_layout* l, int64_t n, int64_t capacity, void* dev_slab
 
 int soax_free(soax_t* s) {
     if (!s) return SOAX_ERR_INVALID_ARG;
+    if (s->graph.exec) cudaGraphExecDestroy(s->graph.exec);
     delete s;
     return SOAX_OK;
 }
@@ -196,14 +209,78 @@ int soax_download(const soax_t* s, void* const* host_comps, int64_t n, void* str
 
 int soax_step(soax_t* s, const soax_step_params* p, int32_t nsteps, void* stream) {
     if (!s || !p || nsteps < 0) return SOAX_ERR_INVALID_ARG;
-    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(s->layout->step(s->comp, s->n, p, (cudaStream_t)stream));
+    cudaStream_t st = (cudaStream_t)stream;
+    // Graph replay needs a capturable stream (not the legacy default stream) that is not already being captured.
+    bool use_graph = g_tune.step_graph && nsteps >= 2 && s->n > 0 && st != nullptr && st != cudaStreamLegacy;
+    if (use_graph) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+    }
+    if (use_graph) {
+        StepGraph& g = s->graph;
+        const bool same = g.exec && g.nsteps == nsteps && g.n == s->n && std::memcmp(&g.params, p, sizeof(*p)) == 0 &&
+                          std::memcmp(&g.tune, &g_tune, sizeof(Tuning)) == 0;
+        if (!same) {
+            if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                int rc = SOAX_OK;
+                for (int32_t i = 0; i < nsteps && rc == SOAX_OK; ++i) rc = s->layout->step(s->comp, s->n, p, st);
+                const cudaError_t e = cudaStreamEndCapture(st, &graph);
+                if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+                if (e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) g.exec = nullptr;
+                if (graph) cudaGraphDestroy(graph);
+            }
+            cudaGetLastError();
+            if (g.exec) { std::memcpy(&g.params, p, sizeof(*p)); g.nsteps = nsteps; g.n = s->n; g.tune = g_tune; }
+        } else {
+            g_launches.fetch_add(nsteps, std::memory_order_relaxed);  // the replay launches the same nsteps kernels
+        }
+        if (g.exec) { SOAX_CUDA(cudaGraphLaunch(g.exec, st)); return SOAX_OK; }
+    }
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(s->layout->step(s->comp, s->n, p, st));
     return SOAX_OK;
 }
 
 int soax_step_aos(const soax_layout* l, void* dev_aos, int64_t n, const soax_step_params* p, int32_t nsteps,
                   int32_t variant, void* stream) {
     if (!l || !p || nsteps < 0 || n < 0 || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
-    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(l->step_aos(dev_aos, n, p, variant, (cudaStream_t)stream));
+    cudaStream_t st = (cudaStream_t)stream;
+    // Same graph replay as soax_step, so that the AoS baseline is timed under the same launch mechanism as the SoA
+    // path.  There is no container to keep the graph with: one entry per host thread, keyed by the whole call.
+    struct AosGraph : StepGraph { const soax_layout* layout = nullptr; void* aos = nullptr; int32_t variant = 0;
+                                  ~AosGraph() { /* the context may be gone at thread exit: leak the exec */ } };
+    static thread_local AosGraph g;
+    bool use_graph = g_tune.step_graph && nsteps >= 2 && n > 0 && st != nullptr && st != cudaStreamLegacy;
+    if (use_graph) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+    }
+    if (use_graph) {
+        const bool same = g.exec && g.layout == l && g.aos == dev_aos && g.variant == variant && g.nsteps == nsteps && g.n == n &&
+                          std::memcmp(&g.params, p, sizeof(*p)) == 0 && std::memcmp(&g.tune, &g_tune, sizeof(Tuning)) == 0;
+        if (!same) {
+            if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                int rc = SOAX_OK;
+                for (int32_t i = 0; i < nsteps && rc == SOAX_OK; ++i) rc = l->step_aos(dev_aos, n, p, variant, st);
+                const cudaError_t e = cudaStreamEndCapture(st, &graph);
+                if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+                if (e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) g.exec = nullptr;
+                if (graph) cudaGraphDestroy(graph);
+            }
+            cudaGetLastError();
+            if (g.exec) {
+                std::memcpy(&g.params, p, sizeof(*p));
+                g.nsteps = nsteps; g.n = n; g.tune = g_tune; g.layout = l; g.aos = dev_aos; g.variant = variant;
+            }
+        } else {
+            g_launches.fetch_add(nsteps, std::memory_order_relaxed);
+        }
+        if (g.exec) { SOAX_CUDA(cudaGraphLaunch(g.exec, st)); return SOAX_OK; }
+    }
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(l->step_aos(dev_aos, n, p, variant, st));
     return SOAX_OK;
 }
 
@@ -275,6 +352,7 @@ int soax_tune(const char* key, int64_t value) {
     else if (!std::strcmp(key, "step_block")) { if (v < 32 || v > 512 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.step_block = v; }
     else if (!std::strcmp(key, "step_persist")) { if (v < 0 || v > 64) return SOAX_ERR_INVALID_ARG; g_tune.step_persist = v; }
     else if (!std::strcmp(key, "aos_block")) { if (v < 32 || v > 1024 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.aos_block = v; }
+    else if (!std::strcmp(key, "step_graph")) { if (v < 0 || v > 1) return SOAX_ERR_INVALID_ARG; g_tune.step_graph = v; }
     else if (!std::strcmp(key, "bin_bits")) { if (v < 0 || v > 9) return SOAX_ERR_INVALID_ARG; g_tune.bin_bits = v; }
     else if (!std::strcmp(key, "bin_stage")) { if (v < 0 || v > 2) return SOAX_ERR_INVALID_ARG; g_tune.bin_stage = v; }
     else return SOAX_ERR_INVALID_ARG;

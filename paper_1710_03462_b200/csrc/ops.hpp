@@ -17,6 +17,7 @@ struct Tuning {
     int step_ppt = 4;       // particles per thread in the SoA step kernels: 1, 2 or 4
     int step_block = 256;   // threads per CTA
     int step_persist = 0;   // 0: one CTA per tile of work; k > 0: persistent grid of k CTAs per SM
+    int step_graph = 1;     // 1: soax_step(nsteps >= 2) on a capturable stream replays a captured graph of nsteps launches
     int aos_block = 256;
     int xpose_tile = 512;   // records per transpose tile
     int bin_bits = 0;       // digit width of the counting-sort passes: 0 = default (6), else 1..9

@@ -326,6 +326,62 @@ def test_paper_float_benchmark_euler(gpu, size_extra):
     assert np.array_equal(bits(got["pos"]), bits(epos)) and np.array_equal(bits(got["vel"]), bits(evel))
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("size_extra,n", [(0, 10001), (8, 4099), (32, 777)])
+def test_paper_float_benchmark_aos_kernels(gpu, size_extra, n, variant):
+    """K5 on the paper's own record Particle<SIZE> (Listing 4): both AoS kernels equal the oracle
+    bitwise, leave v and temp[SIZE] untouched, and equal the SoA kernel (same operation sequence)."""
+    torch, B, Cn = gpu
+    host = inputs.make_b6(n, seed=2)
+    rec = np.zeros((n, 6 + size_extra), np.float32)
+    rec[:, 0:3], rec[:, 3:6] = host["pos"].T, host["vel"].T
+    rec[:, 6:] = np.arange(n * size_extra, dtype=np.float32).reshape(n, size_extra)
+    stride, offs = B.soax_layout_aos(B.soax_layout_define(Cn.B6(size_extra)), True)
+    assert stride == 24 + 4 * size_extra and list(offs[:6]) == [0, 4, 8, 12, 16, 20]      # PAPER.md:237: 24 bytes at SIZE=0
+    aos = torch.from_numpy(rec.view(np.uint8).reshape(-1).copy()).cuda()
+    Cn.aos_step(Cn.B6(size_extra), aos, n, B.SOAX_STEP_EULER_NOWRAP, 1e-3, 5, variant)
+    got = aos.cpu().numpy().view(np.float32).reshape(n, 6 + size_extra)
+    epos, evel = oracle.b6_euler(host["pos"], host["vel"], size_extra, np.float32(1e-3), 5)
+    assert np.array_equal(bits(got[:, 0:3].T), bits(epos))
+    assert np.array_equal(bits(got[:, 3:6].T), bits(evel))
+    assert np.array_equal(got[:, 6:], rec[:, 6:])
+    full = dict(host)
+    if size_extra:
+        full["temp"] = np.ascontiguousarray(rec[:, 6:].T)
+    s = to_device(Cn, Cn.B6(size_extra), full)
+    s.step(B.SOAX_STEP_EULER_NOWRAP, 1e-3, nsteps=5)
+    assert np.array_equal(s.to_aos().cpu().numpy(), got.view(np.uint8).reshape(-1))
+
+
+# ------------------------------------------------------------------------------- graph replay of the step loop
+def test_step_graph_replay_on_side_stream(gpu):
+    """soax_step(nsteps >= 2) on a capturable stream replays a captured graph: same bits as the oracle, also when the
+    call is repeated (replay), when its parameters change (re-capture) and after a resize."""
+    torch, B, Cn = gpu
+    n = 30011
+    host = inputs.make_r1(n, seed=5)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = to_device(Cn, Cn.R1, host)
+        l0 = B.soax_launch_count()
+        s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=7)      # capture + launch
+        s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=7)      # replay
+        s.step(B.SOAX_STEP_DRIFT, DT, nsteps=3)                          # other parameters: re-capture
+        s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, 2 * DT, nsteps=7)
+        assert B.soax_launch_count() - l0 == 7 + 7 + 3 + 7
+        torch.cuda.current_stream().synchronize()
+        exp = oracle.symplectic_euler(oracle.drift(oracle.symplectic_euler(host, DT, 14), DT, 3), 2 * DT, 7)
+        check_r1(s.download(), exp)
+        B.soax_resize(s.handle, 1000)                                    # fewer live particles: the old graph must not run
+        s.step(B.SOAX_STEP_DRIFT, DT, nsteps=3)
+        torch.cuda.current_stream().synchronize()
+        B.soax_resize(s.handle, n)
+        got = s.download()
+        exp2 = oracle.drift(inputs.take(exp, np.arange(1000)), DT, 3)
+        for name in exp2:
+            assert np.array_equal(bits(got[name][:, :1000]), bits(exp2[name])), name
+            assert np.array_equal(bits(got[name][:, 1000:]), bits(exp[name][:, 1000:])), name
+
+
 # ------------------------------------------------------------------------------------------- error behaviour
 def test_error_codes(gpu):
     torch, B, Cn = gpu
