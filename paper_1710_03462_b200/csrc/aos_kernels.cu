@@ -231,6 +231,126 @@ __global__ void __launch_bounds__(kTile) soa_to_aos_kernel(Ptrs<L::ncomp> a, uns
     }
 }
 
+// ---- a6 / a7, pipelined (default): a persistent CTA walks its tiles with a ring of NS shared-memory stages --------
+// A stage holds R*kTile records.  AoS -> SoA: the bulk copy of the tile NS-1 places ahead is in flight while the
+// current one is read out of shared memory (each thread takes records t, t+256, ... so that every warp reads
+// neighbouring records -- 2-way bank conflicts at a 40-byte stride -- and writes 128/256 contiguous bytes per
+// component array).  SoA -> AoS: all R*ncomp global loads of a thread are issued first (R*40 bytes in flight per
+// thread for R1), then the records are assembled in the stage and leave as ONE bulk store whose read of shared
+// memory overlaps the loads of the next tile.  Records behind the last full tile go straight between the two
+// global images, piece by piece.
+template <class L, int R, int NS> constexpr int ring_smem() { return NS * R * kTile * L::aos_stride + 64; }
+
+template <class L>
+__device__ __forceinline__ void tail_aos_to_soa(const Ptrs<L::ncomp>& a, const unsigned char* aos, int64_t from, int64_t n) {
+    for (int64_t i = from + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const unsigned char* rec = aos + i * L::aos_stride;
+        for_each_comp<L>([&](auto ci) {
+            constexpr int C = decltype(ci)::value;
+            using T = typename L::template comp_type<C>;
+            comp_ptr<L, C>(a)[i] = ld_piecewise<T, comp_align<L, C>()>(rec + L::aos_offset(C));
+        });
+    }
+}
+template <class L>
+__device__ __forceinline__ void tail_soa_to_aos(const Ptrs<L::ncomp>& a, unsigned char* aos, int64_t from, int64_t n) {
+    for (int64_t i = from + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        unsigned char* rec = aos + i * L::aos_stride;
+        for_each_comp<L>([&](auto ci) {
+            constexpr int C = decltype(ci)::value;
+            using T = typename L::template comp_type<C>;
+            st_piecewise<T, comp_align<L, C>()>(rec + L::aos_offset(C), comp_ptr<L, C>(a)[i]);
+        });
+    }
+}
+
+template <class L, int R, int NS>
+__global__ void __launch_bounds__(kTile) aos_to_soa_ring_kernel(Ptrs<L::ncomp> a, const unsigned char* aos, int64_t n) {
+    constexpr int SB = R * kTile * L::aos_stride, TILE = R * kTile, S = L::aos_stride;
+    extern __shared__ __align__(128) unsigned char sm[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(sm + NS * SB);
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int64_t nfull = n / TILE;
+    const int64_t mine = nfull > blockIdx.x ? (nfull - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;  // tiles of this CTA
+    auto issue = [&](int64_t k) {  // thread 0: start the bulk copy of this CTA's k-th tile into stage k % NS
+        const int64_t t = blockIdx.x + k * gridDim.x;
+        mbar_expect_tx(&full[k % NS], SB);
+        bulk_g2s(sm + (k % NS) * SB, aos + t * (int64_t)TILE * S, SB, &full[k % NS]);
+    };
+    if (tid == 0)
+        for (int64_t k = 0; k < NS - 1 && k < mine; ++k) issue(k);
+    for (int64_t k = 0; k < mine; ++k) {
+        // stage (k-1) % NS was read in the previous iteration; its reads completed before the barrier that ended it
+        if (tid == 0 && k + NS - 1 < mine) issue(k + NS - 1);
+        mbar_wait(&full[k % NS], (uint32_t)((k / NS) & 1));
+        const unsigned char* st = sm + (k % NS) * SB;
+        const int64_t t0 = (blockIdx.x + k * gridDim.x) * (int64_t)TILE;
+        for_each_comp<L>([&](auto ci) {
+            constexpr int C = decltype(ci)::value;
+            using T = typename L::template comp_type<C>;
+            T v[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) v[r] = ld_piecewise<T, comp_align<L, C>()>(st + (tid + r * kTile) * S + L::aos_offset(C));
+#pragma unroll
+            for (int r = 0; r < R; ++r) comp_ptr<L, C>(a)[t0 + tid + r * kTile] = v[r];  // consumes the reads before the barrier
+        });
+        __syncthreads();
+    }
+    tail_aos_to_soa<L>(a, aos, nfull * TILE, n);
+}
+
+template <class L, int R, int NS>
+__global__ void __launch_bounds__(kTile) soa_to_aos_ring_kernel(Ptrs<L::ncomp> a, unsigned char* aos, int64_t n) {
+    constexpr int SB = R * kTile * L::aos_stride, TILE = R * kTile, S = L::aos_stride;
+    extern __shared__ __align__(128) unsigned char sm[];
+    const int tid = threadIdx.x;
+    const int64_t nfull = n / TILE;
+    const int64_t mine = nfull > blockIdx.x ? (nfull - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    for (int64_t k = 0; k < mine; ++k) {
+        unsigned char* st = sm + (k % NS) * SB;
+        const int64_t t0 = (blockIdx.x + k * gridDim.x) * (int64_t)TILE;
+        // the bulk store that last read this stage was committed NS iterations ago: at most NS-1 younger ones may be pending
+        if (tid == 0 && k >= NS) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(NS - 1) : "memory");
+        __syncthreads();
+        // every global load of the thread is issued before the first shared-memory store (bit images in registers)
+        unsigned long long v[L::ncomp][R];
+        for_each_comp<L>([&](auto ci) {
+            constexpr int C = decltype(ci)::value;
+            using T = typename L::template comp_type<C>;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const T x = ld_vec<T, 1>(comp_ptr<L, C>(a) + t0 + tid + r * kTile).v[0];
+                v[C][r] = 0;
+                memcpy(&v[C][r], &x, sizeof(T));
+            }
+        });
+        for_each_comp<L>([&](auto ci) {
+            constexpr int C = decltype(ci)::value;
+            using T = typename L::template comp_type<C>;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                T x;
+                memcpy(&x, &v[C][r], sizeof(T));
+                st_piecewise<T, comp_align<L, C>()>(st + (tid + r * kTile) * S + L::aos_offset(C), x);
+            }
+        });
+        fence_async_smem();
+        __syncthreads();
+        if (tid == 0) {
+            bulk_s2g(aos + t0 * S, st, SB);
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait_read();  // shared memory must outlive the last bulk stores' reads
+    tail_soa_to_aos<L>(a, aos, nfull * TILE, n);
+}
+
 // ---- host side -----------------------------------------------------------------------------------------------------
 template <class L>
 static unsigned tile_grid(int64_t n, int ctas_per_sm) {
@@ -281,14 +401,60 @@ int step_aos_entry(void* aos, int64_t n, const soax_step_params* p, int variant,
     }
 }
 
+template <class L, int R, int NS>
+static unsigned ring_grid(int64_t n) {
+    constexpr int by_smem = (220 * 1024) / ring_smem<L, R, NS>();
+    constexpr int per_sm = by_smem < 8 ? by_smem : 8;
+    const int64_t ntiles = n / (R * kTile);
+    const int64_t cap = (int64_t)kSMs * (g_tune.xpose_ctas > 0 && g_tune.xpose_ctas < per_sm ? g_tune.xpose_ctas : per_sm);
+    return (unsigned)(ntiles < cap ? (ntiles < 1 ? 1 : ntiles) : cap);
+}
+template <class L, int R, int NS>
+static int launch_a2s(void* const* comps, const void* aos, int64_t n, cudaStream_t st) {
+    if constexpr (ring_smem<L, R, NS>() > 220 * 1024) return SOAX_ERR_UNSUPPORTED;
+    else {
+        static const bool ready = cudaFuncSetAttribute(aos_to_soa_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()) == cudaSuccess;
+        if (!ready) return cuda_fail(cudaGetLastError());
+        aos_to_soa_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
+        return launched();
+    }
+}
+template <class L, int R, int NS>
+static int launch_s2a(void* const* comps, void* aos, int64_t n, cudaStream_t st) {
+    if constexpr (ring_smem<L, R, NS>() > 220 * 1024) return SOAX_ERR_UNSUPPORTED;
+    else {
+        static const bool ready = cudaFuncSetAttribute(soa_to_aos_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()) == cudaSuccess;
+        if (!ready) return cuda_fail(cudaGetLastError());
+        soa_to_aos_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
+        return launched();
+    }
+}
+// Measured on B200: every shape plateaus at 6.0-6.1 TB/s for R1 -- an out-of-place copy with 1 + ncomp
+// streams -- so the defaults are simply the best per direction: AoS->SoA likes big bulk copies (4 x 256 records per
+// stage, one stage, several CTAs per SM), SoA->AoS likes 2 x 256 (80 bytes of loads in flight per thread for R1).
+// soax_tune("xpose_r"/"xpose_ns") override both directions for sweeps.
+#define SOAX_RING_SWITCH(FN, DEFAULT_R, ...)                                                        \
+    {                                                                                               \
+        int r_ = g_tune.xpose_r > 0 ? g_tune.xpose_r : DEFAULT_R;                                   \
+        const int ns_ = g_tune.xpose_ns > 0 ? g_tune.xpose_ns : 1;                                  \
+        while (r_ > 1 && ns_ * r_ * kTile * L::aos_stride + 64 > 110 * 1024) r_ >>= 1; /* two CTAs per SM at least */ \
+        switch (r_ * 10 + ns_) {                                                                    \
+            case 11: return FN<L, 1, 1>(__VA_ARGS__); case 12: return FN<L, 1, 2>(__VA_ARGS__);     \
+            case 21: return FN<L, 2, 1>(__VA_ARGS__); case 22: return FN<L, 2, 2>(__VA_ARGS__);     \
+            case 41: return FN<L, 4, 1>(__VA_ARGS__); case 42: return FN<L, 4, 2>(__VA_ARGS__);     \
+            default: return SOAX_ERR_INVALID_ARG;                                                   \
+        }                                                                                           \
+    }
 template <class L>
 int aos_to_soa_entry(void* const* comps, const void* aos, int64_t n, cudaStream_t st) {
+    if (g_tune.xpose_ring) SOAX_RING_SWITCH(launch_a2s, 4, comps, aos, n, st)
     constexpr int smem = kTile * L::aos_stride;
     aos_to_soa_kernel<L><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
     return launched();
 }
 template <class L>
 int soa_to_aos_entry(void* const* comps, void* aos, int64_t n, cudaStream_t st) {
+    if (g_tune.xpose_ring) SOAX_RING_SWITCH(launch_s2a, 2, comps, aos, n, st)
     constexpr int smem = kTile * L::aos_stride;
     soa_to_aos_kernel<L><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
     return launched();

@@ -353,6 +353,10 @@ int soax_tune(const char* key, int64_t value) {
     else if (!std::strcmp(key, "step_persist")) { if (v < 0 || v > 64) return SOAX_ERR_INVALID_ARG; g_tune.step_persist = v; }
     else if (!std::strcmp(key, "aos_block")) { if (v < 32 || v > 1024 || v % 32) return SOAX_ERR_INVALID_ARG; g_tune.aos_block = v; }
     else if (!std::strcmp(key, "step_graph")) { if (v < 0 || v > 1) return SOAX_ERR_INVALID_ARG; g_tune.step_graph = v; }
+    else if (!std::strcmp(key, "xpose_ring")) { if (v < 0 || v > 1) return SOAX_ERR_INVALID_ARG; g_tune.xpose_ring = v; }
+    else if (!std::strcmp(key, "xpose_r")) { if (v != 0 && v != 1 && v != 2 && v != 4) return SOAX_ERR_INVALID_ARG; g_tune.xpose_r = v; }
+    else if (!std::strcmp(key, "xpose_ns")) { if (v < 0 || v > 2) return SOAX_ERR_INVALID_ARG; g_tune.xpose_ns = v; }
+    else if (!std::strcmp(key, "xpose_ctas")) { if (v < 0 || v > 8) return SOAX_ERR_INVALID_ARG; g_tune.xpose_ctas = v; }
     else if (!std::strcmp(key, "bin_bits")) { if (v < 0 || v > 9) return SOAX_ERR_INVALID_ARG; g_tune.bin_bits = v; }
     else if (!std::strcmp(key, "bin_stage")) { if (v < 0 || v > 2) return SOAX_ERR_INVALID_ARG; g_tune.bin_stage = v; }
     else return SOAX_ERR_INVALID_ARG;

@@ -19,7 +19,8 @@ struct Tuning {
     int step_persist = 0;   // 0: one CTA per tile of work; k > 0: persistent grid of k CTAs per SM
     int step_graph = 1;     // 1: soax_step(nsteps >= 2) on a capturable stream replays a captured graph of nsteps launches
     int aos_block = 256;
-    int xpose_tile = 512;   // records per transpose tile
+    int xpose_ring = 1;     // 1: pipelined ring transposes (default), 0: one tile per CTA visit
+    int xpose_r = 0, xpose_ns = 0, xpose_ctas = 0;  // ring shape override: 256*r records per stage, ns stages, CTAs per SM cap (0 = default)
     int bin_bits = 0;       // digit width of the counting-sort passes: 0 = default (6), else 1..9
     int bin_stage = 2;      // 2: TMA-ring scatter (default), 1: shared-memory staged scatter, 0: direct scatter
 };

@@ -131,19 +131,29 @@ def test_energy_hand_fixture_on_gpu(gpu):
 
 
 # ------------------------------------------------------------------------------- a5, a6, a7: AoS (config 3)
-@pytest.mark.parametrize("n", [1 << 16, 70001, 255, 1])
-def test_aos_soa_transposes_byte_exact(gpu, n):
+# shape = (xpose_ring, xpose_r, xpose_ns, xpose_ctas): the default ring transposes, the one-tile-per-visit kernels they
+# replaced, and ring shapes forced deep (two stages, one CTA per SM: every CTA walks many tiles) at a size with a tail
+@pytest.mark.parametrize("n,shape", [(1 << 16, (1, 0, 0, 0)), (70001, (1, 0, 0, 0)), (255, (1, 0, 0, 0)), (1, (1, 0, 0, 0)),
+                                     (70001, (0, 0, 0, 0)), (255, (0, 0, 0, 0)),
+                                     (1024 * 700 + 13, (1, 1, 2, 1)), (1024 * 700 + 13, (1, 4, 2, 1)), (1024 * 700 + 13, (1, 2, 1, 1))])
+def test_aos_soa_transposes_byte_exact(gpu, n, shape):
     torch, B, Cn = gpu
     rng = np.random.default_rng(n)
     raw = rng.integers(0, 256, 40 * n, dtype=np.uint8)                # arbitrary bytes: NaN payloads, denormals, ...
     aos = torch.from_numpy(raw).cuda()
     s = Cn.Soax(Cn.R1, n)
-    s.from_aos(aos, n)
-    got = s.download()
+    try:
+        for key, v in zip(("xpose_ring", "xpose_r", "xpose_ns", "xpose_ctas"), shape):
+            B.soax_tune(key, v)
+        s.from_aos(aos, n)
+        got = s.download()
+        back = s.to_aos()
+    finally:
+        for key, v in (("xpose_ring", 1), ("xpose_r", 0), ("xpose_ns", 0), ("xpose_ctas", 0)):
+            B.soax_tune(key, v)
     exp = oracle.r1_aos_to_soa(raw)
     for name in exp:
         assert np.array_equal(bits(got[name]), bits(exp[name])), name
-    back = s.to_aos()
     assert np.array_equal(back.cpu().numpy(), raw)                    # round trip is byte exact
     assert np.array_equal(oracle.r1_soa_to_aos(exp), raw)
 
