@@ -175,7 +175,7 @@ def device_fill(torch, s, seed: int) -> None:
         s.comp_view("flags").copy_(torch.randint(0, 256, (n,), generator=g, device="cuda", dtype=torch.uint8))
 
 
-def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5"), iters: int = 3) -> dict:
+def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5", "expr"), iters: int = 3) -> dict:
     """The other section-8(a) rows, each timed alone with CUDA events (N=1, rank 0): reported beside the headline."""
     ex = {}
     n = s.n
@@ -190,7 +190,34 @@ def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config
         _extra_config4(torch, B, Cn, peak, ex, gbs, iters)
     if "config5" in which:
         _extra_config5(torch, B, Cn, peak, ex, gbs, iters)
+    if "expr" in which:
+        _extra_expr(torch, B, Cn, s, peak, ex, gbs)
     return ex
+
+
+SE_PROGRAM = "vel = fma(float(dt), float(-(k*(pos - 0.5))), vel); pos = wrap(fma(dt, double(vel), pos))"
+
+
+def _extra_expr(torch, B, Cn, s, peak, ex, gbs):
+    """NEXT-2, the B200 form of the paper's Fig. 11 ("SoAx == hand-written SoA"): the symplectic-Euler step
+    written by the user as program text and compiled by soax_expr_compile, against the hand-written kernel, same data;
+    and the paper's own expression as the smallest program."""
+    import time
+    n = s.n
+    t0 = time.perf_counter()
+    prog = Cn.Program(Cn.R1, SE_PROGRAM, ["dt", "k"])
+    compile_s = time.perf_counter() - t0
+    B.soax_tune("step_graph", 0)                                  # launch both one by one: same launch mechanism
+    ms_hand = ev_time_ms(torch, lambda: s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=20), 3, 1) / 20
+    B.soax_tune("step_graph", 1)
+    ms_expr = ev_time_ms(torch, lambda: prog.run(s, nsteps=20, dt=DT, k=1.0), 3, 1) / 20
+    small = Cn.Program(Cn.R1, "pos[0] = vel[1] - vel[2]")
+    ms_small = ev_time_ms(torch, lambda: small.run(s, nsteps=20), 3, 1) / 20
+    ex["next2_expr_vs_hand"] = {
+        "n": n, "program": SE_PROGRAM, "nvrtc_compile_s": compile_s, "expr_step_ms": ms_expr, "hand_step_ms": ms_hand,
+        "expr_over_hand_time": ms_expr / ms_hand, "expr_GBps_72B": gbs(72, n, ms_expr), "expr_frac_of_peak": gbs(72, n, ms_expr) / peak,
+        "paper_expression": "pos[0] = vel[1] - vel[2]", "paper_expression_ms": ms_small,
+        "paper_expression_GBps_16B": gbs(16, n, ms_small)}
 
 
 def _extra_energy(torch, B, Cn, s, peak, ex, gbs):
@@ -262,6 +289,9 @@ def run_tour(torch, B, Cn) -> None:
         s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=1)            # a4  (config 2)
         s.energy_async(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC)                    # a8
         s.step(B.SOAX_STEP_DRIFT, DT, nsteps=1)                                # a2
+    prog = Cn.Program(Cn.R1, SE_PROGRAM, ["dt", "k"])
+    for _ in range(2):
+        prog.run(s, dt=DT, k=1.0)                                              # NEXT-2: the generated kernel
     aos = s.to_aos()
     for _ in range(2):
         s.to_aos(aos)                                                          # a7  (config 3)
@@ -549,7 +579,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["soax", "reference"], default="soax")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
-    ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5: run just those")
+    ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5,expr: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
     ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (run length, alignment, digit width)")

@@ -186,6 +186,43 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
                      uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
                      size_t scratch_bytes, void* stream);
 
+/* ---- NEXT-2: user-written fused element-wise programs ----------------
+ * The paper lets the user write whole-array arithmetic, `soax.posArr(0) = soax.velArr(1) - soax.velArr(2)`
+ * (PAPER.md:294), and fuses it with expression templates into one loop / one kernel without temporaries ("loop
+ * fusion").  Here the user passes the program as TEXT; soax_expr_compile checks it
+ * against the layout, generates ONE CUDA kernel for the whole program (every array it reads is loaded once with
+ * 128/256-bit accesses, every array it assigns is stored once, 4 particles per thread like the built-in step
+ * kernels) and compiles it for sm_100a with NVRTC; soax_expr_run launches it on the live particles.
+ *   program := stmt { ';' stmt }       stmt := target ('=' | '+=' | '-=' | '*=' | '/=') expr
+ *   target  := field | field[c]        a float or double field; a dim-3 field without index expands the statement
+ *                                      over c = 0, 1, 2 with every un-indexed dim-3 field read as its component c
+ *   expr    := + - * / unary-  < <= > >= == !=  &  ( )  numbers  scalar names  field reads  and the calls
+ *              fma(a,b,c) sqrt(x) abs(x) min(a,b) max(a,b) floor(x) wrap(x) float(x) double(x) select(cond,a,b)
+ * Semantics: statements run in order for each particle and later statements see earlier assignments; typing is
+ * C's: float op float is float, anything with a double is double, an assignment rounds to the target's type
+ * (`a += b` is `a = (T)(a + b)`); named scalars and literals with a '.' or exponent are double, integer literals
+ * take the type of the other operand; integer fields can only be compared, masked with '&', or converted with
+ * float()/double(); wrap(x) is the periodic wrap into [0,1) of Q3.  Nothing is contracted: the only fused
+ * multiply-adds are the fma() the user writes, division and sqrt are IEEE (-fmad=false -prec-div -prec-sqrt).
+ * scalar_names: nscalars <= 16 names usable in the program; their values are passed to every run.
+ * Errors: INVALID_ARG (syntax/type error, unknown name, wrong component index -- the run-time face of
+ * PAPER.md:320; soax_expr_error() holds the message with the character position), UNSUPPORTED (NVRTC cannot be
+ * loaded; set the environment variable SOAX_NVRTC to libnvrtc.so.12), CUDA.  Compilation needs no GPU; the code is
+ * loaded onto the device at the first run.  soax_expr_run: INVALID_ARG if the container's layout is not the one
+ * the program was compiled for or nscalars differs. */
+typedef struct soax_expr soax_expr; /* opaque compiled program; free with soax_expr_free */
+int soax_expr_compile(const soax_layout* layout, const char* source, const char* const* scalar_names,
+                      int32_t nscalars, soax_expr** out);
+int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* stream);
+int soax_expr_free(soax_expr* e);
+/* Message of the last failed soax_expr_compile on the calling thread ("" if none). */
+const char* soax_expr_error(void);
+/* The generated CUDA source (owned by the handle), for inspection. */
+const char* soax_expr_cuda_source(const soax_expr* e);
+/* Algorithmic bytes per particle the compiled kernel reads and writes (arrays read before being assigned /
+ * arrays assigned): the roofline denominator of a user program. */
+int soax_expr_traffic(const soax_expr* e, int32_t* bytes_read, int32_t* bytes_written);
+
 /* ---- diagnostics ------------------------------------------------------------------------------------------ */
 const char* soax_strerror(int status);
 /* The cudaError_t (as int) of the last failed CUDA call made by this library on the calling thread, 0 if none. */

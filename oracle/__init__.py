@@ -48,6 +48,8 @@ def lib() -> C.CDLL:
         L.soax_oracle_r1_bin.argtypes = [vp, i64, i32, vp, vp, vp, vp, vp]
         L.soax_oracle_r1_permute.argtypes = [vp, vp, i64, vp]
         L.soax_oracle_b6_euler.argtypes = [vp, i64, i32, C.c_float, i32]
+        L.soax_oracle_fma_f64.argtypes = [vp, vp, vp, vp, i64]
+        L.soax_oracle_fma_f32.argtypes = [vp, vp, vp, vp, i64]
         _lib = L
     return _lib
 
@@ -170,3 +172,14 @@ def b6_euler(pos: np.ndarray, vel: np.ndarray, size_extra: int, dt: float, nstep
     aos[:, 3:6] = vel.T
     lib().soax_oracle_b6_euler(_p(aos), n, size_extra, dt, nsteps)
     return np.ascontiguousarray(aos[:, 0:3].T), np.ascontiguousarray(aos[:, 3:6].T)
+
+
+def fma(a: np.ndarray, b: np.ndarray, c: np.ndarray) -> np.ndarray:
+    """Element-wise correctly rounded a*b+c (std::fma / std::fmaf) on equal-length float64 or float32 arrays."""
+    assert a.dtype == b.dtype == c.dtype and a.shape == b.shape == c.shape and a.ndim == 1
+    a, b, c = (np.ascontiguousarray(x) for x in (a, b, c))
+    out = np.empty_like(a)
+    fn = lib().soax_oracle_fma_f64 if a.dtype == np.float64 else lib().soax_oracle_fma_f32
+    assert a.dtype in (np.float64, np.float32)
+    fn(_p(a), _p(b), _p(c), _p(out), a.size)
+    return out

@@ -269,4 +269,13 @@ void soax_oracle_b6_euler(void* aos, int64_t n, int32_t size_extra, float dt, in
         }
 }
 
+// ---- NEXT-2: the one elementary operation numpy lacks, for oracle/expr.py: a correctly rounded fused multiply-add
+//      over arrays (std::fma / std::fmaf are correctly rounded with or without hardware FMA).
+void soax_oracle_fma_f64(const double* a, const double* b, const double* c, double* out, int64_t n) {
+    for (int64_t i = 0; i < n; ++i) out[i] = std::fma(a[i], b[i], c[i]);
+}
+void soax_oracle_fma_f32(const float* a, const float* b, const float* c, float* out, int64_t n) {
+    for (int64_t i = 0; i < n; ++i) out[i] = std::fmaf(a[i], b[i], c[i]);
+}
+
 }  // extern "C"

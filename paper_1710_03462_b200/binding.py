@@ -64,6 +64,12 @@ SIGNATURES = {
     "soax_reduce_energy": (C.c_int, [_vp, _i32, _f64, _f64, _vp, _sz, _vp, _vp]),
     "soax_scratch_bytes": (_sz, [_vp, _i64, _i32]),
     "soax_bin_permute": (C.c_int, [_vp, _vp, _i32, _f64, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "soax_expr_compile": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
+    "soax_expr_run": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _vp]),
+    "soax_expr_free": (C.c_int, [_vp]),
+    "soax_expr_error": (C.c_char_p, []),
+    "soax_expr_cuda_source": (C.c_char_p, [_vp]),
+    "soax_expr_traffic": (C.c_int, [_vp, C.POINTER(_i32), C.POINTER(_i32)]),
     "soax_strerror": (C.c_char_p, [C.c_int]),
     "soax_last_cuda_error": (C.c_int, []),
     "soax_launch_count": (_i64, []),
@@ -213,6 +219,41 @@ def soax_bin_permute(src: int, dst: int, grid_dim: int, drift_dt: float, dev_cou
                      stream: int = 0) -> None:
     _check(lib().soax_bin_permute(src, dst, grid_dim, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
                                   dev_scratch, scratch_bytes, stream), "soax_bin_permute")
+
+
+# ---- fused element-wise programs (NEXT-2) ---------------------------------------------------------------------------------
+def soax_expr_compile(layout: int, source: str, scalar_names: Sequence[str] = ()) -> int:
+    names = (C.c_char_p * max(len(scalar_names), 1))(*[n.encode() for n in scalar_names])
+    out = _vp()
+    status = lib().soax_expr_compile(layout, source.encode(), names, len(scalar_names), C.byref(out))
+    if status != SOAX_OK:
+        e = SoaxError(status, "soax_expr_compile")
+        e.args = (f"{e.args[0]}: {lib().soax_expr_error().decode()}",)
+        raise e
+    return out.value
+
+
+def soax_expr_run(s: int, e: int, scalars: Sequence[float] = (), stream: int = 0) -> None:
+    arr = (_f64 * max(len(scalars), 1))(*[float(x) for x in scalars])
+    _check(lib().soax_expr_run(s, e, arr, len(scalars), stream), "soax_expr_run")
+
+
+def soax_expr_free(e: int) -> None:
+    _check(lib().soax_expr_free(e), "soax_expr_free")
+
+
+def soax_expr_error() -> str:
+    return lib().soax_expr_error().decode()
+
+
+def soax_expr_cuda_source(e: int) -> str:
+    return lib().soax_expr_cuda_source(e).decode()
+
+
+def soax_expr_traffic(e: int) -> tuple[int, int]:
+    r, w = _i32(), _i32()
+    _check(lib().soax_expr_traffic(e, C.byref(r), C.byref(w)), "soax_expr_traffic")
+    return r.value, w.value
 
 
 # ---- diagnostics ------------------------------------------------------------------------------------------------------

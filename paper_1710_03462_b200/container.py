@@ -147,6 +147,34 @@ class Soax:
         return {"counts": counts, "offsets": offsets, "perm": perm[:n], "kinetic": kin, "scratch": scratch}
 
 
+class Program:
+    """A fused element-wise program compiled for one layout (soax_expr_compile): the paper's whole-array expressions
+    `soax.posArr(0) = soax.velArr(1) - soax.velArr(2)` as ONE generated kernel per program."""
+
+    def __init__(self, fields, source: str, scalar_names=()):
+        self.fields, self.source, self.scalar_names = tuple(fields), source, tuple(scalar_names)
+        self.layout = B.soax_layout_define(self.fields)
+        self.handle = B.soax_expr_compile(self.layout, source, self.scalar_names)
+        self.bytes_read, self.bytes_written = B.soax_expr_traffic(self.handle)
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h:
+            try:
+                B.soax_expr_free(h)
+            except Exception:
+                pass
+
+    @property
+    def cuda_source(self) -> str:
+        return B.soax_expr_cuda_source(self.handle)
+
+    def run(self, s: Soax, nsteps: int = 1, **scalars) -> None:
+        vals = [scalars[k] for k in self.scalar_names]
+        for _ in range(nsteps):
+            B.soax_expr_run(s.handle, self.handle, vals, _stream())
+
+
 def aos_step(fields, aos: torch.Tensor, n: int, kind: int, dt: float, nsteps: int = 1, variant: int = 0, k: float = 1.0,
              center: float = 0.5) -> None:
     layout = B.soax_layout_define(fields)

@@ -5,6 +5,7 @@
 #include <new>
 
 #include "common.cuh"
+#include "expr.hpp"
 #include "ops.hpp"
 
 namespace soax {
@@ -327,6 +328,52 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
               dev_scratch, scratch_bytes};
     dst->n = src->n;
     return src->layout->bin_permute(a, (cudaStream_t)stream);
+}
+
+// ---- NEXT-2: fused element-wise programs (expr.cu) ----------------------------------------------------------------
+struct soax_expr {
+    CompiledExpr* impl;
+    const soax_layout* layout;
+};
+
+int soax_expr_compile(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars,
+                      soax_expr** out) {
+    if (!l || !source || !out || nscalars < 0 || nscalars > 16 || (nscalars > 0 && !scalar_names)) return SOAX_ERR_INVALID_ARG;
+    ExprLayoutInfo info{};
+    info.nfields = l->nfields;
+    info.ncomp = l->ncomp;
+    for (int f = 0; f < l->nfields; ++f) { info.fname[f] = l->fname[f]; info.fdim[f] = l->fdim[f]; info.fbegin[f] = l->fbegin[f]; }
+    for (int c = 0; c < l->ncomp; ++c) { info.cdtype[c] = l->cdtype[c]; info.csize[c] = l->csize[c]; }
+    CompiledExpr* impl = nullptr;
+    SOAX_TRY(expr_compile(info, l, source, scalar_names, nscalars, &impl));
+    soax_expr* e = new (std::nothrow) soax_expr{impl, l};
+    if (!e) { expr_free(impl); return SOAX_ERR_ALLOC; }
+    *out = e;
+    return SOAX_OK;
+}
+
+int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* stream) {
+    if (!s || !e) return SOAX_ERR_INVALID_ARG;
+    if (s->layout != e->layout) return SOAX_ERR_INVALID_ARG;
+    return expr_run(e->impl, s->layout, s->comp, s->n, scalars, nscalars, (cudaStream_t)stream);
+}
+
+int soax_expr_free(soax_expr* e) {
+    if (!e) return SOAX_ERR_INVALID_ARG;
+    expr_free(e->impl);
+    delete e;
+    return SOAX_OK;
+}
+
+const char* soax_expr_error(void) { return expr_error(); }
+const char* soax_expr_cuda_source(const soax_expr* e) { return e ? expr_cuda_source(e->impl) : nullptr; }
+int soax_expr_traffic(const soax_expr* e, int32_t* bytes_read, int32_t* bytes_written) {
+    if (!e) return SOAX_ERR_INVALID_ARG;
+    int r = 0, w = 0;
+    expr_traffic(e->impl, &r, &w);
+    if (bytes_read) *bytes_read = r;
+    if (bytes_written) *bytes_written = w;
+    return SOAX_OK;
 }
 
 const char* soax_strerror(int status) {

@@ -32,6 +32,7 @@
 
 #include "common.cuh"
 #include "expr.hpp"
+#include "ops.hpp"
 
 namespace soax {
 namespace {
@@ -224,6 +225,7 @@ class Parser {
         if (op != "=" && op != "+=" && op != "-=" && op != "*=" && op != "/=") throw ParseError{"expected '=', '+=', '-=', '*=' or '/='", toks_[at_ - 1].pos};
         if (op != "=") mark_read(comp);
         Val rhs = expr();
+        if (rhs.ty == T_ILIT) rhs = to_float(rhs, ty, id.pos);  // an integer literal takes the type of the target
         if (!is_float(rhs.ty)) fail("the right-hand side must be a floating-point value (use float()/double())");
         std::string value = rhs.code;
         if (op != "=") {  // a op= b  is  a = (T)(a op b)  with the usual promotion of a and b
@@ -405,8 +407,13 @@ template <class T, int P> __device__ __forceinline__ Vec<T, P> ld_vec(const T* p
     Vec<T, P> r;
     unsigned* w = reinterpret_cast<unsigned*>(&r);
     if constexpr (B == 32) {
+#ifndef SOAX_NO_256BIT
         asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                      : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]), "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7]) : "l"(p));
+#else
+        asm volatile("ld.global.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "l"(p));
+        asm volatile("ld.global.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4+16];" : "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7]) : "l"(p));
+#endif
     } else if constexpr (B == 16) {
         asm volatile("ld.global.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "l"(p));
     } else if constexpr (B == 8) {
@@ -420,8 +427,13 @@ template <class T, int P> __device__ __forceinline__ void st_vec(T* p, const Vec
     constexpr int B = sizeof(T) * P;
     const unsigned* w = reinterpret_cast<const unsigned*>(&r);
     if constexpr (B == 32) {
+#ifndef SOAX_NO_256BIT
         asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                      :: "l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]) : "memory");
+#else
+        asm volatile("st.global.L1::no_allocate.v4.b32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
+        asm volatile("st.global.L1::no_allocate.v4.b32 [%0+16], {%1,%2,%3,%4};" :: "l"(p), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]) : "memory");
+#endif
     } else if constexpr (B == 16) {
         asm volatile("st.global.L1::no_allocate.v4.b32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
     } else if constexpr (B == 8) {
@@ -491,6 +503,8 @@ struct Nvrtc {
     int (*GetCUBIN)(void*, char*) = nullptr;
     int (*DestroyProgram)(void**) = nullptr;
     const char* (*GetErrorString)(int) = nullptr;
+    int (*Version)(int*, int*) = nullptr;
+    bool wide256 = false;  // PTX ISA 8.8 (CUDA 12.9): ld/st.global.v8.b32
     std::string tried;
 };
 
@@ -500,7 +514,9 @@ Nvrtc* nvrtc() {
     std::call_once(once, [] {
         std::vector<std::string> names;
         if (const char* env = std::getenv("SOAX_NVRTC")) names.push_back(env);
-        for (const char* n : {"libnvrtc.so.12", "/usr/local/cuda/lib64/libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so"}) names.push_back(n);
+        // absolute toolkit paths first: a bare soname would resolve to whatever NVRTC the process already holds (PyTorch
+        // bundles an older one whose PTX ISA lacks the 256-bit accesses)
+        for (const char* n : {"/usr/local/cuda/lib64/libnvrtc.so.12", "/usr/local/cuda/lib64/libnvrtc.so", "libnvrtc.so.12", "libnvrtc.so"}) names.push_back(n);
         for (const std::string& n : names) {
             N.h = dlopen(n.c_str(), RTLD_NOW | RTLD_LOCAL);
             if (N.h) break;
@@ -516,6 +532,9 @@ Nvrtc* nvrtc() {
         N.GetCUBIN = reinterpret_cast<decltype(N.GetCUBIN)>(sym("nvrtcGetCUBIN"));
         N.DestroyProgram = reinterpret_cast<decltype(N.DestroyProgram)>(sym("nvrtcDestroyProgram"));
         N.GetErrorString = reinterpret_cast<decltype(N.GetErrorString)>(sym("nvrtcGetErrorString"));
+        N.Version = reinterpret_cast<decltype(N.Version)>(sym("nvrtcVersion"));
+        int major = 0, minor = 0;
+        if (N.Version && N.Version(&major, &minor) == 0) N.wide256 = major > 12 || (major == 12 && minor >= 9);
         if (!N.CreateProgram || !N.CompileProgram || !N.GetCUBINSize || !N.GetCUBIN || !N.DestroyProgram || !N.GetProgramLogSize || !N.GetProgramLog) {
             dlclose(N.h);
             N.h = nullptr;
@@ -537,8 +556,9 @@ int compile_cubin(const std::string& src, std::vector<char>& cubin) {
         return SOAX_ERR_ALLOC;
     }
     // the arithmetic contract: no contraction, IEEE division and square root, no flush to zero
-    const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false", "-lineinfo"};
-    const int rc = N->CompileProgram(prog, (int)(sizeof(opts) / sizeof(opts[0])), opts);
+    std::vector<const char*> opts = {"--gpu-architecture=sm_100a", "-std=c++17", "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false", "-lineinfo"};
+    if (!N->wide256) opts.push_back("-DSOAX_NO_256BIT");  // older NVRTC: a 32-byte access becomes two 128-bit ones
+    const int rc = N->CompileProgram(prog, (int)opts.size(), opts.data());
     if (rc != 0) {
         size_t len = 0;
         N->GetProgramLogSize(prog, &len);

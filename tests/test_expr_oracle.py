@@ -1,0 +1,154 @@
+"""CPU tests of NEXT-2 (fused element-wise programs): the expression ORACLE
+(oracle/expr.py) pinned by things other than itself -- the already pinned step oracles, exact rational arithmetic
+with one explicit IEEE rounding per operation (tests/exact.py), hand values -- and the host side of the product's
+compiler (soax_expr_compile needs NVRTC but no GPU): syntax/type errors, generated code shape, traffic accounting.
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import expr as oexpr
+from paper_1710_03462_b200 import inputs
+from tests.exact import F, rn32, rn64, to_f32, to_f64, wrap_exact
+
+DT = 1e-3
+SE = "vel = fma(float(dt), float(-(k*(pos - 0.5))), vel); pos = wrap(fma(dt, double(vel), pos))"
+
+
+def bits(a):
+    a = np.ascontiguousarray(a)
+    return a.view({4: np.uint32, 8: np.uint64, 1: np.uint8}[a.dtype.itemsize])
+
+
+# ------------------------------------------------------------------------------------------- oracle pins
+def test_program_reproduces_the_pinned_step_oracles_bit_for_bit():
+    h = inputs.make_r1(4099, seed=3)
+    h["vel"] *= 40.0                                                 # many particles cross a face
+    cur = h
+    for _ in range(5):
+        cur = oexpr.run(cur, SE, {"dt": DT, "k": 1.0})
+    ref = oracle.symplectic_euler(h, DT, 5)
+    assert np.array_equal(bits(cur["pos"]), bits(ref["pos"])) and np.array_equal(bits(cur["vel"]), bits(ref["vel"]))
+    assert np.array_equal(cur["id"], h["id"])
+    d = oexpr.run(h, "pos = wrap(fma(dt, double(vel), pos))", {"dt": DT})
+    assert np.array_equal(bits(d["pos"]), bits(oracle.drift(h, DT, 1)["pos"]))
+
+
+def test_eq1_on_the_papers_float_record():
+    """PAPER.md:136 Eq. 1 on Listing 4's all-float record: one float fma per component (Q2, Q19)."""
+    rng = np.random.default_rng(0)
+    pos, vel = rng.random((3, 777), np.float32), rng.standard_normal((3, 777)).astype(np.float32)
+    out = oexpr.run({"pos": pos, "vel": vel}, "pos = fma(float(dt), vel, pos)", {"dt": DT})
+    ref_pos, _ = oracle.b6_euler(pos, vel, 0, DT, 1)
+    assert np.array_equal(bits(out["pos"]), bits(ref_pos))
+
+
+def test_each_operation_rounds_once_exact_rational():
+    """Every arithmetic node is ONE IEEE operation in the promoted type: restated with exact rationals."""
+    rng = np.random.default_rng(1)
+    n = 200
+    f = {"pos": rng.random((3, n)) * 3 - 1, "vel": rng.standard_normal((3, n)).astype(np.float32)}
+    dt = 0.1
+    # float - float stays float; product with a double scalar is a double product of the converted float, then a double add
+    out = oexpr.run(f, "vel[0] = vel[1] - vel[2]; pos[0] = pos[0] + vel[1]*dt; pos[1] = fma(dt, double(vel[1]), pos[1]);"
+                       "pos[2] = wrap(pos[2]); vel[1] = float(pos[1]) * vel[1]; vel[2] /= 3", {"dt": dt})
+    contracted_differs = 0
+    for i in range(n):
+        v1, v2 = F(f["vel"][1, i]), F(f["vel"][2, i])
+        assert out["vel"][0, i] == to_f32(rn32(v1 - v2))
+        two_roundings = rn64(F(f["pos"][0, i]) + rn64(v1 * F(dt)))
+        assert out["pos"][0, i] == to_f64(two_roundings)
+        fused = rn64(F(f["pos"][1, i]) + v1 * F(dt))
+        assert out["pos"][1, i] == to_f64(fused)
+        contracted_differs += rn64(F(f["pos"][0, i]) + v1 * F(dt)) != two_roundings
+        assert out["pos"][2, i] == to_f64(wrap_exact(F(f["pos"][2, i])))
+        assert out["vel"][1, i] == to_f32(rn32(rn32(fused) * v1))                    # float(pos[1]) sees the NEW pos[1]
+        assert out["vel"][2, i] == to_f32(rn32(v2 / 3))                              # integer literal takes the float type
+    assert contracted_differs > 0                                    # the pin can tell a contracted product from a plain one
+
+
+def test_hand_values_sequencing_vector_form_and_masks():
+    f = {"id": np.array([[7, 8, 9, 10]], np.int32), "pos": np.array([[.5, .25, 1.5, -0.25]] * 3),
+         "vel": np.array([[1, 2, 3, 4], [10, 20, 30, 40], [0, 0, 0, 0]], np.float32),
+         "flags": np.array([[1, 2, 3, 0]], np.uint8)}
+    out = oexpr.run(f, "pos[0] = vel[1] - vel[0]")                                   # PAPER.md:294's example shape
+    assert out["pos"][0].tolist() == [9, 18, 27, 36] and out["pos"][1].tolist() == f["pos"][1].tolist()
+    out = oexpr.run(f, "vel += 1; pos = vel")                                        # vector form; later statements see earlier ones
+    assert out["pos"].tolist() == [[2, 3, 4, 5], [11, 21, 31, 41], [1, 1, 1, 1]]
+    out = oexpr.run(f, "vel[2] = select((flags & 1) != 0, vel[0], -vel[1]); pos[2] = wrap(pos[2]);"
+                       "pos[1] = select(double(id) >= 9, max(pos[1], 1), min(pos[1], 0)); vel[0] = sqrt(abs(vel[0] - 5)) * 2")
+    assert out["vel"][2].tolist() == [1, -20, 3, -40]
+    assert out["pos"][2].tolist() == [.5, .25, .5, .75]
+    assert out["pos"][1].tolist() == [0, 0, 1.5, 1]
+    assert out["vel"][0].tolist() == [4, np.float32(np.sqrt(np.float32(3))) * 2, np.float32(np.sqrt(np.float32(2))) * 2, 2]
+    assert np.array_equal(out["id"], f["id"]) and np.array_equal(out["flags"], f["flags"])
+    assert oexpr.run(f, "pos[0] = wrap(-1e-20 * pos[0] * 0 - 1e-20)")["pos"][0].tolist() == [0, 0, 0, 0]   # Q3: -tiny wraps to 0, not 1
+
+
+@pytest.mark.parametrize("bad", ["pos[3] = 1.0", "pos = id", "foo = 1.0", "id = 1.0", "pos[0] = select(vel[0], 1, 2)",
+                                 "pos[0] = vel", "pos[0] = flags + 1.0", "pos[0] = frob(1.0)"])
+def test_oracle_rejects_what_the_language_rejects(bad):
+    f = {"id": np.zeros((1, 2), np.int32), "pos": np.zeros((3, 2)), "vel": np.zeros((3, 2), np.float32),
+         "flags": np.zeros((1, 2), np.uint8)}
+    with pytest.raises(oexpr.ExprError):
+        oexpr.run(f, bad)
+
+
+# ------------------------------------------------------------------------- host side of the product's compiler
+@pytest.fixture(scope="module")
+def compiler():
+    from paper_1710_03462_b200 import binding as B, container as Cn
+    try:
+        e = B.soax_expr_compile(B.soax_layout_define(Cn.R1), "pos[0] = pos[0]", [])
+    except B.SoaxError as err:
+        if err.status == B.SOAX_ERR_UNSUPPORTED:
+            pytest.skip("NVRTC is not installed on this machine")
+        raise
+    B.soax_expr_free(e)
+    return B, Cn
+
+
+def test_compile_generates_one_fused_kernel(compiler):
+    B, Cn = compiler
+    L = B.soax_layout_define(Cn.R1)
+    e = B.soax_expr_compile(L, SE, ["dt", "k"])
+    src = B.soax_expr_cuda_source(e)
+    assert src.count("__global__") == 1                              # the whole program is ONE kernel (loop fusion)
+    assert src.count("= ld_vec<") == 6 and src.count("    st_vec<") == 6   # every array loaded once and stored once
+    assert "a.p[0]" not in src                                       # id is never touched: unused fields cost nothing
+    assert B.soax_expr_traffic(e) == (36, 36)                        # 72 B/particle, as the hand-written kernel
+    B.soax_expr_free(e)
+    e = B.soax_expr_compile(L, "pos[0] = vel[1] - vel[2]", [])       # PAPER.md:294; pos[0] is overwritten: not loaded
+    assert B.soax_expr_traffic(e) == (8, 8)
+    assert B.soax_expr_cuda_source(e).count("= ld_vec<") == 2
+    B.soax_expr_free(e)
+    e = B.soax_expr_compile(B.soax_layout_define(Cn.R2), "acc = select((flags & 1) != 0, -(k / double(mass)) * (pos - 0.5), acc)", ["k"])
+    assert B.soax_expr_traffic(e) == (1 + 4 + 24 + 24, 24)
+    B.soax_expr_free(e)
+
+
+@pytest.mark.parametrize("bad,msg", [("pos[3] = 1.0", "outside field 'pos'"), ("pos = id", "floating-point"), ("foo = 1.0", "unknown field"),
+                                     ("id = 1.0", "integer field"), ("pos[0] = select(vel[0], 1, 2)", "comparison"),
+                                     ("pos[0] = vel", "components"), ("pos[0] = flags + 1.0", "unknown name"),
+                                     ("pos[0] = frob(1.0)", "unknown function"), ("pos[0] = vel[1] -", "expected a value"),
+                                     ("pos[0] = 1.0 pos[1] = 2.0", "';'"), ("pos[0] = dt", "unknown name"), ("", "assigns nothing"),
+                                     ("pos[0] = fma(1.0, 2.0)", "takes 3"), ("pos[0] = 1.0 $ 2", "unexpected character")])
+def test_compile_errors_carry_a_message(compiler, bad, msg):
+    B, Cn = compiler
+    with pytest.raises(B.SoaxError) as ei:
+        B.soax_expr_compile(B.soax_layout_define(Cn.R1), bad, [])
+    assert ei.value.status == B.SOAX_ERR_INVALID_ARG and msg in str(ei.value)
+    assert msg in B.soax_expr_error()
+
+
+def test_compile_argument_checks(compiler):
+    B, Cn = compiler
+    L = B.soax_layout_define(Cn.R1)
+    with pytest.raises(B.SoaxError):
+        B.soax_expr_compile(L, "pos[0] = pos", ["pos"])              # a scalar may not shadow a field
+    with pytest.raises(B.SoaxError):
+        B.soax_expr_compile(L, "pos[0] = 1.0", [f"s{i}" for i in range(17)])
+    assert B.lib().soax_expr_compile(None, b"x", None, 0, None) == B.SOAX_ERR_INVALID_ARG
+    assert B.lib().soax_expr_free(None) == B.SOAX_ERR_INVALID_ARG
