@@ -175,7 +175,7 @@ def device_fill(torch, s, seed: int) -> None:
         s.comp_view("flags").copy_(torch.randint(0, 256, (n,), generator=g, device="cuda", dtype=torch.uint8))
 
 
-def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5", "expr"), iters: int = 3) -> dict:
+def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5", "expr", "container"), iters: int = 3) -> dict:
     """The other section-8(a) rows, each timed alone with CUDA events (N=1, rank 0): reported beside the headline."""
     ex = {}
     n = s.n
@@ -192,7 +192,40 @@ def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config
         _extra_config5(torch, B, Cn, peak, ex, gbs, iters)
     if "expr" in which:
         _extra_expr(torch, B, Cn, s, peak, ex, gbs)
+    if "container" in which:
+        _extra_container(torch, B, Cn, s, peak, ex, gbs)
     return ex
+
+
+def _extra_container(torch, B, Cn, s, peak, ex, gbs):
+    """NEXT-3: removal of 10 % of 2^24 R1 particles by kill mask -- the paper's overwrite-with-last
+    (in place: only the ~0.09 n rows that fill holes move) and the stable compaction (every survivor moves once) -- and a
+    bulk getElement of 2^20 random rows.  Algorithmic bytes: mask 2 x 1 B/particle (count pass + rank pass); stable:
+    + 40 B read and 40 B written per survivor; swap-last: + 2 x 40 B per moved row (sector-granular traffic is higher)."""
+    n = s.n
+    g = torch.Generator(device="cuda")
+    g.manual_seed(5)
+    kill = (torch.rand(n, generator=g, device="cuda") < 0.1).to(torch.uint8)
+    scratch = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
+    d = Cn.Soax(Cn.R1, 0, capacity=n)
+    t = Cn.Soax(Cn.R1, 0, capacity=n)
+    m = s.remove(kill, stable=True, dst=d, scratch=scratch)
+    ms_stable = ev_time_ms(torch, lambda: s.remove(kill, stable=True, dst=d, scratch=scratch), 10)
+
+    def swap():
+        B.soax_resize(t.handle, n)                                # same rows every time: t is a scratch copy of s
+        t.remove(kill, scratch=scratch)
+    t.copy_from(s)
+    ms_swap = ev_time_ms(torch, swap, 10)
+    idx = torch.randint(0, n, (1 << 20,), generator=g, device="cuda", dtype=torch.int32)
+    out = torch.empty((1 << 20) * 40, dtype=torch.uint8, device="cuda")
+    ms_get = ev_time_ms(torch, lambda: s.get_elements(idx, out), 10)
+    ex["next3_container"] = {
+        "n": n, "kill_fraction": 1 - m / n, "remove_stable_ms": ms_stable,
+        "remove_stable_GBps": (2 * n + 80 * m) / ms_stable / 1e6, "remove_stable_frac_of_peak": (2 * n + 80 * m) / ms_stable / 1e6 / peak,
+        "remove_swap_last_ms": ms_swap, "remove_swap_last_particles_per_s": n / (ms_swap * 1e-3),
+        "get_elements_rows": 1 << 20, "get_elements_ms": ms_get, "get_elements_rows_per_s": (1 << 20) / (ms_get * 1e-3),
+        "note": "soax_remove synchronises the stream once at its end (the handle needs the survivor count): the host round trip is inside these times"}
 
 
 SE_PROGRAM = "vel = fma(float(dt), float(-(k*(pos - 0.5))), vel); pos = wrap(fma(dt, double(vel), pos))"
@@ -579,7 +612,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["soax", "reference"], default="soax")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
-    ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5,expr: run just those")
+    ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5,expr,container: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
     ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (run length, alignment, digit width)")

@@ -186,6 +186,39 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
                      uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
                      size_t scratch_bytes, void* stream);
 
+/* ---- NEXT-3: container operations on the device ---------------------------------
+ * soax_remove deletes the particles whose byte in dev_kill (n bytes, one per live particle) is non-zero, from EVERY
+ * component array:
+ *   SOAX_REMOVE_SWAP_LAST  the paper's default, "the element to remove is overwritten by the last element"
+ *                          (PAPER.md:175): in place (dst must be NULL), unordered.  For a set of flagged
+ *                          particles the rule is applied in the usual forward loop (Q20): i walks up;
+ *                          a flagged a[i] is overwritten by a[n-1], n shrinks, and slot i is examined again.
+ *                          Equivalently: with m = n - #flagged, the k-th flagged slot below m (ascending)
+ *                          receives the k-th surviving particle at or above m counted from the end; no other
+ *                          row moves.
+ *   SOAX_REMOVE_STABLE     order-preserving compaction into dst (same layout, no aliasing, capacity >= survivors;
+ *                          s is left untouched).
+ * The result is unique and deterministic for any mask.  The survivor count is written to *host_new_n (HOST) and
+ * becomes the live count of s (SWAP_LAST) or dst (STABLE).  Because the handle must know that count, this call
+ * SYNCHRONISES `stream` once, after all its kernels have been enqueued (they read the count on the device).
+ * dev_scratch: >= soax_remove_scratch_bytes(n) bytes, 256-byte aligned.
+ * Errors: INVALID_ARG, ALLOC (scratch too small; STABLE: dst capacity < survivors -- dst then holds the
+ * survivors that fit and its live count is unchanged), UNSUPPORTED (n >= 2^32), CUDA. */
+typedef enum { SOAX_REMOVE_SWAP_LAST = 0, SOAX_REMOVE_STABLE = 1 } soax_remove_mode;
+size_t soax_remove_scratch_bytes(int64_t n);
+int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, void* dev_scratch, size_t scratch_bytes,
+                int64_t* host_new_n, void* stream);
+/* push_back of m particle objects (PAPER.md:304-307 `soax.push_back(particle)`): m packed AoS records (see
+ * soax_layout_aos, 16-byte aligned) are appended behind the live particles; the live count grows by m.
+ * ALLOC if n + m exceeds the capacity (the caller owns the memory: to regrow, soax_alloc a larger slab and
+ * soax_copy into it -- the paper's resize). */
+int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream);
+/* Bulk getElement (PAPER.md:304 `soax.getElement(i)`): rows dev_idx[0..m) (uint32, each < n, repeats allowed) as m
+ * packed AoS records in dev_aos (16-byte aligned).  Indices are not range-checked. */
+int soax_get_elements(const soax_t* s, const uint32_t* dev_idx, int64_t m, void* dev_aos, void* stream);
+/* Copy the live particles of src into dst (same layout, capacity >= n); dst's live count becomes src's. */
+int soax_copy(soax_t* dst, const soax_t* src, void* stream);
+
 /* ---- NEXT-2: user-written fused element-wise programs ----------------
  * The paper lets the user write whole-array arithmetic, `soax.posArr(0) = soax.velArr(1) - soax.velArr(2)`
  * (PAPER.md:294), and fuses it with expression templates into one loop / one kernel without temporaries ("loop

@@ -49,6 +49,11 @@ def lib() -> C.CDLL:
         L.soax_oracle_r1_permute.argtypes = [vp, vp, i64, vp]
         L.soax_oracle_b6_euler.argtypes = [vp, i64, i32, C.c_float, i32]
         L.soax_oracle_fma_f64.argtypes = [vp, vp, vp, vp, i64]
+        L.soax_oracle_remove_swap_last.restype = i64
+        L.soax_oracle_remove_swap_last.argtypes = [vp, i64, i64, vp]
+        L.soax_oracle_remove_stable.restype = i64
+        L.soax_oracle_remove_stable.argtypes = [vp, i64, i64, vp]
+        L.soax_oracle_get_elements.argtypes = [vp, i64, vp, i64, vp]
         L.soax_oracle_fma_f32.argtypes = [vp, vp, vp, vp, i64]
         _lib = L
     return _lib
@@ -182,4 +187,31 @@ def fma(a: np.ndarray, b: np.ndarray, c: np.ndarray) -> np.ndarray:
     fn = lib().soax_oracle_fma_f64 if a.dtype == np.float64 else lib().soax_oracle_fma_f32
     assert a.dtype in (np.float64, np.float32)
     fn(_p(a), _p(b), _p(c), _p(out), a.size)
+    return out
+
+
+# ---- NEXT-3: container operations on packed records (uint8 array of n*stride bytes) ---------------------------------
+def remove_swap_last(aos_bytes: np.ndarray, stride: int, kill: np.ndarray) -> np.ndarray:
+    """PAPER.md:175 in a forward loop: a flagged record is overwritten by the last one and the slot is examined again
+    (Q20).  Returns the new bytes."""
+    a = np.array(aos_bytes, dtype=np.uint8)
+    n = a.size // stride
+    k = np.array(kill[:n], dtype=np.uint8)                          # consumed by the routine
+    m = lib().soax_oracle_remove_swap_last(_p(a), n, stride, _p(k))
+    return a[:m * stride].copy()
+
+
+def remove_stable(aos_bytes: np.ndarray, stride: int, kill: np.ndarray) -> np.ndarray:
+    a = np.array(aos_bytes, dtype=np.uint8)
+    n = a.size // stride
+    k = np.ascontiguousarray(kill[:n], np.uint8)
+    m = lib().soax_oracle_remove_stable(_p(a), n, stride, _p(k))
+    return a[:m * stride].copy()
+
+
+def get_elements(aos_bytes: np.ndarray, stride: int, idx: np.ndarray) -> np.ndarray:
+    a = np.ascontiguousarray(aos_bytes, np.uint8)
+    i = np.ascontiguousarray(idx, np.uint32)
+    out = np.empty(i.size * stride, np.uint8)
+    lib().soax_oracle_get_elements(_p(a), stride, _p(i), i.size, _p(out))
     return out

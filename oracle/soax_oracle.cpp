@@ -269,6 +269,43 @@ void soax_oracle_b6_euler(void* aos, int64_t n, int32_t size_extra, float dt, in
         }
 }
 
+// ---- NEXT-3: container operations on an array of structs of any record size ----------
+// The paper's default removal: "the element to remove is overwritten by the last element", stated for
+// ONE element.  For a set of flagged elements it is applied in the usual forward loop (Q20): walk i upwards;
+// if element i is flagged, overwrite it (record AND flag) with the last element, shrink by one and look at slot i
+// again -- the element that arrived may be flagged too.  `kill` is consumed (modified).  Returns the new length.
+int64_t soax_oracle_remove_swap_last(void* aos, int64_t n, int64_t stride, uint8_t* kill) {
+    unsigned char* a = (unsigned char*)aos;
+    int64_t i = 0;
+    while (i < n) {
+        if (kill[i]) {
+            if (i != n - 1) std::memcpy(a + i * stride, a + (n - 1) * stride, (size_t)stride);
+            kill[i] = kill[n - 1];
+            --n;
+        } else {
+            ++i;
+        }
+    }
+    return n;
+}
+// Order-preserving removal: survivors keep their relative order.  Returns the new length.
+int64_t soax_oracle_remove_stable(void* aos, int64_t n, int64_t stride, const uint8_t* kill) {
+    unsigned char* a = (unsigned char*)aos;
+    int64_t m = 0;
+    for (int64_t i = 0; i < n; ++i)
+        if (!kill[i]) {
+            if (m != i) std::memmove(a + m * stride, a + i * stride, (size_t)stride);
+            ++m;
+        }
+    return m;
+}
+// getElement(idx[k]) for k = 0..m-1: copies of whole records.
+void soax_oracle_get_elements(const void* aos, int64_t stride, const uint32_t* idx, int64_t m, void* out) {
+    const unsigned char* a = (const unsigned char*)aos;
+    unsigned char* o = (unsigned char*)out;
+    for (int64_t k = 0; k < m; ++k) std::memcpy(o + k * stride, a + (int64_t)idx[k] * stride, (size_t)stride);
+}
+
 // ---- NEXT-2: the one elementary operation numpy lacks, for oracle/expr.py: a correctly rounded fused multiply-add
 //      over arrays (std::fma / std::fmaf are correctly rounded with or without hardware FMA).
 void soax_oracle_fma_f64(const double* a, const double* b, const double* c, double* out, int64_t n) {

@@ -17,6 +17,7 @@ SOAX_OK, SOAX_ERR_INVALID_ARG, SOAX_ERR_UNKNOWN_LAYOUT, SOAX_ERR_UNSUPPORTED, SO
 SOAX_I32, SOAX_I64, SOAX_U8, SOAX_F32, SOAX_F64 = 0, 1, 2, 3, 4
 SOAX_STEP_DRIFT, SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, SOAX_STEP_EULER_NOWRAP = 0, 1, 2, 3
 SOAX_ENERGY_KINETIC, SOAX_ENERGY_KINETIC_PLUS_HARMONIC = 0, 1
+SOAX_REMOVE_SWAP_LAST, SOAX_REMOVE_STABLE = 0, 1
 DTYPE_SIZE = {SOAX_I32: 4, SOAX_I64: 8, SOAX_U8: 1, SOAX_F32: 4, SOAX_F64: 8}
 
 
@@ -64,6 +65,11 @@ SIGNATURES = {
     "soax_reduce_energy": (C.c_int, [_vp, _i32, _f64, _f64, _vp, _sz, _vp, _vp]),
     "soax_scratch_bytes": (_sz, [_vp, _i64, _i32]),
     "soax_bin_permute": (C.c_int, [_vp, _vp, _i32, _f64, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "soax_remove_scratch_bytes": (_sz, [_i64]),
+    "soax_remove": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _sz, C.POINTER(_i64), _vp]),
+    "soax_push_back_aos": (C.c_int, [_vp, _vp, _i64, _vp]),
+    "soax_get_elements": (C.c_int, [_vp, _vp, _i64, _vp, _vp]),
+    "soax_copy": (C.c_int, [_vp, _vp, _vp]),
     "soax_expr_compile": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
     "soax_expr_run": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _vp]),
     "soax_expr_free": (C.c_int, [_vp]),
@@ -219,6 +225,30 @@ def soax_bin_permute(src: int, dst: int, grid_dim: int, drift_dt: float, dev_cou
                      stream: int = 0) -> None:
     _check(lib().soax_bin_permute(src, dst, grid_dim, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
                                   dev_scratch, scratch_bytes, stream), "soax_bin_permute")
+
+
+# ---- container operations (NEXT-3) ------------------------------------------------------------------------------------
+def soax_remove_scratch_bytes(n: int) -> int:
+    return lib().soax_remove_scratch_bytes(n)
+
+
+def soax_remove(s: int, dst: int | None, dev_kill: int, mode: int, dev_scratch: int, scratch_bytes: int, stream: int = 0) -> int:
+    """Returns the survivor count (the call synchronises the stream once)."""
+    new_n = _i64()
+    _check(lib().soax_remove(s, dst, dev_kill, mode, dev_scratch, scratch_bytes, C.byref(new_n), stream), "soax_remove")
+    return new_n.value
+
+
+def soax_push_back_aos(s: int, dev_aos: int, m: int, stream: int = 0) -> None:
+    _check(lib().soax_push_back_aos(s, dev_aos, m, stream), "soax_push_back_aos")
+
+
+def soax_get_elements(s: int, dev_idx: int, m: int, dev_aos: int, stream: int = 0) -> None:
+    _check(lib().soax_get_elements(s, dev_idx, m, dev_aos, stream), "soax_get_elements")
+
+
+def soax_copy(dst: int, src: int, stream: int = 0) -> None:
+    _check(lib().soax_copy(dst, src, stream), "soax_copy")
 
 
 # ---- fused element-wise programs (NEXT-2) ---------------------------------------------------------------------------------

@@ -147,6 +147,33 @@ class Soax:
         return {"counts": counts, "offsets": offsets, "perm": perm[:n], "kinetic": kin, "scratch": scratch}
 
 
+    # ---- container operations (NEXT-3) --------------------------------------------------------
+    def remove(self, kill: torch.Tensor, stable: bool = False, dst: "Soax | None" = None, scratch: torch.Tensor | None = None) -> int:
+        """kill: uint8 device tensor, one byte per live particle, non-zero = remove.  Unstable (the paper's overwrite
+        with the last element) works in place; stable compacts into `dst`.  Returns the survivor count."""
+        assert kill.dtype == torch.uint8 and kill.is_contiguous() and kill.numel() >= self.n
+        need = B.soax_remove_scratch_bytes(self.n)
+        if scratch is None:
+            scratch = torch.empty(max(need, 256), dtype=torch.uint8, device=self.slab.device)
+        return B.soax_remove(self.handle, dst.handle if stable else None, kill.data_ptr(),
+                             B.SOAX_REMOVE_STABLE if stable else B.SOAX_REMOVE_SWAP_LAST, scratch.data_ptr(), scratch.numel(), _stream())
+
+    def push_back_aos(self, aos: torch.Tensor, m: int) -> None:
+        B.soax_push_back_aos(self.handle, aos.data_ptr(), m, _stream())
+
+    def get_elements(self, idx: torch.Tensor, aos: torch.Tensor | None = None) -> torch.Tensor:
+        """idx: int32/uint32 device tensor of row numbers; returns the rows as packed AoS records (uint8 tensor)."""
+        assert idx.dtype in (torch.int32, torch.uint32) and idx.is_contiguous()
+        stride, _ = B.soax_layout_aos(self.layout, True)
+        m = idx.numel()
+        aos = torch.empty(max(m * stride, 16), dtype=torch.uint8, device=self.slab.device) if aos is None else aos
+        B.soax_get_elements(self.handle, idx.data_ptr(), m, aos.data_ptr(), _stream())
+        return aos[:m * stride]
+
+    def copy_from(self, src: "Soax") -> None:
+        B.soax_copy(self.handle, src.handle, _stream())
+
+
 class Program:
     """A fused element-wise program compiled for one layout (soax_expr_compile): the paper's whole-array expressions
     `soax.posArr(0) = soax.velArr(1) - soax.velArr(2)` as ONE generated kernel per program."""

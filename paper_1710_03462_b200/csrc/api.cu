@@ -30,6 +30,8 @@ struct soax_layout {
     int (*energy)(void* const*, int64_t, int, double, double, void*, double*, cudaStream_t);
     int (*bin_permute)(const BinArgs&, cudaStream_t);
     size_t (*bin_scratch)(int64_t, int);
+    int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, int64_t*, int64_t, cudaStream_t);
+    int (*gather_rows)(void* const*, const uint32_t*, int64_t, void*, cudaStream_t);
 };
 
 // A captured `nsteps`-launch step loop, kept with the container and replayed while the call is the same: small
@@ -76,6 +78,8 @@ soax_layout describe(const char* name) {
     d.energy = &energy_entry<L>;
     d.bin_permute = &bin_permute_entry<L>;
     d.bin_scratch = &bin_scratch_bytes<L>;
+    d.remove = &remove_entry<L>;
+    d.gather_rows = &gather_rows_entry<L>;
     return d;
 }
 
@@ -328,6 +332,58 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
               dev_scratch, scratch_bytes};
     dst->n = src->n;
     return src->layout->bin_permute(a, (cudaStream_t)stream);
+}
+
+// ---- NEXT-3: container operations (container_kernels.cu) ------------------------------------------------------------
+size_t soax_remove_scratch_bytes(int64_t n) { return n < 0 ? 0 : remove_scratch_bytes(n); }
+
+int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, void* dev_scratch, size_t scratch_bytes,
+                int64_t* host_new_n, void* stream) {
+    if (!s || !host_new_n || (s->n > 0 && (!dev_kill || !dev_scratch)) || !aligned(dev_scratch, kAlign)) return SOAX_ERR_INVALID_ARG;
+    if (mode != SOAX_REMOVE_SWAP_LAST && mode != SOAX_REMOVE_STABLE) return SOAX_ERR_INVALID_ARG;
+    if (s->n >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
+    if (mode == SOAX_REMOVE_SWAP_LAST) {
+        if (dst) return SOAX_ERR_INVALID_ARG;  // in place
+    } else {
+        if (!dst || dst == s || dst->layout != s->layout) return SOAX_ERR_INVALID_ARG;
+        for (int c = 0; c < s->layout->ncomp; ++c)
+            if (s->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
+    }
+    if (s->n > 0 && scratch_bytes < remove_scratch_bytes(s->n)) return SOAX_ERR_ALLOC;
+    int64_t m = 0;
+    const int rc = s->layout->remove(s->comp, dst ? dst->comp : nullptr, dev_kill, s->n, mode, dev_scratch, &m,
+                                     dst ? dst->capacity : 0, (cudaStream_t)stream);
+    *host_new_n = m;
+    if (rc != SOAX_OK) return rc;
+    if (mode == SOAX_REMOVE_SWAP_LAST) s->n = m; else dst->n = m;
+    return SOAX_OK;
+}
+
+int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream) {
+    if (!s || m < 0 || (m > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    if (s->n + m > s->capacity) return SOAX_ERR_ALLOC;  // the caller owns the memory: regrow = soax_alloc a larger slab + soax_copy
+    if (m == 0) return SOAX_OK;
+    void* tail[kMaxComp];
+    for (int c = 0; c < s->layout->ncomp; ++c) tail[c] = static_cast<char*>(s->comp[c]) + (size_t)s->n * s->layout->csize[c];
+    SOAX_TRY(s->layout->aos_to_soa(tail, dev_aos, m, (cudaStream_t)stream));
+    s->n += m;
+    return SOAX_OK;
+}
+
+int soax_get_elements(const soax_t* s, const uint32_t* dev_idx, int64_t m, void* dev_aos, void* stream) {
+    if (!s || m < 0 || (m > 0 && (!dev_idx || !dev_aos)) || !aligned(dev_aos, 16) || !aligned(dev_idx, 4)) return SOAX_ERR_INVALID_ARG;
+    return s->layout->gather_rows(const_cast<void* const*>(s->comp), dev_idx, m, dev_aos, (cudaStream_t)stream);
+}
+
+int soax_copy(soax_t* dst, const soax_t* src, void* stream) {
+    if (!dst || !src || dst == src || dst->layout != src->layout) return SOAX_ERR_INVALID_ARG;
+    if (dst->capacity < src->n) return SOAX_ERR_ALLOC;
+    for (int c = 0; c < src->layout->ncomp; ++c)
+        if (src->n > 0)
+            SOAX_CUDA(cudaMemcpyAsync(dst->comp[c], src->comp[c], (size_t)src->n * src->layout->csize[c], cudaMemcpyDeviceToDevice,
+                                      (cudaStream_t)stream));
+    dst->n = src->n;
+    return SOAX_OK;
 }
 
 // ---- NEXT-2: fused element-wise programs (expr.cu) ----------------------------------------------------------------

@@ -1,0 +1,110 @@
+"""GPU parity of NEXT-3 (container operations): removal by kill mask (the paper's
+overwrite-with-last, and a stable compaction), push_back of AoS records, bulk getElement and copy -- byte-exact
+against the oracle on the packed AoS image of the container (every component of every row is compared)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1710_03462_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_1710_03462_b200 import binding as B, container as Cn
+    B.lib()
+    return torch, B, Cn
+
+
+def device(Cn, fields, host, capacity=None):
+    n = next(iter(host.values())).shape[1]
+    s = Cn.Soax(fields, n, capacity)
+    s.upload(host)
+    return s
+
+
+def image(s):
+    return s.to_aos().cpu().numpy()
+
+
+def masks(n, seed):
+    rng = np.random.default_rng(seed)
+    yield (rng.random(n) < 0.5).astype(np.uint8)
+    yield (rng.random(n) < 0.03).astype(np.uint8) * 255              # any non-zero byte counts
+    yield (rng.random(n) < 0.97).astype(np.uint8)
+    yield np.zeros(n, np.uint8)
+    yield np.ones(n, np.uint8)
+    k = np.zeros(n, np.uint8); k[: n // 2] = 1; yield k               # every hole below m, every mover above
+    k = np.zeros(n, np.uint8); k[n // 2:] = 1; yield k                # pure truncation: nothing moves
+
+
+@pytest.mark.parametrize("n", [1 << 15, 70001, 4097, 31, 1])
+def test_remove_matches_oracle(gpu, n):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(n, seed=n)
+    base = oracle.r1_soa_to_aos(host)
+    for kill in masks(n, n):
+        kd = torch.from_numpy(kill).cuda()
+        s = device(Cn, Cn.R1, host)
+        m = s.remove(kd)                                             # the paper's default: overwrite with the last element
+        exp = oracle.remove_swap_last(base, 40, kill)
+        assert m == exp.size // 40 == s.n == n - int((kill != 0).sum())
+        assert np.array_equal(image(s), exp)
+        s = device(Cn, Cn.R1, host)
+        d = Cn.Soax(Cn.R1, 0, capacity=n)
+        m2 = s.remove(kd, stable=True, dst=d)
+        assert m2 == m == d.n and s.n == n
+        assert np.array_equal(image(d), oracle.remove_stable(base, 40, kill))
+        assert np.array_equal(image(s), base)                        # the source of a stable removal is untouched
+
+
+def test_remove_wide_record_and_errors(gpu):
+    torch, B, Cn = gpu
+    n = 20011
+    host = inputs.make_r2(n, seed=3)
+    s = device(Cn, Cn.R2, host)
+    base = image(s)
+    kill = (np.random.default_rng(9).random(n) < 0.4).astype(np.uint8)
+    kd = torch.from_numpy(kill).cuda()
+    d = Cn.Soax(Cn.R2, 0, capacity=n)
+    s.remove(kd, stable=True, dst=d)
+    assert np.array_equal(image(d), oracle.remove_stable(base, 89, kill))
+    s.remove(kd)
+    assert np.array_equal(image(s), oracle.remove_swap_last(base, 89, kill))
+    small = Cn.Soax(Cn.R2, 0, capacity=10)
+    s2 = device(Cn, Cn.R2, host)
+    with pytest.raises(B.SoaxError) as ei:
+        s2.remove(kd, stable=True, dst=small)
+    assert ei.value.status == B.SOAX_ERR_ALLOC
+    with pytest.raises(B.SoaxError):
+        B.soax_remove(s2.handle, s2.handle, kd.data_ptr(), B.SOAX_REMOVE_STABLE, kd.data_ptr(), 1 << 20)   # dst aliases s
+    e = Cn.Soax(Cn.R2, 0, capacity=4)
+    assert e.remove(kd) == 0
+
+
+def test_push_back_get_elements_copy(gpu):
+    torch, B, Cn = gpu
+    n, m = 5000, 3001
+    a, b = inputs.make_r1(n, seed=1), inputs.make_r1(m, seed=2)
+    s = device(Cn, Cn.R1, a, capacity=n + m)
+    extra = torch.from_numpy(oracle.r1_soa_to_aos(b)).cuda()
+    s.push_back_aos(extra, m)                                        # PAPER.md:304-307 push_back(particle), bulk
+    assert s.n == n + m
+    whole = np.concatenate([oracle.r1_soa_to_aos(a), oracle.r1_soa_to_aos(b)])
+    assert np.array_equal(image(s), whole)
+    with pytest.raises(B.SoaxError) as ei:
+        s.push_back_aos(extra, 1)
+    assert ei.value.status == B.SOAX_ERR_ALLOC                       # no regrow: the caller owns the memory
+    idx = np.random.default_rng(4).integers(0, n + m, 1234).astype(np.uint32)
+    idx[:3] = [0, n + m - 1, 0]
+    got = s.get_elements(torch.from_numpy(idx.view(np.int32)).cuda()).cpu().numpy()
+    assert np.array_equal(got, oracle.get_elements(whole, 40, idx))   # PAPER.md:304 getElement(i), bulk
+    idx = np.arange(512, dtype=np.uint32)[::-1].copy()                # exactly two full 256-record tiles
+    got = s.get_elements(torch.from_numpy(idx.view(np.int32)).cuda()).cpu().numpy()
+    assert np.array_equal(got, oracle.get_elements(whole, 40, idx))
+    big = Cn.Soax(Cn.R1, 0, capacity=2 * (n + m))                     # the paper's resize: larger slab + copy
+    big.copy_from(s)
+    assert big.n == n + m and np.array_equal(image(big), whole)
