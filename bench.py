@@ -325,6 +325,14 @@ def run_tour(torch, B, Cn) -> None:
     prog = Cn.Program(Cn.R1, SE_PROGRAM, ["dt", "k"])
     for _ in range(2):
         prog.run(s, dt=DT, k=1.0)                                              # NEXT-2: the generated kernel
+    kill = (torch.rand(n, device="cuda") < 0.1).to(torch.uint8)
+    d = Cn.Soax(Cn.R1, 0, capacity=n)
+    for _ in range(2):
+        s.remove(kill, stable=True, dst=d)                                     # NEXT-3: stable compaction
+        d.remove(kill[:d.n].contiguous())                                      # NEXT-3: overwrite-with-last, in place
+    idx = torch.randint(0, n, (1 << 20,), device="cuda", dtype=torch.int32)
+    s.get_elements(idx)                                                        # NEXT-3: bulk getElement
+    del d
     aos = s.to_aos()
     for _ in range(2):
         s.to_aos(aos)                                                          # a7  (config 3)
