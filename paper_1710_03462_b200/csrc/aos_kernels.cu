@@ -318,27 +318,26 @@ __global__ void __launch_bounds__(kTile) soa_to_aos_ring_kernel(Ptrs<L::ncomp> a
         // the bulk store that last read this stage was committed NS iterations ago: at most NS-1 younger ones may be pending
         if (tid == 0 && k >= NS) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(NS - 1) : "memory");
         __syncthreads();
-        // every global load of the thread is issued before the first shared-memory store (bit images in registers)
-        unsigned long long v[L::ncomp][R];
-        for_each_comp<L>([&](auto ci) {
-            constexpr int C = decltype(ci)::value;
-            using T = typename L::template comp_type<C>;
+        // every global load of the thread is issued before the first shared-memory store; typed registers per component
+        // (a common 64-bit image makes the compiler funnel the loads through one temporary and serialise them)
+        constexpr int kGroup = 16;
+        constexpr int kGroups = (L::ncomp + kGroup - 1) / kGroup;
+        for_each_int<kGroups>([&](auto gi) {
+            constexpr int G0 = decltype(gi)::value * kGroup;
+            constexpr int GN = L::ncomp - G0 < kGroup ? L::ncomp - G0 : kGroup;
+            CompRegs<L, G0, R, std::make_integer_sequence<int, GN>> v;
+            for_each_int<GN>([&](auto ci) {
+                constexpr int C = G0 + decltype(ci)::value;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const T x = ld_vec<T, 1>(comp_ptr<L, C>(a) + t0 + tid + r * kTile).v[0];
-                v[C][r] = 0;
-                memcpy(&v[C][r], &x, sizeof(T));
-            }
-        });
-        for_each_comp<L>([&](auto ci) {
-            constexpr int C = decltype(ci)::value;
-            using T = typename L::template comp_type<C>;
+                for (int r = 0; r < R; ++r) v.template get<C>()[r] = comp_ptr<L, C>(a)[t0 + tid + r * kTile];
+            });
+            for_each_int<GN>([&](auto ci) {
+                constexpr int C = G0 + decltype(ci)::value;
+                using T = typename L::template comp_type<C>;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                T x;
-                memcpy(&x, &v[C][r], sizeof(T));
-                st_piecewise<T, comp_align<L, C>()>(st + (tid + r * kTile) * S + L::aos_offset(C), x);
-            }
+                for (int r = 0; r < R; ++r)
+                    st_piecewise<T, comp_align<L, C>()>(st + (tid + r * kTile) * S + L::aos_offset(C), v.template get<C>()[r]);
+            });
         });
         fence_async_smem();
         __syncthreads();

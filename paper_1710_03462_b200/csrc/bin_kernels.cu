@@ -560,13 +560,29 @@ __global__ void __launch_bounds__(kSortThreads, 2) scatter_ring_kernel(Ptrs<L::n
 // off[c] = first sorted slot whose key is >= c, for c = 0..ncell (off[ncell] = n)
 __global__ void __launch_bounds__(256) boundaries_kernel(const uint32_t* __restrict__ sorted, int64_t n, uint32_t ncell,
                                                          uint32_t* __restrict__ off) {
+    // four consecutive sorted keys per thread (one 128-bit load) plus the key before them
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
-        const uint32_t cur = sorted[j];
-        const uint32_t first = j == 0 ? 0u : sorted[j - 1] + 1u;
-        for (uint32_t c = first; c <= cur; ++c) off[c] = (uint32_t)j;
-        if (j == n - 1)
-            for (uint32_t c = cur + 1; c <= ncell; ++c) off[c] = (uint32_t)n;
+    const int64_t ngroups = (n + 3) / 4;
+    for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < ngroups; g += stride) {
+        const int64_t j0 = g * 4;
+        uint32_t k[4];
+        if (j0 + 4 <= n) {
+            const uint4 v = *reinterpret_cast<const uint4*>(sorted + j0);
+            k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) k[i] = j0 + i < n ? sorted[j0 + i] : 0u;
+        }
+        uint32_t first = j0 == 0 ? 0u : sorted[j0 - 1] + 1u;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int64_t j = j0 + i;
+            if (j >= n) break;
+            for (uint32_t c = first; c <= k[i]; ++c) off[c] = (uint32_t)j;
+            first = k[i] + 1u;
+            if (j == n - 1)
+                for (uint32_t c = k[i] + 1u; c <= ncell; ++c) off[c] = (uint32_t)n;
+        }
     }
 }
 __global__ void __launch_bounds__(256) counts_kernel(const uint32_t* __restrict__ off, uint32_t ncell, uint32_t* counts,

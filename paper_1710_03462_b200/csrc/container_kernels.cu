@@ -9,43 +9,50 @@
 //     atomics).
 //   * gather of arbitrary rows into packed AoS records -- the bulk form of getElement(i);
 //     push_back of AoS records is soax_aos_to_soa at an offset (api.cu).
-// Tiles of 4096 mask bytes; element e of a tile is handled by thread e % 512 in round e / 512, so that every array
-// access of a warp is to 32 consecutive elements; in-tile ranks come from warp ballots and a 128-segment scan.
+// Mask bytes are counted per SEGMENT of 256 (one warp's worth: 8 rounds of 32 lanes) and per tile of 16 segments; a
+// one-CTA scan turns the tile counts into prefixes.  The data kernels have no shared memory and no CTA barrier: each
+// warp owns one segment, rebuilds its prefix from the tile prefix + the counts of the segments before it, ranks its
+// 256 elements with ballots, and moves them -- warps in different phases overlap freely, which a barrier-phased CTA
+// (mask, rank, load, store) does not allow at one CTA per SM.
 #include "common.cuh"
 #include "ops.hpp"
 #include "tma.cuh"
 
 namespace soax {
 
-constexpr int kCThreads = 512;
-constexpr int kCItems = 8;
-constexpr int kCTile = kCThreads * kCItems;  // 4096
-constexpr int kCSegs = kCTile / 32;          // 128 warp-sized segments per tile
+constexpr int kSeg = 256;                    // mask bytes per segment = elements per warp
+constexpr int kSegRounds = kSeg / 32;        // 8
+constexpr int kCTile = 4096;                 // mask bytes per tile (count kernel CTA)
+constexpr int kSegsPerTile = kCTile / kSeg;  // 16
 
-// ---- pass 1: flagged bytes per tile ---------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restrict__ kill, int64_t n, uint32_t* __restrict__ tile_count) {
+// ---- pass 1: flagged bytes per segment and per tile ----------------------------------------------------------------
+// thread t owns mask bytes [16 t, 16 t + 16) of the tile; 16 consecutive threads cover one segment
+__global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restrict__ kill, int64_t n, uint32_t* __restrict__ tile_count,
+                                                         uint32_t* __restrict__ seg_count) {
     __shared__ uint32_t sm[8];
-    const int64_t t0 = (int64_t)blockIdx.x * kCTile;
+    const int64_t b0 = (int64_t)blockIdx.x * kCTile + 16 * threadIdx.x;
     uint32_t c = 0;
-    if (t0 + kCTile <= n && (reinterpret_cast<uintptr_t>(kill) & 15) == 0) {
-        const uint4 v = reinterpret_cast<const uint4*>(kill + t0)[threadIdx.x];  // 16 mask bytes per thread
+    if (b0 + 16 <= n && (reinterpret_cast<uintptr_t>(kill) & 15) == 0) {
+        const uint4 v = *reinterpret_cast<const uint4*>(kill + b0);
         const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int b = 0; b < 4; ++b) c += ((w[i] >> (8 * b)) & 0xffu) != 0;
     } else {
-        for (int i = threadIdx.x; i < kCTile; i += 256)
-            if (t0 + i < n) c += kill[t0 + i] != 0;
+        for (int i = 0; i < 16; ++i)
+            if (b0 + i < n) c += kill[b0 + i] != 0;
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) c += __shfl_down_sync(0xffffffffu, c, o);
+    for (int o = 8; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);  // sum over the 16 threads of a segment
+    if ((threadIdx.x & 15) == 0) seg_count[(int64_t)blockIdx.x * kSegsPerTile + (threadIdx.x >> 4)] = c;
+    c += __shfl_xor_sync(0xffffffffu, c, 16);  // both segments of the warp
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = c;
     __syncthreads();
     if (threadIdx.x == 0) {
-        uint32_t s = 0;
-        for (int w = 0; w < 8; ++w) s += sm[w];
-        tile_count[blockIdx.x] = s;
+        uint32_t t = 0;
+        for (int w = 0; w < 8; ++w) t += sm[w];
+        tile_count[blockIdx.x] = t;
     }
 }
 
@@ -101,65 +108,52 @@ __global__ void __launch_bounds__(1024) kill_scan_kernel(uint32_t* __restrict__ 
     }
 }
 
-// ---- in-tile exclusive rank of the flagged elements -------------------------------------------------------------------
-// flag[k] belongs to element k*512 + tid of the tile.  Returns in rank[k] the number of flagged elements of the tile
-// with a smaller element index.  seg: >= kCSegs + 32 words of shared memory.
-__device__ __forceinline__ void tile_rank(const bool (&flag)[kCItems], uint32_t (&rank)[kCItems], uint32_t* seg) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t lt = (1u << lane) - 1u;
-    uint32_t bal[kCItems];
+// ---- per-warp ranking of one segment ----------------------------------------------------------------------------------
+// Element k*32 + lane of segment `seg` (k = 0..7).  Returns the ballots of the flagged elements and `before` = number
+// of flagged elements in front of the segment.
+struct SegRank {
+    uint32_t bal[kSegRounds];
+    uint32_t before;
+};
+__device__ __forceinline__ SegRank seg_rank(const uint8_t* __restrict__ kill, int64_t n, int64_t seg, const uint32_t* __restrict__ tile_prefix,
+                                            const uint32_t* __restrict__ seg_count) {
+    const int lane = threadIdx.x & 31;
+    SegRank r;
+    const int64_t e0 = seg * kSeg + lane;
+    uint8_t f[kSegRounds];
 #pragma unroll
-    for (int k = 0; k < kCItems; ++k) {
-        bal[k] = __ballot_sync(0xffffffffu, flag[k]);
-        if (lane == 0) seg[k * (kCThreads / 32) + warp] = __popc(bal[k]);  // segment index = element index / 32
-    }
-    __syncthreads();
-    if (threadIdx.x < kCSegs) {  // exclusive scan of the 128 segment counts by the first four warps
-        const uint32_t x = seg[threadIdx.x];
-        uint32_t inc = x;
+    for (int k = 0; k < kSegRounds; ++k) f[k] = e0 + k * 32 < n ? kill[e0 + k * 32] : (uint8_t)0;
+    const int64_t tile = seg / kSegsPerTile;
+    const int s_in = (int)(seg % kSegsPerTile);
+    uint32_t c = lane < s_in ? seg_count[tile * kSegsPerTile + lane] : 0u;  // counts of the segments before this one
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += y;
-        }
-        seg[threadIdx.x] = inc - x;
-        if (lane == 31) seg[kCSegs + warp] = inc;
-    }
-    __syncthreads();
+    for (int o = 8; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    r.before = tile_prefix[tile] + __shfl_sync(0xffffffffu, c, 0);
 #pragma unroll
-    for (int k = 0; k < kCItems; ++k) {
-        const int s = k * (kCThreads / 32) + warp;
-        uint32_t before = seg[s];
-        for (int w = 0; w < (s >> 5); ++w) before += seg[kCSegs + w];
-        rank[k] = before + __popc(bal[k] & lt);
-    }
-    __syncthreads();  // seg may be reused by the caller
+    for (int k = 0; k < kSegRounds; ++k) r.bal[k] = __ballot_sync(0xffffffffu, f[k] != 0);
+    return r;
 }
 
 // ---- SWAP_LAST: the slots to fill (flagged, below m) and the rows that fill them (surviving, at or above m) -----------
-__global__ void __launch_bounds__(kCThreads) holes_movers_kernel(const uint8_t* __restrict__ kill, int64_t n, const uint64_t* __restrict__ info,
-                                                                 const uint32_t* __restrict__ tile_prefix, uint32_t* __restrict__ holes,
-                                                                 uint32_t* __restrict__ movers) {
+__global__ void __launch_bounds__(256) holes_movers_kernel(const uint8_t* __restrict__ kill, int64_t n, const uint64_t* __restrict__ info,
+                                                           const uint32_t* __restrict__ tile_prefix, const uint32_t* __restrict__ seg_count,
+                                                           uint32_t* __restrict__ holes, uint32_t* __restrict__ movers) {
     const int64_t m = n - (int64_t)info[0];  // survivors; read from the device so that the host need not wait for it
     const uint32_t h = (uint32_t)info[1];
     if (h == 0) return;                      // nothing flagged below m: truncation alone removes them
-    __shared__ uint32_t seg[kCSegs + 32];
-    const int64_t t0 = (int64_t)blockIdx.x * kCTile;
-    bool flag[kCItems];
-    uint32_t rank[kCItems];
+    const int64_t seg = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (seg * kSeg >= n) return;
+    const int lane = threadIdx.x & 31;
+    const uint32_t lt = (1u << lane) - 1u;
+    const SegRank r = seg_rank(kill, n, seg, tile_prefix, seg_count);
+    uint32_t run = r.before;
 #pragma unroll
-    for (int k = 0; k < kCItems; ++k) {
-        const int64_t e = t0 + k * kCThreads + threadIdx.x;
-        flag[k] = e < n && kill[e] != 0;
-    }
-    tile_rank(flag, rank, seg);
-    const uint32_t before = tile_prefix[blockIdx.x];
-#pragma unroll
-    for (int k = 0; k < kCItems; ++k) {
-        const int64_t e = t0 + k * kCThreads + threadIdx.x;
+    for (int k = 0; k < kSegRounds; ++k) {
+        const int64_t e = seg * kSeg + k * 32 + lane;
+        const uint32_t ks = run + __popc(r.bal[k] & lt);  // flagged elements with a smaller index
+        run += __popc(r.bal[k]);
         if (e >= n) continue;
-        const uint32_t ks = before + rank[k];  // flagged elements with a smaller index
-        if (flag[k]) {
+        if (r.bal[k] >> lane & 1u) {
             if (e < m) holes[ks] = (uint32_t)e;
         } else if (e >= m) {
             movers[h - 1u - ((uint32_t)(e - m) - (ks - h))] = (uint32_t)e;  // survivors in [m, e), counted from the end
@@ -173,46 +167,69 @@ __global__ void __launch_bounds__(256) move_rows_kernel(Ptrs<L::ncomp> a, const 
     const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= (uint32_t)info[1]) return;  // the grid is sized for the worst case n / 2: surplus CTAs leave at once
     const uint32_t to = holes[k], from = movers[k];
-    for_each_comp<L>([&](auto ci) {
-        constexpr int C = decltype(ci)::value;
-        comp_ptr<L, C>(a)[to] = comp_ptr<L, C>(a)[from];
+    // all loads, then all stores: interleaved, every load would have to wait for the store before it (same arrays)
+    constexpr int kGroup = 16;
+    constexpr int kGroups = (L::ncomp + kGroup - 1) / kGroup;
+    for_each_int<kGroups>([&](auto gi) {
+        constexpr int G0 = decltype(gi)::value * kGroup;
+        constexpr int GN = L::ncomp - G0 < kGroup ? L::ncomp - G0 : kGroup;
+        CompRegs<L, G0, 1, std::make_integer_sequence<int, GN>> v;
+        for_each_int<GN>([&](auto ci) {
+            constexpr int C = G0 + decltype(ci)::value;
+            v.template get<C>()[0] = comp_ptr<L, C>(a)[from];
+        });
+        for_each_int<GN>([&](auto ci) {
+            constexpr int C = G0 + decltype(ci)::value;
+            comp_ptr<L, C>(a)[to] = v.template get<C>()[0];
+        });
     });
 }
 
 // ---- STABLE: dst[i - #flagged before i] = src[i] for every surviving i, every component array ---------------------------
 template <class L>
-__global__ void __launch_bounds__(kCThreads) compact_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst, const uint8_t* __restrict__ kill, int64_t n,
-                                                            const uint32_t* __restrict__ tile_prefix, int64_t dst_capacity) {
-    __shared__ uint32_t seg[kCSegs + 32];
-    const int64_t t0 = (int64_t)blockIdx.x * kCTile;
-    bool flag[kCItems];
-    uint32_t rank[kCItems];
+__global__ void __launch_bounds__(256, 2) compact_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst, const uint8_t* __restrict__ kill, int64_t n,
+                                                      const uint32_t* __restrict__ tile_prefix, const uint32_t* __restrict__ seg_count,
+                                                      int64_t dst_capacity) {
+    const int64_t seg = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (seg * kSeg >= n) return;
+    const int lane = threadIdx.x & 31;
+    const uint32_t lt = (1u << lane) - 1u;
+    const SegRank r = seg_rank(kill, n, seg, tile_prefix, seg_count);
+    const int64_t s0 = seg * kSeg;                // first source element of the segment
+    const int64_t d0 = s0 - (int64_t)r.before;    // first destination slot of the segment's survivors
+    const uint32_t room = dst_capacity > d0 ? (uint32_t)min((int64_t)kSeg, dst_capacity - d0) : 0u;
+    uint32_t slot[kSegRounds], live = 0, run = 0;  // slot within the segment's run of survivors; bit k of live: moves
 #pragma unroll
-    for (int k = 0; k < kCItems; ++k) {
-        const int64_t e = t0 + k * kCThreads + threadIdx.x;
-        flag[k] = e < n && kill[e] != 0;
+    for (int k = 0; k < kSegRounds; ++k) {
+        const uint32_t surv = ~r.bal[k];
+        slot[k] = run + __popc(surv & lt);
+        run += 32u - __popc(r.bal[k]);
+        // too small a destination is reported by the host (ALLOC); never write past it
+        if (s0 + k * 32 + lane < n && (surv >> lane & 1u) && slot[k] < room) live |= 1u << k;
     }
-    tile_rank(flag, rank, seg);
-    const int64_t before = tile_prefix[blockIdx.x];
-    int64_t dest[kCItems];
+    // Component arrays move in groups of up to kGroup: every load of a group is issued before its first store.  The values
+    // sit in TYPED per-component registers (CompRegs): funnelling them through a common 64-bit image made the compiler
+    // reuse one temporary per load and serialise the loads.
+    constexpr int kGroup = 4;
+    constexpr int kGroups = (L::ncomp + kGroup - 1) / kGroup;
+    for_each_int<kGroups>([&](auto gi) {
+        constexpr int G0 = decltype(gi)::value * kGroup;
+        constexpr int GN = L::ncomp - G0 < kGroup ? L::ncomp - G0 : kGroup;
+        CompRegs<L, G0, kSegRounds, std::make_integer_sequence<int, GN>> v;
+        for_each_int<GN>([&](auto ci) {
+            constexpr int C = G0 + decltype(ci)::value;
+            const auto* s = comp_ptr<L, C>(src) + s0 + lane;
 #pragma unroll
-    for (int k = 0; k < kCItems; ++k) {
-        const int64_t e = t0 + k * kCThreads + threadIdx.x;
-        dest[k] = (e < n && !flag[k]) ? e - before - rank[k] : -1;
-        if (dest[k] >= dst_capacity) dest[k] = -1;  // too small a destination is reported by the host (ALLOC); never write past it
-    }
-    for_each_comp<L>([&](auto ci) {
-        constexpr int C = decltype(ci)::value;
-        using T = typename L::template comp_type<C>;
-        const T* s = comp_ptr<L, C>(src);
-        T* d = comp_ptr<L, C>(dst);
-        T v[kCItems];
+            for (int k = 0; k < kSegRounds; ++k)
+                if (live >> k & 1u) v.template get<C>()[k] = s[k * 32];
+        });
+        for_each_int<GN>([&](auto ci) {
+            constexpr int C = G0 + decltype(ci)::value;
+            auto* d = comp_ptr<L, C>(dst) + d0;
 #pragma unroll
-        for (int k = 0; k < kCItems; ++k)
-            if (dest[k] >= 0) v[k] = s[t0 + k * kCThreads + threadIdx.x];
-#pragma unroll
-        for (int k = 0; k < kCItems; ++k)
-            if (dest[k] >= 0) d[dest[k]] = v[k];
+            for (int k = 0; k < kSegRounds; ++k)
+                if (live >> k & 1u) d[slot[k]] = v.template get<C>()[k];
+        });
     });
 }
 
@@ -229,11 +246,23 @@ __global__ void __launch_bounds__(kGTile) gather_rows_kernel(Ptrs<L::ncomp> a, c
         if ((int)threadIdx.x < cnt) {
             const uint32_t row = idx[t0 + threadIdx.x];
             unsigned char* rec = sm + threadIdx.x * S;
-            for_each_comp<L>([&](auto ci) {  // byte images: the record is packed, fields may be misaligned (Q1)
-                constexpr int C = decltype(ci)::value;
-                using T = typename L::template comp_type<C>;
-                const T v = comp_ptr<L, C>(a)[row];
-                memcpy(rec + L::aos_offset(C), &v, sizeof(T));
+            // all the (random) loads of a group of components first, then the stores into the packed record, whose
+            // fields may be misaligned (Q1): byte images
+            constexpr int kGroup = 16;
+            constexpr int kGroups = (L::ncomp + kGroup - 1) / kGroup;
+            for_each_int<kGroups>([&](auto gi) {
+                constexpr int G0 = decltype(gi)::value * kGroup;
+                constexpr int GN = L::ncomp - G0 < kGroup ? L::ncomp - G0 : kGroup;
+                CompRegs<L, G0, 1, std::make_integer_sequence<int, GN>> v;
+                for_each_int<GN>([&](auto ci) {
+                    constexpr int C = G0 + decltype(ci)::value;
+                    v.template get<C>()[0] = comp_ptr<L, C>(a)[row];
+                });
+                for_each_int<GN>([&](auto ci) {
+                    constexpr int C = G0 + decltype(ci)::value;
+                    using T = typename L::template comp_type<C>;
+                    memcpy(rec + L::aos_offset(C), v.template get<C>(), sizeof(T));
+                });
             });
         }
         __syncthreads();
@@ -255,13 +284,14 @@ __global__ void __launch_bounds__(kGTile) gather_rows_kernel(Ptrs<L::ncomp> a, c
 // ---- host side ----------------------------------------------------------------------------------------------------------------
 struct RemovePlan {
     int64_t ntiles;
-    size_t tile_count, info, holes, movers, total;
+    size_t tile_count, seg_count, info, holes, movers, total;
     explicit RemovePlan(int64_t n) {
         ntiles = (n + kCTile - 1) / kCTile;
         if (ntiles < 1) ntiles = 1;
         size_t o = 0;
         auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1, kAlign); return at; };
         tile_count = take((size_t)ntiles * 4);
+        seg_count = take((size_t)ntiles * kSegsPerTile * 4);
         info = take(2 * sizeof(uint64_t));
         holes = take(((size_t)n / 2 + 1) * 4);  // #holes = #movers <= min(K, n - K) <= n / 2
         movers = take(((size_t)n / 2 + 1) * 4);
@@ -277,10 +307,12 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
     const RemovePlan plan(n);
     char* sc = static_cast<char*>(scratch);
     uint32_t* tile_count = reinterpret_cast<uint32_t*>(sc + plan.tile_count);
+    uint32_t* seg_count = reinterpret_cast<uint32_t*>(sc + plan.seg_count);
     uint64_t* info = reinterpret_cast<uint64_t*>(sc + plan.info);
     uint32_t* holes = reinterpret_cast<uint32_t*>(sc + plan.holes);
     uint32_t* movers = reinterpret_cast<uint32_t*>(sc + plan.movers);
-    kill_count_kernel<<<(unsigned)plan.ntiles, 256, 0, st>>>(kill, n, tile_count);
+    kill_count_kernel<<<(unsigned)plan.ntiles, 256, 0, st>>>(kill, n, tile_count, seg_count);
+    const unsigned seg_blocks = (unsigned)(((n + kSeg - 1) / kSeg + 7) / 8);  // 8 warps = 8 segments per CTA
     SOAX_TRY(launched());
     kill_scan_kernel<<<1, 1024, 0, st>>>(tile_count, plan.ntiles, kill, n, info);
     SOAX_TRY(launched());
@@ -289,13 +321,13 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
     uint64_t host_info[2] = {0, 0};
     SOAX_CUDA(cudaMemcpyAsync(host_info, info, sizeof host_info, cudaMemcpyDeviceToHost, st));
     if (mode == SOAX_REMOVE_SWAP_LAST) {
-        holes_movers_kernel<<<(unsigned)plan.ntiles, kCThreads, 0, st>>>(kill, n, info, tile_count, holes, movers);
+        holes_movers_kernel<<<seg_blocks, 256, 0, st>>>(kill, n, info, tile_count, seg_count, holes, movers);
         SOAX_TRY(launched());
         const unsigned blocks = (unsigned)((n / 2 + 255) / 256);  // #holes <= n / 2
         move_rows_kernel<L><<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(make_ptrs<L>(src), holes, movers, info);
         SOAX_TRY(launched());
     } else {
-        compact_kernel<L><<<(unsigned)plan.ntiles, kCThreads, 0, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, tile_count, dst_capacity);
+        compact_kernel<L><<<seg_blocks, 256, 0, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, tile_count, seg_count, dst_capacity);
         SOAX_TRY(launched());
     }
     SOAX_CUDA(cudaStreamSynchronize(st));

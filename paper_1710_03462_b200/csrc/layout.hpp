@@ -124,6 +124,22 @@ __host__ __device__ inline void for_each_comp(F&& f) {
     for_each_comp_impl(static_cast<F&&>(f), std::make_integer_sequence<int, L::ncomp>{});
 }
 
+// for_each_int<N>(f): f(std::integral_constant<int, I>{}) for I = 0..N-1.
+template <int N, class F>
+__host__ __device__ inline void for_each_int(F&& f) {
+    for_each_comp_impl(static_cast<F&&>(f), std::make_integer_sequence<int, N>{});
+}
+
+// CompRegs<L, C0, N, integer_sequence<int, 0..M-1>>: N registers of the right type for each of the components C0..C0+M-1.
+template <int C, class T, int N> struct CompSlot { T v[N]; };
+template <class L, int C0, int N, class Seq> struct CompRegs;
+template <class L, int C0, int N, int... Is>
+struct CompRegs<L, C0, N, std::integer_sequence<int, Is...>> : CompSlot<C0 + Is, typename L::template comp_type<C0 + Is>, N>... {
+    template <int C> __host__ __device__ typename L::template comp_type<C>* get() {
+        return static_cast<CompSlot<C, typename L::template comp_type<C>, N>&>(*this).v;
+    }
+};
+
 // ---- the layouts this library instantiates -----------------------------------------------------------------
 // R1: the program summary's record: configs 1, 2, 3, 5.
 using R1 = Layout<Field<id_tag, int32_t, 1>, Field<pos_tag, double, 3>, Field<vel_tag, float, 3>>;
