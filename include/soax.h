@@ -66,6 +66,15 @@ typedef struct soax_container soax_t;            /* opaque container: layout + n
  * Errors: INVALID_ARG (null, nfields <= 0, bad dtype/dim), UNKNOWN_LAYOUT. */
 int soax_layout_define(const soax_field* fields, int32_t nfields, const soax_layout** out);
 
+/* Run-time layouts.  The paper's container is generic over ANY attribute list; the compiled
+ * registry above covers the records of the benchmark configs.  This call accepts any field list (names: C
+ * identifiers, unique; sum of dims <= 48): if a compiled instantiation matches it is returned, otherwise a run-time
+ * descriptor is created (an identical list returns the same handle).  A run-time layout supports the container
+ * (soax_alloc, soax_field_ptr, soax_resize, soax_upload, soax_download, soax_copy, soax_layout_*) and user-written
+ * fused programs (soax_expr_compile / soax_expr_run generate their kernel from the descriptor); the hand-written
+ * kernel families (soax_step, transposes, energy, binning, removal, gather) answer UNSUPPORTED. */
+int soax_layout_define_dynamic(const soax_field* fields, int32_t nfields, const soax_layout** out);
+
 /* Number of fields / of component arrays (sum of dims) of a layout; negative status on error. */
 int soax_layout_nfields(const soax_layout* layout);
 int soax_layout_ncomp(const soax_layout* layout);

@@ -45,6 +45,7 @@ _lib = None
 _vp, _i64, _i32, _f64, _sz = C.c_void_p, C.c_int64, C.c_int32, C.c_double, C.c_size_t
 SIGNATURES = {
     "soax_layout_define": (C.c_int, [C.POINTER(soax_field), _i32, C.POINTER(_vp)]),
+    "soax_layout_define_dynamic": (C.c_int, [C.POINTER(soax_field), _i32, C.POINTER(_vp)]),
     "soax_layout_nfields": (C.c_int, [_vp]),
     "soax_layout_ncomp": (C.c_int, [_vp]),
     "soax_layout_comp": (C.c_int, [_vp, _i32, C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32)]),
@@ -118,6 +119,14 @@ def soax_layout_define(fields: Sequence[tuple[str, int, int]]) -> int:
     arr = (soax_field * len(fields))(*[soax_field(n.encode(), int(dt), int(dim)) for n, dt, dim in fields])
     out = _vp()
     _check(lib().soax_layout_define(arr, len(fields), C.byref(out)), "soax_layout_define")
+    return out.value
+
+
+def soax_layout_define_dynamic(fields: Sequence[tuple[str, int, int]]) -> int:
+    """Any field list: a compiled layout if one matches, else a run-time layout (container + expression programs)."""
+    arr = (soax_field * len(fields))(*[soax_field(n.encode(), int(dt), int(dim)) for n, dt, dim in fields])
+    out = _vp()
+    _check(lib().soax_layout_define_dynamic(arr, len(fields), C.byref(out)), "soax_layout_define_dynamic")
     return out.value
 
 

@@ -33,9 +33,9 @@ def _stream() -> int:
 class Soax:
     """An SoA particle container on the current CUDA device (the paper's `Soax<ArrayTypes> soax(n)`)."""
 
-    def __init__(self, fields, n: int, capacity: int | None = None, device="cuda"):
+    def __init__(self, fields, n: int, capacity: int | None = None, device="cuda", dynamic: bool = False):
         self.fields = tuple(fields)
-        self.layout = B.soax_layout_define(self.fields)
+        self.layout = (B.soax_layout_define_dynamic if dynamic else B.soax_layout_define)(self.fields)
         self.capacity = n if capacity is None else capacity
         self.slab_bytes = B.soax_slab_bytes(self.layout, self.capacity)
         self.slab = torch.empty(self.slab_bytes, dtype=torch.uint8, device=device)
@@ -178,9 +178,9 @@ class Program:
     """A fused element-wise program compiled for one layout (soax_expr_compile): the paper's whole-array expressions
     `soax.posArr(0) = soax.velArr(1) - soax.velArr(2)` as ONE generated kernel per program."""
 
-    def __init__(self, fields, source: str, scalar_names=()):
+    def __init__(self, fields, source: str, scalar_names=(), dynamic: bool = False):
         self.fields, self.source, self.scalar_names = tuple(fields), source, tuple(scalar_names)
-        self.layout = B.soax_layout_define(self.fields)
+        self.layout = (B.soax_layout_define_dynamic if dynamic else B.soax_layout_define)(self.fields)
         self.handle = B.soax_expr_compile(self.layout, source, self.scalar_names)
         self.bytes_read, self.bytes_written = B.soax_expr_traffic(self.handle)
 

@@ -2,7 +2,10 @@
 // Every step of the hot path runs in the kernels of the sibling .cu files; nothing here computes on the host.
 #include <cstdlib>
 #include <cstring>
+#include <deque>
+#include <mutex>
 #include <new>
+#include <string>
 
 #include "common.cuh"
 #include "expr.hpp"
@@ -128,6 +131,67 @@ int soax_layout_define(const soax_field* fields, int32_t nfields, const soax_lay
     return SOAX_ERR_UNKNOWN_LAYOUT;
 }
 
+// A run-time layout: the same descriptor as a compiled one, with no kernel families behind it (every family entry is
+// null -> SOAX_ERR_UNSUPPORTED).  Descriptors live in a process-wide list and are never freed (handles are immutable
+// and valid for the process lifetime, like the compiled ones); an identical field list returns the same handle.
+namespace {
+struct DynLayout {
+    soax_layout desc{};
+    std::string names[kMaxComp];
+};
+std::mutex g_dyn_mu;
+std::deque<DynLayout> g_dyn;
+
+bool is_identifier(const char* s) {
+    if (!((*s >= 'a' && *s <= 'z') || (*s >= 'A' && *s <= 'Z') || *s == '_')) return false;
+    for (; *s; ++s)
+        if (!((*s >= 'a' && *s <= 'z') || (*s >= 'A' && *s <= 'Z') || (*s >= '0' && *s <= '9') || *s == '_')) return false;
+    return true;
+}
+bool same_fields(const soax_layout& l, const soax_field* fields, int nfields) {
+    if (l.nfields != nfields) return false;
+    for (int f = 0; f < nfields; ++f)
+        if (std::strcmp(l.fname[f], fields[f].name) != 0 || l.fdtype[f] != fields[f].dtype || l.fdim[f] != fields[f].dim) return false;
+    return true;
+}
+}  // namespace
+
+int soax_layout_define_dynamic(const soax_field* fields, int32_t nfields, const soax_layout** out) {
+    const int rc = soax_layout_define(fields, nfields, out);  // a compiled instantiation wins: it has every kernel family
+    if (rc != SOAX_ERR_UNKNOWN_LAYOUT) return rc;
+    int ncomp = 0;
+    for (int f = 0; f < nfields; ++f) {
+        if (!is_identifier(fields[f].name)) return SOAX_ERR_INVALID_ARG;
+        for (int g = 0; g < f; ++g)
+            if (std::strcmp(fields[f].name, fields[g].name) == 0) return SOAX_ERR_INVALID_ARG;
+        ncomp += fields[f].dim;
+        if (ncomp > kMaxComp) return SOAX_ERR_INVALID_ARG;
+    }
+    std::lock_guard<std::mutex> lock(g_dyn_mu);
+    for (const DynLayout& d : g_dyn)
+        if (same_fields(d.desc, fields, nfields)) { *out = &d.desc; return SOAX_OK; }
+    g_dyn.emplace_back();  // deque: earlier descriptors never move
+    DynLayout& d = g_dyn.back();
+    d.desc.name = "dynamic";
+    d.desc.nfields = nfields;
+    d.desc.ncomp = ncomp;
+    int c = 0;
+    for (int f = 0; f < nfields; ++f) {
+        d.names[f] = fields[f].name;
+        d.desc.fname[f] = d.names[f].c_str();
+        d.desc.fdtype[f] = fields[f].dtype;
+        d.desc.fdim[f] = fields[f].dim;
+        d.desc.fbegin[f] = c;
+        for (int k = 0; k < fields[f].dim; ++k, ++c) {
+            d.desc.cfield[c] = f;
+            d.desc.cdtype[c] = fields[f].dtype;
+            d.desc.csize[c] = dtype_size(fields[f].dtype);
+        }
+    }
+    *out = &d.desc;
+    return SOAX_OK;
+}
+
 int soax_layout_nfields(const soax_layout* l) { return l ? l->nfields : SOAX_ERR_INVALID_ARG; }
 int soax_layout_ncomp(const soax_layout* l) { return l ? l->ncomp : SOAX_ERR_INVALID_ARG; }
 
@@ -214,6 +278,7 @@ int soax_download(const soax_t* s, void* const* host_comps, int64_t n, void* str
 
 int soax_step(soax_t* s, const soax_step_params* p, int32_t nsteps, void* stream) {
     if (!s || !p || nsteps < 0) return SOAX_ERR_INVALID_ARG;
+    if (!s->layout->step) return SOAX_ERR_UNSUPPORTED;  // run-time layout: no compiled kernel families
     cudaStream_t st = (cudaStream_t)stream;
     // Graph replay needs a capturable stream (not the legacy default stream) that is not already being captured.
     bool use_graph = g_tune.step_graph && nsteps >= 2 && s->n > 0 && st != nullptr && st != cudaStreamLegacy;
@@ -250,6 +315,7 @@ int soax_step(soax_t* s, const soax_step_params* p, int32_t nsteps, void* stream
 int soax_step_aos(const soax_layout* l, void* dev_aos, int64_t n, const soax_step_params* p, int32_t nsteps,
                   int32_t variant, void* stream) {
     if (!l || !p || nsteps < 0 || n < 0 || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    if (!l->step_aos) return SOAX_ERR_UNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
     // Same graph replay as soax_step, so that the AoS baseline is timed under the same launch mechanism as the SoA
     // path.  There is no container to keep the graph with: one entry per host thread, keyed by the whole call.
@@ -291,12 +357,14 @@ int soax_step_aos(const soax_layout* l, void* dev_aos, int64_t n, const soax_ste
 
 int soax_aos_to_soa(soax_t* dst, const void* dev_aos, int64_t n, void* stream) {
     if (!dst || n < 0 || n > dst->capacity || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    if (!dst->layout->aos_to_soa) return SOAX_ERR_UNSUPPORTED;
     dst->n = n;
     return n == 0 ? SOAX_OK : dst->layout->aos_to_soa(dst->comp, dev_aos, n, (cudaStream_t)stream);
 }
 
 int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream) {
     if (!src || n < 0 || n > src->n || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    if (!src->layout->soa_to_aos) return SOAX_ERR_UNSUPPORTED;
     return n == 0 ? SOAX_OK : src->layout->soa_to_aos(const_cast<void* const*>(src->comp), dev_aos, n, (cudaStream_t)stream);
 }
 
@@ -306,12 +374,13 @@ int soax_reduce_energy(const soax_t* s, int32_t kind, double k, double center, v
                        double* dev_out, void* stream) {
     if (!s || !dev_scratch || !dev_out || !aligned(dev_scratch, 8) || !aligned(dev_out, 8)) return SOAX_ERR_INVALID_ARG;
     if (scratch_bytes < kEnergyScratchBytes) return SOAX_ERR_ALLOC;
+    if (!s->layout->energy) return SOAX_ERR_UNSUPPORTED;
     return s->layout->energy(const_cast<void* const*>(s->comp), s->n, kind, k, center, dev_scratch, dev_out,
                              (cudaStream_t)stream);
 }
 
 size_t soax_scratch_bytes(const soax_layout* l, int64_t n, int32_t grid_dim) {
-    if (!l || n < 0 || ilog2_exact(grid_dim) < 0) return 0;
+    if (!l || n < 0 || ilog2_exact(grid_dim) < 0 || !l->bin_scratch) return 0;
     return l->bin_scratch(n, ilog2_exact(grid_dim));
 }
 
@@ -322,6 +391,7 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
         return SOAX_ERR_INVALID_ARG;
     const int log2g = ilog2_exact(grid_dim);
     if (log2g < 0 || dst->capacity < src->n) return SOAX_ERR_INVALID_ARG;
+    if (!src->layout->bin_permute) return SOAX_ERR_UNSUPPORTED;
     for (int c = 0; c < src->layout->ncomp; ++c)
         if (src->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
     if (src->n >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
@@ -341,7 +411,7 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
                 int64_t* host_new_n, void* stream) {
     if (!s || !host_new_n || (s->n > 0 && (!dev_kill || !dev_scratch)) || !aligned(dev_scratch, kAlign)) return SOAX_ERR_INVALID_ARG;
     if (mode != SOAX_REMOVE_SWAP_LAST && mode != SOAX_REMOVE_STABLE) return SOAX_ERR_INVALID_ARG;
-    if (s->n >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
+    if (s->n >= ((int64_t)1 << 32) || !s->layout->remove) return SOAX_ERR_UNSUPPORTED;
     if (mode == SOAX_REMOVE_SWAP_LAST) {
         if (dst) return SOAX_ERR_INVALID_ARG;  // in place
     } else {
@@ -361,6 +431,7 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
 
 int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream) {
     if (!s || m < 0 || (m > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    if (!s->layout->aos_to_soa) return SOAX_ERR_UNSUPPORTED;
     if (s->n + m > s->capacity) return SOAX_ERR_ALLOC;  // the caller owns the memory: regrow = soax_alloc a larger slab + soax_copy
     if (m == 0) return SOAX_OK;
     void* tail[kMaxComp];
@@ -372,6 +443,7 @@ int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream) 
 
 int soax_get_elements(const soax_t* s, const uint32_t* dev_idx, int64_t m, void* dev_aos, void* stream) {
     if (!s || m < 0 || (m > 0 && (!dev_idx || !dev_aos)) || !aligned(dev_aos, 16) || !aligned(dev_idx, 4)) return SOAX_ERR_INVALID_ARG;
+    if (!s->layout->gather_rows) return SOAX_ERR_UNSUPPORTED;
     return s->layout->gather_rows(const_cast<void* const*>(s->comp), dev_idx, m, dev_aos, (cudaStream_t)stream);
 }
 

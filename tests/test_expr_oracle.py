@@ -152,3 +152,44 @@ def test_compile_argument_checks(compiler):
         B.soax_expr_compile(L, "pos[0] = 1.0", [f"s{i}" for i in range(17)])
     assert B.lib().soax_expr_compile(None, b"x", None, 0, None) == B.SOAX_ERR_INVALID_ARG
     assert B.lib().soax_expr_free(None) == B.SOAX_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------- run-time layouts
+MY_FIELDS = None
+
+
+def my_fields(B):
+    return (("tag", B.SOAX_I64, 1), ("x", B.SOAX_F64, 2), ("temperature", B.SOAX_F32, 1), ("w", B.SOAX_F64, 5), ("alive", B.SOAX_U8, 1))
+
+
+def test_dynamic_layout_descriptor_and_program(compiler):
+    """the container is generic over any attribute list.  A field list that matches no compiled
+    instantiation becomes a run-time layout: container + expression programs work, compiled kernel families do not."""
+    B, Cn = compiler
+    f = my_fields(B)
+    L = B.soax_layout_define_dynamic(f)
+    assert L == B.soax_layout_define_dynamic(f)                      # identical list -> same handle
+    assert B.soax_layout_define_dynamic(Cn.R1) == B.soax_layout_define(Cn.R1)   # a compiled instantiation wins
+    with pytest.raises(B.SoaxError) as ei:
+        B.soax_layout_define(f)
+    assert ei.value.status == B.SOAX_ERR_UNKNOWN_LAYOUT               # the strict call still only knows compiled layouts
+    assert B.soax_layout_nfields(L) == 5 and B.soax_layout_ncomp(L) == 10
+    assert [B.soax_layout_comp(L, c) for c in (0, 2, 3, 8, 9)] == [(0, 0, B.SOAX_I64), (1, 1, B.SOAX_F64), (2, 0, B.SOAX_F32),
+                                                                   (3, 4, B.SOAX_F64), (4, 0, B.SOAX_U8)]
+    stride, offs = B.soax_layout_aos(L, True)
+    assert stride == 8 + 16 + 4 + 40 + 1 and offs == [0, 8, 16, 24, 28, 36, 44, 52, 60, 68]
+    assert B.soax_slab_bytes(L, 1000) == 8192 + 2 * 8192 + 4096 + 5 * 8192 + 1024
+    h = B.soax_alloc(L, 10, 1000, 256 * 4096, B.soax_slab_bytes(L, 1000))      # fake device pointer: never dereferenced
+    assert B.soax_field_ptr(h, 3, 4) - B.soax_field_ptr(h, 0, 0) == 8192 + 2 * 8192 + 4096 + 4 * 8192
+    with pytest.raises(B.SoaxError) as ei:
+        B.soax_step(h, B.step_params(B.SOAX_STEP_DRIFT, 1e-3), 1)
+    assert ei.value.status == B.SOAX_ERR_UNSUPPORTED
+    assert B.soax_scratch_bytes(L, 1000, 8) == 0
+    B.soax_free(h)
+    e = B.soax_expr_compile(L, "w[4] = select(alive != 0, w[0] * double(temperature) + x[1], w[4]); x = x * 2", [])
+    assert B.soax_expr_traffic(e) == (1 + 8 + 4 + 8 + 8 + 8, 8 + 16)
+    B.soax_expr_free(e)
+    for bad in ([("a b", B.SOAX_F32, 1), ("c", B.SOAX_F32, 1)], [("a", B.SOAX_F32, 1), ("a", B.SOAX_F64, 1)], [("a", B.SOAX_F32, 49)]):
+        with pytest.raises(B.SoaxError) as ei:
+            B.soax_layout_define_dynamic(bad)
+        assert ei.value.status == B.SOAX_ERR_INVALID_ARG
