@@ -108,3 +108,30 @@ def test_push_back_get_elements_copy(gpu):
     big = Cn.Soax(Cn.R1, 0, capacity=2 * (n + m))                     # the paper's resize: larger slab + copy
     big.copy_from(s)
     assert big.n == n + m and np.array_equal(image(big), whole)
+
+
+def test_every_call_accepts_an_empty_container(gpu):
+    """n = 0 is a legal particle count for every entry point: nothing is launched, sizes stay 0, the energy is 0."""
+    torch, B, Cn = gpu
+    for fields in (Cn.R1, Cn.R2):
+        s = Cn.Soax(fields, 0, capacity=64)
+        for kind in (B.SOAX_STEP_DRIFT, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC):
+            s.step(kind, 1e-3, nsteps=3)
+        assert s.energy(B.SOAX_ENERGY_KINETIC) == 0.0 and s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC) == 0.0
+        aos = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        s.to_aos(aos)
+        s.from_aos(aos, 0)
+        s.push_back_aos(aos, 0)
+        assert s.n == 0 and s.get_elements(torch.zeros(0, dtype=torch.int32, device="cuda")).numel() == 0
+        d = Cn.Soax(fields, 0, capacity=64)
+        assert s.remove(torch.zeros(1, dtype=torch.uint8, device="cuda")) == 0
+        assert s.remove(torch.zeros(1, dtype=torch.uint8, device="cuda"), stable=True, dst=d) == 0 and d.n == 0
+        d.copy_from(s)
+        Cn.Program(fields, "pos = pos + 1").run(s)
+        if fields is Cn.R1:
+            r = s.bin_permute(d, 8, drift_dt=1e-3, want_kinetic=True)
+            assert int(r["counts"].sum()) == 0 and float(r["kinetic"]) == 0.0
+        else:
+            s.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, 1e-3, nsteps=2)
+        torch.cuda.synchronize()
+        assert all(len(v[0]) == 0 for v in s.download().values())
