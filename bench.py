@@ -233,16 +233,15 @@ SE_PROGRAM = "vel = fma(float(dt), float(-(k*(pos - 0.5))), vel); pos = wrap(fma
 
 def _extra_expr(torch, B, Cn, s, peak, ex, gbs):
     """NEXT-2, the B200 form of the paper's Fig. 11 ("SoAx == hand-written SoA"): the symplectic-Euler step
-    written by the user as program text and compiled by soax_expr_compile, against the hand-written kernel, same data;
+    written by the user as program text and compiled by soax_expr_compile, against the hand-written kernel, same data, same
+    launch mechanism (both replay a captured graph of 20 launches);
     and the paper's own expression as the smallest program."""
     import time
     n = s.n
     t0 = time.perf_counter()
     prog = Cn.Program(Cn.R1, SE_PROGRAM, ["dt", "k"])
     compile_s = time.perf_counter() - t0
-    B.soax_tune("step_graph", 0)                                  # launch both one by one: same launch mechanism
     ms_hand = ev_time_ms(torch, lambda: s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=20), 3, 1) / 20
-    B.soax_tune("step_graph", 1)
     ms_expr = ev_time_ms(torch, lambda: prog.run(s, nsteps=20, dt=DT, k=1.0), 3, 1) / 20
     small = Cn.Program(Cn.R1, "pos[0] = vel[1] - vel[2]")
     ms_small = ev_time_ms(torch, lambda: small.run(s, nsteps=20), 3, 1) / 20
@@ -408,8 +407,20 @@ def run_paper_replica(torch, B, Cn, max_log2n: int = 27) -> None:
     SoA of six float arrays against AoS of Particle<SIZE> = {float x[3]; float v[3]; float temp[SIZE]} (Listing 4),
     execution time per particle and step against N (Fig. 8).  AoS kernel = one thread per record
     (K5); `staged` = the TMA-staged best effort.  Prints one JSON line."""
+    import time
     sizes = (0, 8, 16, 32)
     rows = []
+    eq1 = Cn.Program(Cn.B6(0), "pos = fma(float(dt), vel, pos)", ["dt"])      # Eq. 1 as the user writes it (PAPER.md:136, 294)
+
+    def wall_ns(fn, iters: int = 3) -> float:
+        fn()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(iters):
+            fn()
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) * 1e9 / iters
+
     for log2n in range(7, max_log2n + 1, 2):
         n = 1 << log2n
         reps = max(10, min(2000, (1 << 28) // n))                 # steps per timed call: ~2^28 particle-steps
@@ -420,6 +431,13 @@ def run_paper_replica(torch, B, Cn, max_log2n: int = 27) -> None:
             s.comp_view("vel", c).copy_(torch.randn(n, device="cuda"))
         ms = ev_time_ms(torch, lambda: s.step(B.SOAX_STEP_EULER_NOWRAP, DT, nsteps=reps), 3, 1)
         row["soa_ns_per_particle_step"] = ms * 1e6 / (reps * n)
+        # Fig. 11: the generic SoAx expression against the hand-written SoA loop, kernel time (events) and
+        # wall clock around enqueue + synchronise (the paper's std::chrono, which exposes the launch overhead)
+        ms = ev_time_ms(torch, lambda: eq1.run(s, nsteps=reps, dt=DT), 3, 1)
+        row["soax_expr_ns_per_particle_step"] = ms * 1e6 / (reps * n)
+        row["soa_wall_ns_per_particle_step"] = wall_ns(lambda: s.step(B.SOAX_STEP_EULER_NOWRAP, DT, nsteps=reps)) / (reps * n)
+        row["soax_expr_wall_ns_per_particle_step"] = wall_ns(lambda: eq1.run(s, nsteps=reps, dt=DT)) / (reps * n)
+        row["soax_expr_over_hand_soa_time"] = row["soax_expr_ns_per_particle_step"] / row["soa_ns_per_particle_step"]
         del s
         for S in sizes:
             stride = 24 + 4 * S
@@ -444,6 +462,7 @@ def run_paper_replica(torch, B, Cn, max_log2n: int = 27) -> None:
                          "soa_GBps": 36.0 / big["soa_ns_per_particle_step"],
                          **{f"aos{S}_GBps_useful": 36.0 / big[f"aos{S}_ns_per_particle_step"] for S in sizes}},
         "soa_faster_than_aos0_from_n": min(cross) if cross else None,
+        "fig11_soax_expr_over_hand_soa_time": {str(r["n"]): round(r["soax_expr_over_hand_soa_time"], 4) for r in rows},
         "rows": rows, "gpu_launches": B.soax_launch_count()}))
 
 

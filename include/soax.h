@@ -250,12 +250,13 @@ int soax_copy(soax_t* dst, const soax_t* src, void* stream);
  * Errors: INVALID_ARG (syntax/type error, unknown name, wrong component index -- the run-time face of
  * PAPER.md:320; soax_expr_error() holds the message with the character position), UNSUPPORTED (NVRTC cannot be
  * loaded; set the environment variable SOAX_NVRTC to libnvrtc.so.12), CUDA.  Compilation needs no GPU; the code is
- * loaded onto the device at the first run.  soax_expr_run: INVALID_ARG if the container's layout is not the one
- * the program was compiled for or nscalars differs. */
+ * loaded onto the device at the first run.  soax_expr_run applies the program nsteps times (one launch and one
+ * memory pass each; nsteps >= 2 on a capturable stream replays a captured graph, like soax_step): INVALID_ARG if
+ * the container's layout is not the one the program was compiled for or nscalars differs. */
 typedef struct soax_expr soax_expr; /* opaque compiled program; free with soax_expr_free */
 int soax_expr_compile(const soax_layout* layout, const char* source, const char* const* scalar_names,
                       int32_t nscalars, soax_expr** out);
-int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* stream);
+int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, int32_t nsteps, void* stream);
 int soax_expr_free(soax_expr* e);
 /* Message of the last failed soax_expr_compile on the calling thread ("" if none). */
 const char* soax_expr_error(void);

@@ -72,7 +72,7 @@ SIGNATURES = {
     "soax_get_elements": (C.c_int, [_vp, _vp, _i64, _vp, _vp]),
     "soax_copy": (C.c_int, [_vp, _vp, _vp]),
     "soax_expr_compile": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
-    "soax_expr_run": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _vp]),
+    "soax_expr_run": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _i32, _vp]),
     "soax_expr_free": (C.c_int, [_vp]),
     "soax_expr_error": (C.c_char_p, []),
     "soax_expr_cuda_source": (C.c_char_p, [_vp]),
@@ -272,9 +272,9 @@ def soax_expr_compile(layout: int, source: str, scalar_names: Sequence[str] = ()
     return out.value
 
 
-def soax_expr_run(s: int, e: int, scalars: Sequence[float] = (), stream: int = 0) -> None:
+def soax_expr_run(s: int, e: int, scalars: Sequence[float] = (), nsteps: int = 1, stream: int = 0) -> None:
     arr = (_f64 * max(len(scalars), 1))(*[float(x) for x in scalars])
-    _check(lib().soax_expr_run(s, e, arr, len(scalars), stream), "soax_expr_run")
+    _check(lib().soax_expr_run(s, e, arr, len(scalars), nsteps, stream), "soax_expr_run")
 
 
 def soax_expr_free(e: int) -> None:

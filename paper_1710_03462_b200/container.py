@@ -198,8 +198,7 @@ class Program:
 
     def run(self, s: Soax, nsteps: int = 1, **scalars) -> None:
         vals = [scalars[k] for k in self.scalar_names]
-        for _ in range(nsteps):
-            B.soax_expr_run(s.handle, self.handle, vals, _stream())
+        B.soax_expr_run(s.handle, self.handle, vals, nsteps, _stream())
 
 
 def aos_step(fields, aos: torch.Tensor, n: int, kind: int, dt: float, nsteps: int = 1, variant: int = 0, k: float = 1.0,

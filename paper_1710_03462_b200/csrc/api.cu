@@ -462,6 +462,13 @@ int soax_copy(soax_t* dst, const soax_t* src, void* stream) {
 struct soax_expr {
     CompiledExpr* impl;
     const soax_layout* layout;
+    // captured nsteps-launch loop, replayed while the call is the same (as soax_step does; see StepGraph)
+    cudaGraphExec_t exec = nullptr;
+    const soax_container* g_s = nullptr;
+    void* g_comp0 = nullptr;
+    int64_t g_n = 0;
+    int32_t g_nsteps = 0, g_nscalars = 0, g_block = 0;
+    double g_scalars[16] = {};
 };
 
 int soax_expr_compile(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars,
@@ -474,20 +481,56 @@ int soax_expr_compile(const soax_layout* l, const char* source, const char* cons
     for (int c = 0; c < l->ncomp; ++c) { info.cdtype[c] = l->cdtype[c]; info.csize[c] = l->csize[c]; }
     CompiledExpr* impl = nullptr;
     SOAX_TRY(expr_compile(info, l, source, scalar_names, nscalars, &impl));
-    soax_expr* e = new (std::nothrow) soax_expr{impl, l};
+    soax_expr* e = new (std::nothrow) soax_expr();
+    if (e) { e->impl = impl; e->layout = l; }
     if (!e) { expr_free(impl); return SOAX_ERR_ALLOC; }
     *out = e;
     return SOAX_OK;
 }
 
-int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* stream) {
-    if (!s || !e) return SOAX_ERR_INVALID_ARG;
+int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, int32_t nsteps, void* stream) {
+    if (!s || !e || nsteps < 0 || nscalars < 0 || nscalars > 16) return SOAX_ERR_INVALID_ARG;
     if (s->layout != e->layout) return SOAX_ERR_INVALID_ARG;
-    return expr_run(e->impl, s->layout, s->comp, s->n, scalars, nscalars, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    bool use_graph = g_tune.step_graph && nsteps >= 2 && s->n > 0 && st != nullptr && st != cudaStreamLegacy;
+    if (use_graph) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+    }
+    if (use_graph) {
+        const bool same = e->exec && e->g_s == s && e->g_comp0 == s->comp[0] && e->g_n == s->n && e->g_nsteps == nsteps &&
+                          e->g_nscalars == nscalars && e->g_block == g_tune.step_block &&
+                          (nscalars == 0 || std::memcmp(e->g_scalars, scalars, sizeof(double) * nscalars) == 0);
+        if (!same) {
+            if (e->exec) { cudaGraphExecDestroy(e->exec); e->exec = nullptr; }
+            // the first launch loads the generated code: do it outside the capture
+            SOAX_TRY(expr_run(e->impl, s->layout, s->comp, 0, scalars, nscalars, st));
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                int rc = SOAX_OK;
+                for (int32_t i = 0; i < nsteps && rc == SOAX_OK; ++i) rc = expr_run(e->impl, s->layout, s->comp, s->n, scalars, nscalars, st);
+                const cudaError_t err = cudaStreamEndCapture(st, &graph);
+                if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+                if (err == cudaSuccess && graph && cudaGraphInstantiate(&e->exec, graph, 0) != cudaSuccess) e->exec = nullptr;
+                if (graph) cudaGraphDestroy(graph);
+            }
+            cudaGetLastError();
+            if (e->exec) {
+                e->g_s = s; e->g_comp0 = s->comp[0]; e->g_n = s->n; e->g_nsteps = nsteps; e->g_nscalars = nscalars; e->g_block = g_tune.step_block;
+                if (nscalars) std::memcpy(e->g_scalars, scalars, sizeof(double) * nscalars);
+            }
+        } else {
+            g_launches.fetch_add(nsteps, std::memory_order_relaxed);
+        }
+        if (e->exec) { SOAX_CUDA(cudaGraphLaunch(e->exec, st)); return SOAX_OK; }
+    }
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(expr_run(e->impl, s->layout, s->comp, s->n, scalars, nscalars, st));
+    return SOAX_OK;
 }
 
 int soax_expr_free(soax_expr* e) {
     if (!e) return SOAX_ERR_INVALID_ARG;
+    if (e->exec) cudaGraphExecDestroy(e->exec);
     expr_free(e->impl);
     delete e;
     return SOAX_OK;

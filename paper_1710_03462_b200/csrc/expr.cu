@@ -644,7 +644,6 @@ int expr_run(CompiledExpr* E, const void* layout_key, void* const* comps, int64_
              cudaStream_t st) {
     if (E->layout_key != layout_key) return SOAX_ERR_INVALID_ARG;
     if (nscalars != E->nscalars || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
-    if (n == 0) return SOAX_OK;
     {
         std::lock_guard<std::mutex> lock(E->mu);
         if (!E->kernel) {  // the cubin is loaded into the current context on first use
@@ -652,6 +651,7 @@ int expr_run(CompiledExpr* E, const void* layout_key, void* const* comps, int64_
             SOAX_CUDA(cudaLibraryGetKernel(&E->kernel, E->lib, "soax_expr_kernel"));
         }
     }
+    if (n == 0) return SOAX_OK;  // (the code is loaded even then: soax_expr_run relies on it before a stream capture)
     // Args { void* p[ncomp]; double s[max(nscalars,1)]; } -- the layout the generated source declares
     std::vector<unsigned char> args((size_t)E->ncomp * sizeof(void*) + (size_t)(nscalars > 0 ? nscalars : 1) * sizeof(double), 0);
     std::memcpy(args.data(), comps, (size_t)E->ncomp * sizeof(void*));
