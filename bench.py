@@ -353,6 +353,22 @@ def run_tour(torch, B, Cn) -> None:
     scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n5, 64), dtype=torch.uint8, device="cuda")
     for _ in range(2):
         s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch)   # a10-a14 (config 5)
+    del s5, d5, scratch
+    torch.cuda.empty_cache()
+    # NEXT-1: the paper's float record (Listing 4) at N = 2^24 -- SoA and AoS Particle<SIZE> kernels, for the B200
+    # versions of Fig. 9 (global load efficiency) and Fig. 10 (L1 hit rate)
+    nb = 1 << 24
+    sb = Cn.Soax(Cn.B6(0), nb)
+    for c in range(3):
+        sb.comp_view("pos", c).copy_(torch.rand(nb, device="cuda"))
+        sb.comp_view("vel", c).copy_(torch.randn(nb, device="cuda"))
+    sb.step(B.SOAX_STEP_EULER_NOWRAP, DT, nsteps=1)
+    del sb
+    for S in (0, 8, 16, 32):
+        aos = torch.rand(nb * (6 + S), device="cuda", dtype=torch.float32).view(torch.uint8)
+        Cn.aos_step(Cn.B6(S), aos, nb, B.SOAX_STEP_EULER_NOWRAP, DT, 1, 0)
+        Cn.aos_step(Cn.B6(S), aos, nb, B.SOAX_STEP_EULER_NOWRAP, DT, 1, 1)
+        del aos
     torch.cuda.synchronize()
     print(json.dumps({"tour": "done", "gpu_launches": B.soax_launch_count()}))
 
