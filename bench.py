@@ -245,7 +245,16 @@ def _extra_expr(torch, B, Cn, s, peak, ex, gbs):
     ms_expr = ev_time_ms(torch, lambda: prog.run(s, nsteps=20, dt=DT, k=1.0), 3, 1) / 20
     small = Cn.Program(Cn.R1, "pos[0] = vel[1] - vel[2]")
     ms_small = ev_time_ms(torch, lambda: small.run(s, nsteps=20), 3, 1) / 20
+    ke_pe = ("0.5 * fma(k*(pos[2]-c), pos[2]-c, fma(k*(pos[1]-c), pos[1]-c, fma(k*(pos[0]-c), pos[0]-c, "
+             "fma(double(vel[2]), double(vel[2]), fma(double(vel[1]), double(vel[1]), double(vel[0]) * double(vel[0]))))))")
+    red = Cn.SumProgram(Cn.R1, ke_pe, ["k", "c"])
+    e_out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ms_sum = ev_time_ms(torch, lambda: red.sum_async(s, out=e_out, k=1.0, c=0.5), 20)
+    ms_energy = ev_time_ms(torch, lambda: s.energy_async(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, out=e_out), 20)
+    same = red.sum(s, k=1.0, c=0.5) == s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC)
     ex["next2_expr_vs_hand"] = {
+        "sum_program_ms": ms_sum, "hand_energy_ms": ms_energy, "sum_program_over_hand_time": ms_sum / ms_energy,
+        "sum_program_GBps_36B": gbs(36, n, ms_sum), "sum_program_equals_hand_energy_bitwise": bool(same),
         "n": n, "program": SE_PROGRAM, "nvrtc_compile_s": compile_s, "expr_step_ms": ms_expr, "hand_step_ms": ms_hand,
         "expr_over_hand_time": ms_expr / ms_hand, "expr_GBps_72B": gbs(72, n, ms_expr), "expr_frac_of_peak": gbs(72, n, ms_expr) / peak,
         "paper_expression": "pos[0] = vel[1] - vel[2]", "paper_expression_ms": ms_small,

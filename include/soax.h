@@ -258,6 +258,15 @@ int soax_expr_compile(const soax_layout* layout, const char* source, const char*
                       int32_t nscalars, soax_expr** out);
 int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, int32_t nsteps, void* stream);
 int soax_expr_free(soax_expr* e);
+/* User-written REDUCTIONS: `expression` is ONE expression of the same language (no assignment); its per-particle value,
+ * converted to double, is summed over the live particles into *dev_out (device) with the fixed reduction tree of
+ * soax_reduce_energy (a8): run-to-run deterministic, and an expression that restates the energy term operation by
+ * operation reproduces soax_reduce_energy bit for bit.  dev_scratch: >= soax_energy_scratch_bytes() bytes, 8-byte
+ * aligned.  A sum program cannot be passed to soax_expr_run, nor an assignment program to soax_expr_sum (INVALID_ARG). */
+int soax_expr_compile_sum(const soax_layout* layout, const char* expression, const char* const* scalar_names,
+                          int32_t nscalars, soax_expr** out);
+int soax_expr_sum(const soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* dev_scratch,
+                  size_t scratch_bytes, double* dev_out, void* stream);
 /* Message of the last failed soax_expr_compile on the calling thread ("" if none). */
 const char* soax_expr_error(void);
 /* The generated CUDA source (owned by the handle), for inspection. */

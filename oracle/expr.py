@@ -21,6 +21,7 @@ syntax), so this evaluator shares neither parser nor code generator with the CUD
 from __future__ import annotations
 
 import ast
+import math
 
 import numpy as np
 
@@ -255,3 +256,22 @@ def run(fields: dict, source: str, scalars: dict | None = None) -> dict:
             ev.vec_c = c
             ev.assign(target, op, value)
     return {k: np.stack(v) for k, v in state.items()}
+
+
+def total(fields: dict, expression: str, scalars: dict | None = None) -> float:
+    """The reduction programs of soax_expr_compile_sum: the expression is evaluated per particle as in `run`, converted
+    to float64, and the terms are added exactly (math.fsum: the correctly rounded sum, so no summation order is implied)."""
+    n = next(iter(fields.values())).shape[1]
+    state = {k: [np.array(v[c]) for c in range(v.shape[0])] for k, v in fields.items()}
+    dims = {k: v.shape[0] for k, v in fields.items()}
+    try:
+        tree = ast.parse(expression.strip().rstrip(";"), mode="eval")
+    except SyntaxError as e:
+        raise ExprError(str(e)) from e
+    v = _Eval(state, dims, dict(scalars or {}), n).ev(tree.body)
+    if isinstance(v, _IntLit):
+        v = _to(v, np.float64)
+    if not _is_float(v):
+        raise ExprError("the summed expression must be a floating-point value")
+    terms = np.broadcast_to(v.astype(np.float64), (n,))
+    return math.fsum(terms.tolist())

@@ -72,6 +72,8 @@ SIGNATURES = {
     "soax_get_elements": (C.c_int, [_vp, _vp, _i64, _vp, _vp]),
     "soax_copy": (C.c_int, [_vp, _vp, _vp]),
     "soax_expr_compile": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
+    "soax_expr_compile_sum": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
+    "soax_expr_sum": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _vp, _sz, _vp, _vp]),
     "soax_expr_run": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _i32, _vp]),
     "soax_expr_free": (C.c_int, [_vp]),
     "soax_expr_error": (C.c_char_p, []),
@@ -270,6 +272,22 @@ def soax_expr_compile(layout: int, source: str, scalar_names: Sequence[str] = ()
         e.args = (f"{e.args[0]}: {lib().soax_expr_error().decode()}",)
         raise e
     return out.value
+
+
+def soax_expr_compile_sum(layout: int, expression: str, scalar_names: Sequence[str] = ()) -> int:
+    names = (C.c_char_p * max(len(scalar_names), 1))(*[n.encode() for n in scalar_names])
+    out = _vp()
+    status = lib().soax_expr_compile_sum(layout, expression.encode(), names, len(scalar_names), C.byref(out))
+    if status != SOAX_OK:
+        e = SoaxError(status, "soax_expr_compile_sum")
+        e.args = (f"{e.args[0]}: {lib().soax_expr_error().decode()}",)
+        raise e
+    return out.value
+
+
+def soax_expr_sum(s: int, e: int, scalars: Sequence[float], dev_scratch: int, scratch_bytes: int, dev_out: int, stream: int = 0) -> None:
+    arr = (_f64 * max(len(scalars), 1))(*[float(x) for x in scalars])
+    _check(lib().soax_expr_sum(s, e, arr, len(scalars), dev_scratch, scratch_bytes, dev_out, stream), "soax_expr_sum")
 
 
 def soax_expr_run(s: int, e: int, scalars: Sequence[float] = (), nsteps: int = 1, stream: int = 0) -> None:

@@ -201,6 +201,37 @@ class Program:
         B.soax_expr_run(s.handle, self.handle, vals, nsteps, _stream())
 
 
+class SumProgram:
+    """A user-written reduction (soax_expr_compile_sum): the sum over the particles of one expression, in double, with
+    the reduction tree of soax_reduce_energy."""
+
+    def __init__(self, fields, expression: str, scalar_names=(), dynamic: bool = False):
+        self.fields, self.expression, self.scalar_names = tuple(fields), expression, tuple(scalar_names)
+        self.layout = (B.soax_layout_define_dynamic if dynamic else B.soax_layout_define)(self.fields)
+        self.handle = B.soax_expr_compile_sum(self.layout, expression, self.scalar_names)
+        self.bytes_read, _ = B.soax_expr_traffic(self.handle)
+        self._scratch = None
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h:
+            try:
+                B.soax_expr_free(h)
+            except Exception:
+                pass
+
+    def sum_async(self, s: Soax, out: torch.Tensor | None = None, **scalars) -> torch.Tensor:
+        if self._scratch is None:
+            self._scratch = torch.empty(B.soax_energy_scratch_bytes(), dtype=torch.uint8, device=s.slab.device)
+        out = torch.empty(1, dtype=torch.float64, device=s.slab.device) if out is None else out
+        B.soax_expr_sum(s.handle, self.handle, [scalars[k] for k in self.scalar_names], self._scratch.data_ptr(),
+                        self._scratch.numel(), out.data_ptr(), _stream())
+        return out
+
+    def sum(self, s: Soax, **scalars) -> float:
+        return float(self.sum_async(s, **scalars).item())
+
+
 def aos_step(fields, aos: torch.Tensor, n: int, kind: int, dt: float, nsteps: int = 1, variant: int = 0, k: float = 1.0,
              center: float = 0.5) -> None:
     layout = B.soax_layout_define(fields)

@@ -471,8 +471,8 @@ struct soax_expr {
     double g_scalars[16] = {};
 };
 
-int soax_expr_compile(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars,
-                      soax_expr** out) {
+static int expr_compile_any(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars, bool is_sum,
+                            soax_expr** out) {
     if (!l || !source || !out || nscalars < 0 || nscalars > 16 || (nscalars > 0 && !scalar_names)) return SOAX_ERR_INVALID_ARG;
     ExprLayoutInfo info{};
     info.nfields = l->nfields;
@@ -480,12 +480,33 @@ int soax_expr_compile(const soax_layout* l, const char* source, const char* cons
     for (int f = 0; f < l->nfields; ++f) { info.fname[f] = l->fname[f]; info.fdim[f] = l->fdim[f]; info.fbegin[f] = l->fbegin[f]; }
     for (int c = 0; c < l->ncomp; ++c) { info.cdtype[c] = l->cdtype[c]; info.csize[c] = l->csize[c]; }
     CompiledExpr* impl = nullptr;
-    SOAX_TRY(expr_compile(info, l, source, scalar_names, nscalars, &impl));
+    SOAX_TRY(expr_compile(info, l, source, scalar_names, nscalars, is_sum, &impl));
     soax_expr* e = new (std::nothrow) soax_expr();
-    if (e) { e->impl = impl; e->layout = l; }
     if (!e) { expr_free(impl); return SOAX_ERR_ALLOC; }
+    e->impl = impl;
+    e->layout = l;
     *out = e;
     return SOAX_OK;
+}
+
+int soax_expr_compile(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars,
+                      soax_expr** out) {
+    return expr_compile_any(l, source, scalar_names, nscalars, false, out);
+}
+
+int soax_expr_compile_sum(const soax_layout* l, const char* expression, const char* const* scalar_names, int32_t nscalars,
+                          soax_expr** out) {
+    return expr_compile_any(l, expression, scalar_names, nscalars, true, out);
+}
+
+int soax_expr_sum(const soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* dev_scratch, size_t scratch_bytes,
+                  double* dev_out, void* stream) {
+    if (!s || !e || !dev_scratch || !dev_out || !aligned(dev_scratch, 8) || !aligned(dev_out, 8) || nscalars < 0 || nscalars > 16)
+        return SOAX_ERR_INVALID_ARG;
+    if (s->layout != e->layout) return SOAX_ERR_INVALID_ARG;
+    if (scratch_bytes < kEnergyScratchBytes) return SOAX_ERR_ALLOC;
+    return expr_sum(e->impl, s->layout, const_cast<void* const*>(s->comp), s->n, scalars, nscalars, static_cast<double*>(dev_scratch),
+                    dev_out, (cudaStream_t)stream);
 }
 
 int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, int32_t nsteps, void* stream) {

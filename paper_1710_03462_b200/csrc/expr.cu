@@ -126,6 +126,7 @@ struct Program {
     std::vector<bool> assigned;    // component is assigned: must be stored
     std::vector<bool> touched;
     std::string body;              // statements over the locals, one particle
+    bool is_sum = false;           // the program is ONE expression whose per-particle value is summed in double
 };
 
 std::string hex_double(double v) {
@@ -145,6 +146,16 @@ class Parser {
             statement();
             if (peek().kind != Tok::END && !is_op(";")) fail("expected ';' between statements");
         }
+    }
+
+    // a reduction program: one floating-point expression, summed over the particles in double
+    void sum_expression() {
+        Val v = expr();
+        if (is_op(";")) next();
+        if (peek().kind != Tok::END) fail("a sum program is a single expression");
+        if (v.ty == T_ILIT) v = to_float(v, T_F64, 0);
+        if (!is_float(v.ty)) fail("the summed expression must be a floating-point value (use float()/double())");
+        P_.body += "        acc += (double)" + v.code + ";\n";
     }
 
   private:
@@ -462,13 +473,14 @@ std::string generate(const Program& P) {
     std::string s = "// generated by soax_expr_compile -- one fused pass, 4 particles per thread\n";
     s += kPrelude;
     s += "struct Args { void* p[" + std::to_string(L.ncomp) + "]; double s[" + std::to_string(P.scalar_names.empty() ? 1 : P.scalar_names.size()) + "]; };\n";
-    s += "template <int P> __device__ __forceinline__ void group(const Args& a, long long i0) {\n";
+    s += std::string("template <int P> __device__ __forceinline__ ") + (P.is_sum ? "double" : "void") + " group(const Args& a, long long i0) {\n";
     for (int c = 0; c < L.ncomp; ++c) {
         if (!P.touched[c]) continue;
         const std::string T = c_name(L.cdtype[c]), v = "v" + std::to_string(c);
         if (P.read_first[c]) s += "    Vec<" + T + ", P> " + v + " = ld_vec<" + T + ", P>(static_cast<const " + T + "*>(a.p[" + std::to_string(c) + "]) + i0);\n";
         else s += "    Vec<" + T + ", P> " + v + ";\n";
     }
+    if (P.is_sum) s += "    double acc = 0.0;\n";
     s += "#pragma unroll\n    for (int j = 0; j < P; ++j) {\n";
     for (int c = 0; c < L.ncomp; ++c)
         if (P.touched[c]) s += "        " + std::string(c_name(L.cdtype[c])) + "& x" + std::to_string(c) + " = v" + std::to_string(c) + ".v[j];\n";
@@ -479,8 +491,10 @@ std::string generate(const Program& P) {
             const std::string T = c_name(L.cdtype[c]);
             s += "    st_vec<" + T + ", P>(static_cast<" + T + "*>(a.p[" + std::to_string(c) + "]) + i0, v" + std::to_string(c) + ");\n";
         }
+    if (P.is_sum) s += "    return acc;\n";
     s += "}\n";
-    s += R"K(extern "C" __global__ void __launch_bounds__(512) soax_expr_kernel(const Args a, const long long n) {
+    if (!P.is_sum) {
+        s += R"K(extern "C" __global__ void __launch_bounds__(512) soax_expr_kernel(const Args a, const long long n) {
     const long long ngroups = n / 4;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -489,6 +503,36 @@ std::string generate(const Program& P) {
     if (t < n) group<1>(a, t);
 }
 )K";
+    } else {
+        // the reduction tree of the hand-written energy kernel (reduce_kernels.cu), restated: per-thread sums in grid-stride
+        // order, warp shuffles, one shared-memory step; a fixed grid makes the result run-to-run deterministic
+        s += R"K(__device__ __forceinline__ double warp_sum(double x) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    return x;
+}
+extern "C" __global__ void __launch_bounds__(256) soax_expr_kernel(const Args a, const long long n, double* partial) {
+    __shared__ double sm[32];
+    const long long ngroups = n / 4;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double s = 0.0;
+    for (long long g = tid; g < ngroups; g += stride) s += group<4>(a, g * 4);
+    const long long t = ngroups * 4 + tid;
+    if (t < n) s += group<1>(a, t);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+    s = warp_sum(s);
+    __syncthreads();
+    if (lane == 0) sm[warp] = s;
+    __syncthreads();
+    if (warp == 0) {
+        s = lane < nwarp ? sm[lane] : 0.0;
+        s = warp_sum(s);
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+)K";
+    }
     return s;
 }
 
@@ -586,6 +630,7 @@ struct CompiledExpr {
     const void* layout_key = nullptr;
     int ncomp = 0, nscalars = 0;
     int bytes_read = 0, bytes_written = 0;
+    bool is_sum = false;
     std::string source, cuda_source;
     std::vector<char> cubin;
     std::mutex mu;
@@ -594,7 +639,7 @@ struct CompiledExpr {
 };
 
 int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* source, const char* const* scalar_names,
-                 int nscalars, CompiledExpr** out) {
+                 int nscalars, bool is_sum, CompiledExpr** out) {
     g_expr_error.clear();
     Program P;
     P.L = &L;
@@ -608,8 +653,10 @@ int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* so
     P.assigned.assign(L.ncomp, false);
     P.touched.assign(L.ncomp, false);
     try {
+        P.is_sum = is_sum;
         Parser parser(source, P);
-        parser.program();
+        if (is_sum) parser.sum_expression();
+        else parser.program();
     } catch (const ParseError& e) {
         char where[64];
         std::snprintf(where, sizeof where, " (at character %zu)", e.pos);
@@ -618,12 +665,13 @@ int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* so
     }
     bool any = false;
     for (int c = 0; c < L.ncomp; ++c) any |= P.assigned[c];
-    if (!any) { g_expr_error = "the program assigns nothing"; return SOAX_ERR_INVALID_ARG; }
+    if (!any && !is_sum) { g_expr_error = "the program assigns nothing"; return SOAX_ERR_INVALID_ARG; }
     std::unique_ptr<CompiledExpr> E(new (std::nothrow) CompiledExpr());
     if (!E) return SOAX_ERR_ALLOC;
     E->layout_key = layout_key;
     E->ncomp = L.ncomp;
     E->nscalars = nscalars;
+    E->is_sum = is_sum;
     E->source = source;
     for (int c = 0; c < L.ncomp; ++c) {
         if (P.read_first[c]) E->bytes_read += L.csize[c];
@@ -642,7 +690,7 @@ int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* so
 
 int expr_run(CompiledExpr* E, const void* layout_key, void* const* comps, int64_t n, const double* scalars, int nscalars,
              cudaStream_t st) {
-    if (E->layout_key != layout_key) return SOAX_ERR_INVALID_ARG;
+    if (E->layout_key != layout_key || E->is_sum) return SOAX_ERR_INVALID_ARG;
     if (nscalars != E->nscalars || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
     {
         std::lock_guard<std::mutex> lock(E->mu);
@@ -663,6 +711,31 @@ int expr_run(CompiledExpr* E, const void* layout_key, void* const* comps, int64_
     const int64_t blocks = (threads + block - 1) / block;
     SOAX_CUDA(cudaLaunchKernel(reinterpret_cast<const void*>(E->kernel), dim3((unsigned)(blocks < 1 ? 1 : blocks)), dim3((unsigned)block), params, 0, st));
     return launched();
+}
+
+int sum_partials(const double* partial, int m, double* out, cudaStream_t st);  // reduce_kernels.cu
+
+// A sum program: per-CTA partials from the generated kernel (fixed grid, as the hand-written energy reduction), then the
+// library's own fixed-order sum of the partials.
+int expr_sum(CompiledExpr* E, const void* layout_key, void* const* comps, int64_t n, const double* scalars, int nscalars,
+             double* partial, double* out, cudaStream_t st) {
+    if (E->layout_key != layout_key || !E->is_sum) return SOAX_ERR_INVALID_ARG;
+    if (nscalars != E->nscalars || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
+    {
+        std::lock_guard<std::mutex> lock(E->mu);
+        if (!E->kernel) {
+            SOAX_CUDA(cudaLibraryLoadData(&E->lib, E->cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0));
+            SOAX_CUDA(cudaLibraryGetKernel(&E->kernel, E->lib, "soax_expr_kernel"));
+        }
+    }
+    std::vector<unsigned char> args((size_t)E->ncomp * sizeof(void*) + (size_t)(nscalars > 0 ? nscalars : 1) * sizeof(double), 0);
+    std::memcpy(args.data(), comps, (size_t)E->ncomp * sizeof(void*));
+    if (nscalars > 0) std::memcpy(args.data() + (size_t)E->ncomp * sizeof(void*), scalars, (size_t)nscalars * sizeof(double));
+    long long nn = n;
+    void* params[] = {args.data(), &nn, &partial};
+    SOAX_CUDA(cudaLaunchKernel(reinterpret_cast<const void*>(E->kernel), dim3(kEnergyBlocks), dim3(256), params, 0, st));
+    SOAX_TRY(launched());
+    return sum_partials(partial, kEnergyBlocks, out, st);
 }
 
 void expr_free(CompiledExpr* E) {

@@ -193,3 +193,38 @@ def test_dynamic_layout_descriptor_and_program(compiler):
         with pytest.raises(B.SoaxError) as ei:
             B.soax_layout_define_dynamic(bad)
         assert ei.value.status == B.SOAX_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------- reductions
+KE = "0.5 * fma(double(vel[2]), double(vel[2]), fma(double(vel[1]), double(vel[1]), double(vel[0]) * double(vel[0])))"
+KE_PE = ("0.5 * fma(k*(pos[2]-c), pos[2]-c, fma(k*(pos[1]-c), pos[1]-c, fma(k*(pos[0]-c), pos[0]-c, "
+         "fma(double(vel[2]), double(vel[2]), fma(double(vel[1]), double(vel[1]), double(vel[0]) * double(vel[0]))))))")
+
+
+def test_sum_oracle_against_the_pinned_energy_and_the_hand_fixture():
+    """tests/golden/energy_4particles.txt: KE 18.5, total 18.8125 (all dyadic: exact in any order)."""
+    vel = np.array([[1, 2, 2], [0, 0, 0], [3, 4, 0], [-1, -1, -1]], np.float32).T.copy()
+    pos = np.array([[.5, .5, .5], [0, .5, .5], [.25, .75, .5], [.5, .5, 0]], np.float64).T.copy()
+    f = {"id": np.arange(4, dtype=np.int32)[None], "pos": pos, "vel": vel}
+    assert oexpr.total(f, KE) == 18.5 and oexpr.total(f, KE_PE, {"k": 1.0, "c": 0.5}) == 18.8125
+    h = inputs.make_r1(50000, seed=8)
+    for src, kind in ((KE, oracle.KINETIC), (KE_PE, oracle.KINETIC_PLUS_HARMONIC)):
+        a, b = oexpr.total(h, src, {"k": 1.0, "c": 0.5}), oracle.energy(h, kind)
+        assert abs(a - b) <= 1e-13 * abs(b)                          # exact sum vs the oracle's compensated sum
+    assert oexpr.total(h, "1") == 50000.0 and oexpr.total(h, "double(id)") == 50000 * 49999 / 2
+    with pytest.raises(oexpr.ExprError):
+        oexpr.total(h, "id")
+
+
+def test_sum_program_compiles_to_one_reduction_kernel(compiler):
+    B, Cn = compiler
+    L = B.soax_layout_define(Cn.R1)
+    e = B.soax_expr_compile_sum(L, KE, [])
+    src = B.soax_expr_cuda_source(e)
+    assert src.count("__global__") == 1 and "partial[blockIdx.x]" in src and "st_vec<" not in src.split("struct Args")[1]
+    assert B.soax_expr_traffic(e) == (12, 0)                         # reads vel only: 12 B/particle, as the hand KE reduction
+    B.soax_expr_free(e)
+    for bad, msg in (("vel[0] = 1.0", "single expression"), ("id", "floating-point"), ("vel", "components"), ("pos[0] pos[1]", "single expression")):
+        with pytest.raises(B.SoaxError) as ei:
+            B.soax_expr_compile_sum(L, bad, [])
+        assert msg in str(ei.value), (bad, str(ei.value))
