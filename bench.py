@@ -700,11 +700,11 @@ def _run_soax(args) -> None:
         }
         if world == 1:
             t0 = time.perf_counter()
-            n_sample = 1 << 21
+            n_sample = 1 << 22
             rate, secs = time_oracle(host, n_sample, NSTEPS)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs,
                                     "host_cores_available": os.cpu_count(),
-                                    "sample": f"first 2^21 of the 2^24 particles x {NSTEPS} symplectic-Euler steps + 2 energy sums, single thread"}
+                                    "sample": f"first 2^22 of the 2^24 particles x {NSTEPS} symplectic-Euler steps + 2 energy sums, single thread"}
             if not args.no_extras:
                 del pin, out
                 line["extras"] = run_extras(torch, B, Cn, s, peak)
