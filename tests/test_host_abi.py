@@ -180,3 +180,22 @@ def test_two_rank_sharding_gloo(tmp_path):
     for p, o in zip(procs, outs):
         assert p.returncode == 0, o
     assert sorted(o.strip().splitlines()[-1] for o in outs) == ["ok 0", "ok 1"]
+
+
+def test_maximum_sizes_are_refused_before_any_launch():
+    """Permutations, counts and offsets are uint32 (include/soax.h): 2^32 particles or more are UNSUPPORTED for binning and
+    removal.  Checked with fake device pointers: the calls must answer from their argument checks, without touching memory."""
+    L = B.soax_layout_define(Cn.R1)
+    n = 1 << 32
+    bytes_ = B.soax_slab_bytes(L, n)
+    assert bytes_ == 7 * 0 + (4 + 3 * 8 + 3 * 4) * n                  # every array of 2^32 elements is already 256-byte aligned
+    fake = 1 << 40
+    a = B.soax_alloc(L, n, n, fake, bytes_)
+    b = B.soax_alloc(L, 0, n, fake + bytes_, bytes_)
+    for call in (lambda: B.soax_bin_permute(a, b, 64, 0.0, None, None, None, None, 256, 1 << 62),
+                 lambda: B.soax_remove(a, None, 256, B.SOAX_REMOVE_SWAP_LAST, 256, 1 << 62)):
+        with pytest.raises(B.SoaxError) as e:
+            call()
+        assert e.value.status == B.SOAX_ERR_UNSUPPORTED
+    assert B.soax_scratch_bytes(L, (1 << 32) - 1, 64) > 40 * ((1 << 32) - 1)     # the plan itself is computed in 64 bits
+    B.soax_free(a), B.soax_free(b)
