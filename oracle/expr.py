@@ -72,6 +72,7 @@ class _Eval:
     def __init__(self, fields: dict, dims: dict, scalars: dict, n: int):
         self.f, self.dims, self.s, self.n = fields, dims, scalars, n
         self.vec_c = None
+        self.vec_dim = 0
 
     def _full(self, x, dt):
         return np.broadcast_to(_to(x, dt), (self.n,)).astype(dt)
@@ -82,8 +83,8 @@ class _Eval:
         dim = self.dims[name]
         if c is None:
             if dim > 1:
-                if self.vec_c is None or self.vec_c >= dim:
-                    raise ExprError(f"field {name!r} needs a component index")
+                if self.vec_c is None or dim != self.vec_dim:
+                    raise ExprError(f"field {name!r} needs a component index (or the dimension of the vector statement's target)")
                 c = self.vec_c
             else:
                 c = 0
@@ -252,6 +253,7 @@ def run(fields: dict, source: str, scalars: dict | None = None) -> dict:
         tname = target.id if isinstance(target, ast.Name) else getattr(getattr(target, "value", None), "id", None)
         ev = _Eval(state, dims, scalars, n)
         vector_form = isinstance(target, ast.Name) and tname in dims and dims[tname] > 1
+        ev.vec_dim = dims.get(tname, 0)
         for c in (range(dims[tname]) if vector_form else [None]):
             ev.vec_c = c
             ev.assign(target, op, value)

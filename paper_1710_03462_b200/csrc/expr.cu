@@ -163,6 +163,7 @@ class Parser {
     size_t at_ = 0;
     Program& P_;
     int vec_c_ = -1;  // component index substituted for un-indexed dim-3 fields in the statement being expanded
+    int vec_dim_ = 0; // dimension of the target of that statement
 
     const Tok& peek() const { return toks_[at_]; }
     Tok next() { return toks_[at_++]; }
@@ -196,7 +197,7 @@ class Parser {
             if (c < 0 || c >= dim) throw ParseError{"component " + std::to_string(c) + " is outside field '" + id.text + "' of dimension " + std::to_string(dim) + " (PAPER.md:320)", id.pos};
         } else if (dim > 1) {
             if (vec_c_ < 0) throw ParseError{"field '" + id.text + "' has " + std::to_string(dim) + " components: index it, or assign to a vector field", id.pos};
-            if (vec_c_ >= dim) throw ParseError{"vector statement mixes fields of different dimension at '" + id.text + "'", id.pos};
+            if (dim != vec_dim_) throw ParseError{"vector statement mixes fields of different dimension at '" + id.text + "'", id.pos};
             c = vec_c_;
         }
         return P_.L->fbegin[f] + c;
@@ -215,6 +216,7 @@ class Parser {
         const bool vector_form = P_.L->fdim[f] > 1 && !(toks_[at_ + 1].kind == Tok::OP && toks_[at_ + 1].text == "[");
         const int reps = vector_form ? P_.L->fdim[f] : 1;
         size_t end = at_;
+        vec_dim_ = P_.L->fdim[f];
         for (int r = 0; r < reps; ++r) {
             at_ = start;
             vec_c_ = vector_form ? r : -1;

@@ -88,10 +88,10 @@ def test_hand_values_sequencing_vector_form_and_masks():
 
 
 @pytest.mark.parametrize("bad", ["pos[3] = 1.0", "pos = id", "foo = 1.0", "id = 1.0", "pos[0] = select(vel[0], 1, 2)",
-                                 "pos[0] = vel", "pos[0] = flags + 1.0", "pos[0] = frob(1.0)"])
+                                 "pos[0] = vel", "pos[0] = flags + 1.0", "pos[0] = frob(1.0)", "pos = five"])
 def test_oracle_rejects_what_the_language_rejects(bad):
     f = {"id": np.zeros((1, 2), np.int32), "pos": np.zeros((3, 2)), "vel": np.zeros((3, 2), np.float32),
-         "flags": np.zeros((1, 2), np.uint8)}
+         "flags": np.zeros((1, 2), np.uint8), "five": np.zeros((5, 2))}
     with pytest.raises(oexpr.ExprError):
         oexpr.run(f, bad)
 
@@ -189,6 +189,9 @@ def test_dynamic_layout_descriptor_and_program(compiler):
     e = B.soax_expr_compile(L, "w[4] = select(alive != 0, w[0] * double(temperature) + x[1], w[4]); x = x * 2", [])
     assert B.soax_expr_traffic(e) == (1 + 8 + 4 + 8 + 8 + 8, 8 + 16)
     B.soax_expr_free(e)
+    with pytest.raises(B.SoaxError) as ei:
+        B.soax_expr_compile(L, "x = w", [])                          # a 5-vector in a 2-vector statement
+    assert "different dimension" in str(ei.value)
     for bad in ([("a b", B.SOAX_F32, 1), ("c", B.SOAX_F32, 1)], [("a", B.SOAX_F32, 1), ("a", B.SOAX_F64, 1)], [("a", B.SOAX_F32, 49)]):
         with pytest.raises(B.SoaxError) as ei:
             B.soax_layout_define_dynamic(bad)
