@@ -617,27 +617,27 @@ def _run_soax(args) -> None:
     e2e_serial = world * n * NSTEPS * args.steps / (float(ms2.item()) * 1e-3)
     e2e_check = bool(np.isfinite(out["pos"].numpy()).all())
 
-    # The same end-to-end step, software-pipelined over two containers and three streams: while step k computes, the
+    # The same end-to-end step, software-pipelined over three containers and three streams: while step k computes, the
     # inputs of step k+1 are uploaded and the results of step k-1 are downloaded (PCIe is full duplex).  Every step still
     # uploads its own inputs from pinned host memory, runs energy + 100 launches + energy, and downloads pos, vel and the
     # energies, which the host reads before the buffer is used again.
-    s2 = Cn.Soax(Cn.R1, n)
-    conts = [s, s2]
-    out2 = {"pos": torch.empty((3, n), dtype=torch.float64).pin_memory(), "vel": torch.empty((3, n), dtype=torch.float32).pin_memory()}
-    outs = [out, out2]
+    NB = 3                                                    # three buffers: with two, the upload of step k has to wait for
+    conts = [s] + [Cn.Soax(Cn.R1, n) for _ in range(NB - 1)]  # the download of step k-2 and delays the compute of step k
+    outs = [out] + [{"pos": torch.empty((3, n), dtype=torch.float64).pin_memory(), "vel": torch.empty((3, n), dtype=torch.float32).pin_memory()}
+                    for _ in range(NB - 1)]
     dn_ptrs2 = [[None] + [o["pos"][c].data_ptr() for c in range(3)] + [o["vel"][c].data_ptr() for c in range(3)] for o in outs]
-    e_bufs = [torch.zeros(2, dtype=torch.float64, device="cuda") for _ in range(2)]
-    e_hosts = [torch.empty(2, dtype=torch.float64).pin_memory() for _ in range(2)]
+    e_bufs = [torch.zeros(2, dtype=torch.float64, device="cuda") for _ in range(NB)]
+    e_hosts = [torch.empty(2, dtype=torch.float64).pin_memory() for _ in range(NB)]
     cp = torch.cuda.current_stream()
     up, dn = torch.cuda.Stream(), torch.cuda.Stream()
-    ev = {k: [torch.cuda.Event() for _ in range(2)] for k in ("up", "comp", "down")}
+    ev = {k: [torch.cuda.Event() for _ in range(NB)] for k in ("up", "comp", "down")}
     consumed = []
 
     def pipelined(steps):
         for k in range(steps):
-            b = k & 1
-            if k >= 2:
-                ev["down"][b].synchronize()                    # the host consumes the result of step k-2 ...
+            b = k % NB
+            if k >= NB:
+                ev["down"][b].synchronize()                    # the host consumes the result of step k-NB ...
                 consumed.append(float(e_hosts[b][1]))         # ... before its buffers are reused
                 up.wait_event(ev["down"][b])
             B.soax_upload(conts[b].handle, up_ptrs, n, up.cuda_stream)
@@ -652,12 +652,12 @@ def _run_soax(args) -> None:
             with torch.cuda.stream(dn):
                 e_hosts[b].copy_(e_bufs[b], non_blocking=True)
             ev["down"][b].record(dn)
-        for b in range(2):
+        for b in range(min(NB, steps)):
             ev["down"][b].synchronize()
             consumed.append(float(e_hosts[b][1]))
             cp.wait_event(ev["down"][b])
 
-    pipelined(max(2, min(args.warmup, 4)))
+    pipelined(max(NB, min(args.warmup, 4)))
     barrier()
     t_a.record()
     pipelined(args.steps)
@@ -667,9 +667,9 @@ def _run_soax(args) -> None:
     if world > 1:
         dist.all_reduce(ms3, op=dist.ReduceOp.MAX)
     e2e_value = world * n * NSTEPS * args.steps / (float(ms3.item()) * 1e-3)
-    e2e_check = e2e_check and bool(np.isfinite(out2["pos"].numpy()).all()) and bool(np.isfinite(consumed).all()) \
+    e2e_check = e2e_check and all(bool(np.isfinite(o["pos"].numpy()).all()) for o in outs[1:]) and bool(np.isfinite(consumed).all()) \
         and abs(consumed[-1] - float(e_host[1])) <= 1e-9 * abs(float(e_host[1]))   # same inputs every step: same energy
-    del s2, out2
+    del conts, outs
 
     if rank == 0:
         peak, peak_src = measured_peak()
@@ -687,7 +687,7 @@ def _run_soax(args) -> None:
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 40 * n, "d2h_bytes_per_step": 36 * n + 16,
                     "ms_per_step": float(ms3.item()) / args.steps, "finite": e2e_check,
                     "path": "per step: soax_upload (7 pinned host arrays) -> soax_reduce_energy, 100 x soax_step, soax_reduce_energy -> "
-                            "soax_download (pos, vel) + energies, read by the host; software-pipelined over two containers and three "
+                            "soax_download (pos, vel) + energies, read by the host; software-pipelined over three containers and three "
                             "streams (upload of step k+1 and download of step k-1 overlap the compute of step k)",
                     "serial_value": e2e_serial, "serial_ms_per_step": float(ms2.item()) / args.steps,
                     "serial_path": "the same step with nothing overlapped: upload, compute, download, synchronise"},
