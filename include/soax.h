@@ -236,8 +236,10 @@ int soax_copy(soax_t* dst, const soax_t* src, void* stream);
  * 128/256-bit accesses, every array it assigns is stored once, 4 particles per thread like the built-in step
  * kernels) and compiles it for sm_100a with NVRTC; soax_expr_run launches it on the live particles.
  *   program := stmt { ';' stmt }       stmt := target ('=' | '+=' | '-=' | '*=' | '/=') expr
- *   target  := field | field[c]        a float or double field; a dim-3 field without index expands the statement
- *                                      over c = 0, 1, 2 with every un-indexed dim-3 field read as its component c
+ *   target  := field | field[c]        a float or double field; a multi-component field without index expands the
+ *                                      statement over its components c = 0, 1, ...; every other un-indexed
+ *                                      multi-component field in it must have the same dimension and is read as its
+ *                                      component c (scalar fields are read as they are)
  *   expr    := + - * / unary-  < <= > >= == !=  &  ( )  numbers  scalar names  field reads  and the calls
  *              fma(a,b,c) sqrt(x) abs(x) min(a,b) max(a,b) floor(x) wrap(x) float(x) double(x) select(cond,a,b)
  * Semantics: statements run in order for each particle and later statements see earlier assignments; typing is
