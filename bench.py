@@ -277,7 +277,20 @@ def _extra_config3(torch, B, Cn, s, peak, ex, gbs, iters):
     ms_s2a = ev_time_ms(torch, lambda: s.to_aos(aos), 20)
     ms_aos0 = ev_time_ms(torch, lambda: Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, NSTEPS, 0), iters, 1) / NSTEPS
     ms_aos1 = ev_time_ms(torch, lambda: Cn.aos_step(Cn.R1, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, NSTEPS, 1), iters, 1) / NSTEPS
+    # Q1 sensitivity row: the same fields declared {pos; vel; id} -- packed offsets 0/24/36, doubles 8-byte aligned
+    sr = Cn.Soax(Cn.R1R, n)
+    for name, dim in (("pos", 3), ("vel", 3), ("id", 1)):
+        for c in range(dim):
+            sr.comp_view(name, c).copy_(s.comp_view(name, c))
+    aos_r = sr.to_aos()
+    ms_r0 = ev_time_ms(torch, lambda: Cn.aos_step(Cn.R1R, aos_r, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, NSTEPS, 0), iters, 1) / NSTEPS
+    ms_r1 = ev_time_ms(torch, lambda: Cn.aos_step(Cn.R1R, aos_r, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, NSTEPS, 1), iters, 1) / NSTEPS
+    ms_ra2s = ev_time_ms(torch, lambda: sr.from_aos(aos_r, n), 20)
+    del sr, aos_r
     ex["config3_aos_vs_soa"] = {
+        "reordered_record_pos_vel_id": {"aos_step_ms_thread_per_record": ms_r0, "aos_step_ms_smem_staged": ms_r1,
+                                        "soa_over_aos_speedup": ms_r0 / ms_soa, "aos_to_soa_ms": ms_ra2s,
+                                        "note": "Q1 sensitivity: doubles naturally aligned (one 64-bit access instead of two 32-bit ones)"},
         "n": n, "soa_step_ms": ms_soa, "aos_step_ms_thread_per_record": ms_aos0, "aos_step_ms_smem_staged": ms_aos1,
         "soa_over_aos_speedup": ms_aos0 / ms_soa, "soa_over_staged_aos_speedup": ms_aos1 / ms_soa,
         "aos_to_soa_ms": ms_a2s, "soa_to_aos_ms": ms_s2a,

@@ -60,7 +60,8 @@ typedef struct soax_container soax_t;            /* opaque container: layout + n
 /* ---- layout registry (Listing 5; D7/D8 of the component inventory) ----------------------
  * Layouts are COMPILE-TIME typelists (csrc/layout.hpp) whose kernels are generated from C++ templates; this
  * call canonicalises a run-time field list (names, dtypes and dims, in declaration order) and returns the
- * matching instantiation.  Built in: R1 {int32 id; double pos[3]; float vel[3]}, R2 {int64 id;
+ * matching instantiation.  Built in: R1 {int32 id; double pos[3]; float vel[3]}, R1R {double pos[3];
+ * float vel[3]; int32 id} (the same record with naturally aligned AoS offsets: the Q1 sensitivity row), R2 {int64 id;
  * double pos[3]; double vel[3]; double acc[3]; float mass; float charge; uint8 flags} (BASELINE.json config
  * 4) and B6_S {float pos[3]; float vel[3]; float temp[S]} for S in {0, 8, 16, 32}.
  * Errors: INVALID_ARG (null, nfields <= 0, bad dtype/dim), UNKNOWN_LAYOUT. */

@@ -12,6 +12,7 @@ from . import binding as B
 
 # layouts as (name, soax_dtype, dim) lists, declaration order (BASELINE.json config 4)
 R1 = (("id", B.SOAX_I32, 1), ("pos", B.SOAX_F64, 3), ("vel", B.SOAX_F32, 3))
+R1R = (("pos", B.SOAX_F64, 3), ("vel", B.SOAX_F32, 3), ("id", B.SOAX_I32, 1))      # Q1 sensitivity row: naturally aligned AoS
 R2 = (("id", B.SOAX_I64, 1), ("pos", B.SOAX_F64, 3), ("vel", B.SOAX_F64, 3), ("acc", B.SOAX_F64, 3),
       ("mass", B.SOAX_F32, 1), ("charge", B.SOAX_F32, 1), ("flags", B.SOAX_U8, 1))
 

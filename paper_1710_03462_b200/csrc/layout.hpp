@@ -143,6 +143,9 @@ struct CompRegs<L, C0, N, std::integer_sequence<int, Is...>> : CompSlot<C0 + Is,
 // ---- the layouts this library instantiates -----------------------------------------------------------------
 // R1: the program summary's record: configs 1, 2, 3, 5.
 using R1 = Layout<Field<id_tag, int32_t, 1>, Field<pos_tag, double, 3>, Field<vel_tag, float, 3>>;
+// R1R: the same fields declared {pos; vel; id}: packed offsets 0 / 24 / 36, stride 40, every field naturally aligned --
+// the sensitivity row of reading Q1 (what config 3's AoS kernels gain when the doubles are 8-byte aligned).
+using R1R = Layout<Field<pos_tag, double, 3>, Field<vel_tag, float, 3>, Field<id_tag, int32_t, 1>>;
 // R2: the wide heterogeneous record of BASELINE.json config 4.
 using R2 = Layout<Field<id_tag, int64_t, 1>, Field<pos_tag, double, 3>, Field<vel_tag, double, 3>,
                   Field<acc_tag, double, 3>, Field<mass_tag, float, 1>, Field<charge_tag, float, 1>,
@@ -153,6 +156,7 @@ template <> struct B6_of<0> { using type = Layout<Field<pos_tag, float, 3>, Fiel
 template <int S> using B6 = typename B6_of<S>::type;
 
 static_assert(R1::ncomp == 7 && R1::aos_stride == 40 && R1::aos_offset(1) == 4 && R1::aos_offset(4) == 28, "R1 (Q1)");
+static_assert(R1R::aos_stride == 40 && R1R::aos_offset(3) == 24 && R1R::aos_offset(6) == 36, "R1R (Q1 sensitivity row)");
 static_assert(R2::ncomp == 13 && R2::aos_stride == 89, "R2");
 static_assert(B6<0>::aos_stride == 24 && B6<32>::aos_stride == 152, "PAPER.md:237: 24 bytes at SIZE=0");
 

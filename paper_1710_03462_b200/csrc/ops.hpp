@@ -8,7 +8,7 @@
 #include "layout.hpp"
 
 // The layouts compiled into the library.  Adding a layout = one line here (and a `using` in layout.hpp).
-#define SOAX_FOR_EACH_LAYOUT(X) X(R1) X(R2) X(B6<0>) X(B6<8>) X(B6<16>) X(B6<32>)
+#define SOAX_FOR_EACH_LAYOUT(X) X(R1) X(R1R) X(R2) X(B6<0>) X(B6<8>) X(B6<16>) X(B6<32>)
 
 namespace soax {
 

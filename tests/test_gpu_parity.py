@@ -409,3 +409,26 @@ def test_error_codes(gpu):
     with pytest.raises(B.SoaxError) as e:
         b6.bin_permute(Cn.Soax(Cn.B6(0), 10), 4, scratch=torch.empty(1 << 20, dtype=torch.uint8, device="cuda"))
     assert e.value.status == B.SOAX_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_reordered_record_aos_kernels(gpu, variant):
+    """Q1 sensitivity row: the record declared {pos; vel; id} (packed offsets 0/24/36, naturally aligned).  Same fields,
+    same arithmetic: the SoA kernel must match the oracle, and SoA kernel + SoA->AoS must reproduce the AoS kernel's bytes."""
+    torch, B, Cn = gpu
+    n = 70001
+    host = inputs.make_r1(n, seed=9)
+    stride, offs = B.soax_layout_aos(B.soax_layout_define(Cn.R1R), True)
+    assert stride == 40 and offs == [0, 8, 16, 24, 28, 32, 36]
+    s = to_device(Cn, Cn.R1R, host)
+    aos = s.to_aos()
+    packed = np.zeros(n, np.dtype({"names": ["pos", "vel", "id"], "formats": [("<f8", 3), ("<f4", 3), "<i4"], "offsets": [0, 24, 36], "itemsize": 40}))
+    packed["pos"], packed["vel"], packed["id"] = host["pos"].T, host["vel"].T, host["id"][0]
+    assert np.array_equal(aos.cpu().numpy(), packed.view(np.uint8).reshape(-1))       # the packed image is the numpy struct
+    s.step(B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=7)
+    check_r1(s.download(), oracle.symplectic_euler(host, DT, 7))
+    Cn.aos_step(Cn.R1R, aos, n, B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, DT, nsteps=7, variant=variant)
+    assert torch.equal(s.to_aos(), aos)
+    t = Cn.Soax(Cn.R1R, n)
+    t.from_aos(aos, n)
+    check_r1(t.download(), oracle.symplectic_euler(host, DT, 7))
