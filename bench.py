@@ -313,7 +313,9 @@ def _extra_config4(torch, B, Cn, peak, ex, gbs, iters):
     s4 = Cn.Soax(Cn.R2, n4)
     device_fill(torch, s4, 0)
     ms = ev_time_ms(torch, lambda: s4.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=20, k=1.0, flag_mask=1), iters, 1) / 20
+    active = int((s4.comp_view("flags") & 1).sum().item())
     ex["config4_rk2_masked"] = {"n": n4, "ms_per_step": ms, "particle_steps_per_s": n4 / (ms * 1e-3),
+                                "active_particles": active, "active_particle_steps_per_s": active / (ms * 1e-3),
                                 "GBps_63B_byte_granular": gbs(63, n4, ms), "GBps_117p5B_sector_granular": gbs(117.5, n4, ms),
                                 "frac_of_peak_117p5B": gbs(117.5, n4, ms) / peak}
     del s4
