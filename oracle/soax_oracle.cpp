@@ -12,7 +12,9 @@
 // and the linear closed form of the symplectic-Euler map, the exact RK2 energy growth factor, the 4-particle
 // dyadic energy fixture, exact rational summation, byte-exact AoS<->SoA round trips against numpy structured
 // arrays, the 6-particle binning fixture of SURVEY.md 8(c), O(N^2) brute-force ranks for N <= 64, and
-// numpy's stable argsort at larger N.  No function here is "parity unpinned".
+// numpy's stable argsort at larger N; the energy of the wide record (double vel) by the same fixture stored as R2
+// and by exact rationals.  No arithmetic function here is "parity unpinned" (the seeded input generator lives in
+// paper_1710_03462_b200/inputs.py, is unpinned, and feeds both sides the same arrays).
 //
 // Records (declaration order, SURVEY.md section 8 "Records used by the configs"):
 //   R1  PAPER.md:41  {int32 id; double pos[3]; float vel[3]}  packed, stride 40, offsets 0/4,12,20/28,32,36 (Q1)

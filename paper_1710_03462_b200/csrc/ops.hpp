@@ -21,8 +21,10 @@ struct Tuning {
     int aos_block = 256;
     int xpose_ring = 1;     // 1: pipelined ring transposes (default), 0: one tile per CTA visit
     int xpose_r = 0, xpose_ns = 0, xpose_ctas = 0;  // ring shape override: 256*r records per stage, ns stages, CTAs per SM cap (0 = default)
-    int bin_bits = 0;       // digit width of the counting-sort passes: 0 = default (6), else 1..9
-    int bin_stage = 2;      // 2: TMA-ring scatter (default), 1: shared-memory staged scatter, 0: direct scatter
+    int bin_bits = 0;       // digit width of the counting-sort passes: 0 = default (9: two passes for G = 64), else 1..9
+    int bin_cluster = 0;    // 0 = default (clusters of 4 CTAs for digits of 8 or 9 bits, none below); 1, 2, 4, 8, 16: forced
+    int bin_pace = -1;      // pacing of the scatter stores: -1 = default; else bit 12 = CTA barrier between a thread's stores, low 12 bits = nanoseconds of sleep
+    int bin_csync = 1;      // with clusters: 1 = cluster barrier before every array's stores (default), 0 = none
 };
 extern Tuning g_tune;
 

@@ -1,10 +1,11 @@
-"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default tuning).
+"""GPU parity at BASELINE.json's FULL sizes, on the inputs the configs name (inputs.make_r1 / make_r2 with the config's
+seed), in the launch configuration bench.py times (default tuning).
 
-The oracle cannot step 2^24..2^27 particles in seconds, but particles are independent, so it is run on SAMPLED
-particles (the same seeded inputs, gathered before the device steps) and compared bit for bit with the device's
-result at those indices; whole-array statements use properties that hold at any size and library routines that are
-independent of the CUDA path (torch.sort(stable=True) for the unique stable permutation, torch.bincount / cumsum for
-counts and offsets, a gather for the permuted arrays)."""
+The oracle cannot STEP 2^24..2^26 particles 20-100 times in seconds, but particles are independent, so the integrators are
+checked on SAMPLED particles (oracle on the same seeded inputs, bit for bit) plus whole-array properties; the energy sums
+and config 5 (one drift step + binning) are compared with the oracle over ALL particles."""
+import os
+
 import numpy as np
 import pytest
 
@@ -43,10 +44,6 @@ def gather(torch, s, idx):
         out[name] = np.stack([s.comp_view(name, c)[t].cpu().numpy() for c in range(dim)])
     return out
 
-
-def device_fill(torch, s, seed):
-    from bench import device_fill as fill
-    fill(torch, s, seed)
 
 
 def test_config2_full_size_sampled(gpu):
@@ -89,12 +86,15 @@ def test_config2_full_size_sampled(gpu):
 
 
 def test_config4_full_size_sampled(gpu):
+    """BASELINE.json config 4 as written: N = 2^26, record R2, inputs.make_r2(seed 0), 20 masked RK2 steps."""
     torch, B, Cn = gpu
     n = 1 << 26
+    host = inputs.make_r2(n, seed=0, threads=os.cpu_count() or 8)
     s = Cn.Soax(Cn.R2, n)
-    device_fill(torch, s, 0)
+    s.upload(host)
     idx = sample_indices(n)
-    before = gather(torch, s, idx)
+    before = inputs.take(host, idx)
+    e_before = s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC)
     s.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=20, k=1.0, flag_mask=1)
     got = gather(torch, s, idx)
     exp = oracle.rk2_midpoint_masked(before, DT, 20, k=1.0, mask=1)
@@ -105,47 +105,59 @@ def test_config4_full_size_sampled(gpu):
     assert (got["acc"][:, ~active] == 0).all() and (got["acc"][:, active] != 0).any()
     pos = torch.stack([s.comp_view("pos", c) for c in range(3)])
     assert bool((pos >= 0).all()) and bool((pos < 1).all())
+    del pos
+    # fields the step must not touch, bitwise over ALL particles; inactive particles bitwise unchanged in every field
+    for name in ("id", "mass", "charge", "flags"):
+        assert torch.equal(s.comp_view(name).cpu(), torch.from_numpy(host[name][0])), name
+    inactive = torch.from_numpy((host["flags"][0] & 1) == 0)
+    for name in ("pos", "vel", "acc"):
+        for c in range(3):
+            assert torch.equal(s.comp_view(name, c).cpu()[inactive], torch.from_numpy(host[name][c])[inactive]), (name, c)
+    # the energy reduction on the double-velocity record at full size (a8 on R2): oracle = compensated sum in index order
+    o_before = oracle.energy(host, oracle.KINETIC_PLUS_HARMONIC)
+    assert abs(e_before - o_before) <= 1e-10 * o_before
 
 
-def test_config5_full_size_properties(gpu):
+def test_config5_full_size_vs_oracle(gpu):
+    """BASELINE.json config 5 as written: N = 2^27, inputs.make_r1(seed 7), one drift step, 64^3 cells, counts, exclusive
+    scan, stable permutation applied to all arrays, kinetic energy -- ids, counts, offsets and the permutation compared
+    with the ORACLE over all 2^27 particles, bit for bit; every permuted array against oracle-drifted values gathered by
+    the oracle's permutation."""
     torch, B, Cn = gpu
     n, G = 1 << 27, 64
+    host = inputs.make_r1(n, seed=7, threads=os.cpu_count() or 8)
     src, dst = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
-    device_fill(torch, src, 7)
-    idx = sample_indices(n)
-    before = gather(torch, src, idx)
+    src.upload(host)
     r = src.bin_permute(dst, G, drift_dt=DT, want_kinetic=True)
     torch.cuda.synchronize()
     del r["scratch"]
     torch.cuda.empty_cache()
-    # fused drift, sampled against the oracle
-    after = gather(torch, src, idx)
-    exp = oracle.drift(before, DT, 1)
-    for name in exp:
-        assert np.array_equal(bits(after[name]), bits(exp[name])), name
-    # cell keys recomputed with torch from the drifted positions (exact: x*64 then truncation)
-    cell = torch.zeros(n, dtype=torch.int64, device="cuda")
-    for c in range(3):
-        cell = cell * G + (src.comp_view("pos", c) * float(G)).to(torch.int64)
-    assert int(cell.min()) >= 0 and int(cell.max()) < G ** 3
-    counts = torch.bincount(cell, minlength=G ** 3)
-    assert torch.equal(r["counts"].to(torch.int64), counts)
-    assert int(counts.sum()) == n
-    offs = torch.cumsum(counts, 0) - counts
-    assert torch.equal(r["offsets"].to(torch.int64), offs)
-    del counts, offs
-    # the stable permutation is unique: it must equal a stable argsort of the keys
-    perm = r["perm"].to(torch.int64)
-    _, order = torch.sort(cell.to(torch.int32), stable=True)
-    assert torch.equal(perm, order)
-    del order, cell
-    torch.cuda.empty_cache()
-    # every component array was permuted: new.f[j] == old.f[perm[j]] bitwise
-    for name, dt, dim in Cn.R1:
+    for name, dt, dim in Cn.R1:                                      # src is read only (the drift is applied on the way to dst)
         for c in range(dim):
-            assert torch.equal(dst.comp_view(name, c), src.comp_view(name, c)[perm]), (name, c)
+            assert torch.equal(src.comp_view(name, c).cpu(), torch.from_numpy(host[name][c])), (name, c)
+    # the oracle on the whole set: drift, then cell / counts / scan / stable permutation
+    aos = oracle.pack_r1(host)
+    L = oracle.lib()
+    L.soax_oracle_r1_drift(aos.ctypes.data, n, DT, 1)
+    exp = {k: np.empty(m, np.uint32) for k, m in (("cell", n), ("counts", G ** 3), ("offsets", G ** 3), ("perm", n))}
+    assert L.soax_oracle_r1_bin(aos.ctypes.data, n, G, exp["cell"].ctypes.data, exp["counts"].ctypes.data, exp["offsets"].ctypes.data,
+                                exp["perm"].ctypes.data, None) == 0
+    as_i32 = lambda a: torch.from_numpy(a.view(np.int32)).cuda()     # noqa: E731
+    assert torch.equal(r["counts"], as_i32(exp["counts"]))
+    assert torch.equal(r["offsets"], as_i32(exp["offsets"]))
+    perm = as_i32(exp["perm"])
+    assert torch.equal(r["perm"], perm)                              # the unique stable permutation, all 2^27 entries
+    assert int(exp["counts"].sum()) == n
+    perm = perm.to(torch.int64)
+    drifted = oracle.unpack(aos)
+    del aos, exp
+    for name, dt, dim in Cn.R1:                                      # dst.f[j] == drifted.f[perm[j]] bitwise, every array
+        for c in range(dim):
+            want = torch.from_numpy(drifted[name][c]).cuda()[perm]
+            assert torch.equal(dst.comp_view(name, c), want), (name, c)
+            del want
     ids = torch.sort(dst.comp_view("id"))[0]
     assert torch.equal(ids, torch.arange(n, dtype=torch.int32, device="cuda"))     # ids stay a permutation
     ke = float(r["kinetic"].item())
-    ref = 0.5 * sum(float((src.comp_view("vel", c).double() ** 2).sum()) for c in range(3))
-    assert abs(ke - ref) <= 1e-10 * ref and abs(ke / n - 1.5) < 1e-3
+    oke = oracle.energy(host, oracle.KINETIC)                        # the drift does not change vel
+    assert abs(ke - oke) <= 1e-10 * oke and abs(ke / n - 1.5) < 1e-3

@@ -121,6 +121,37 @@ def test_symplectic_euler_general_k_and_center(gpu):
     assert abs(e - o) <= 1e-10 * abs(o)
 
 
+@pytest.mark.parametrize("n", [1, 3, 4099, 100003])
+def test_energy_wide_record_r2(gpu, n):
+    """a8 on the double-velocity record R2 (config 4's layout): both kinds, general k / centre, ragged tails."""
+    torch, B, Cn = gpu
+    host = inputs.make_r2(n, seed=11)
+    host["acc"][:] = np.random.default_rng(1).normal(size=host["acc"].shape)       # must not enter the sum
+    s = to_device(Cn, Cn.R2, host)
+    for kind, okind, k, ctr in ((B.SOAX_ENERGY_KINETIC, oracle.KINETIC, 1.0, 0.5),
+                                (B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, oracle.KINETIC_PLUS_HARMONIC, 1.0, 0.5),
+                                (B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, oracle.KINETIC_PLUS_HARMONIC, 2.5, 0.25)):
+        e = s.energy(kind, k=k, center=ctr)
+        o = oracle.energy(host, okind, k=k, center=ctr)
+        assert abs(e - o) <= 1e-10 * abs(o), (kind, k, ctr)
+        assert s.energy(kind, k=k, center=ctr) == e                                  # run-to-run deterministic
+    if n == 1:                                                                       # one particle: no summation, bit-equal terms
+        assert s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, k=2.5, center=0.25) == oracle.energy(host, oracle.KINETIC_PLUS_HARMONIC, 2.5, 0.25)
+
+
+def test_energy_hand_fixture_r2_on_gpu(gpu):
+    torch, B, Cn = gpu
+    vel = np.array([[1, 2, 2], [0, 0, 0], [3, 4, 0], [-1, -1, -1]], np.float64)       # tests/golden/energy_4particles.txt
+    pos = np.array([[.5, .5, .5], [0, .5, .5], [.25, .75, .5], [.5, .5, 0]], np.float64)
+    host = {"id": np.arange(4, dtype=np.int64)[None, :].copy(), "pos": np.ascontiguousarray(pos.T), "vel": np.ascontiguousarray(vel.T),
+            "acc": np.full((3, 4), 7.0), "mass": np.array([[3, 5, 9, 17]], np.float32), "charge": np.array([[-1, 1, -1, 1]], np.float32),
+            "flags": np.array([[1, 2, 3, 4]], np.uint8)}
+    s = to_device(Cn, Cn.R2, host)
+    assert s.energy(B.SOAX_ENERGY_KINETIC) == 18.5
+    assert s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC) == 18.8125
+    assert s.energy(B.SOAX_ENERGY_KINETIC_PLUS_HARMONIC, k=4.0) == 18.5 + 4.0 * 0.3125
+
+
 def test_energy_hand_fixture_on_gpu(gpu):
     torch, B, Cn = gpu
     vel = np.array([[1, 2, 2], [0, 0, 0], [3, 4, 0], [-1, -1, -1]], np.float32).T.copy()
@@ -263,15 +294,16 @@ def check_bin(host_after_drift, sorted_soa, out, G):
     assert int(out["counts"].sum()) == host_after_drift["id"].shape[1]
 
 
-@pytest.fixture(params=[(2, 0), (2, 9), (2, 4), (1, 0), (0, 0)], ids=["ring", "ring-9bit", "ring-4bit", "staged", "direct"])
+@pytest.fixture(params=[(0, 0, 1), (9, 1, 1), (6, 0, 1), (4, 8, 1), (9, 16, 0), (7, 2, 1)],
+                ids=["default-9bit-cluster4", "9bit-no-cluster", "6bit-3pass", "4bit-5pass-cluster8", "9bit-cluster16-nosync", "7bit-cluster2"])
 def bin_stage(request, gpu):
-    """every scatter variant and digit width of the counting sort (soax_tune bin_stage / bin_bits) must give the
-    same unique result"""
-    gpu[1].soax_tune("bin_stage", request.param[0])
-    gpu[1].soax_tune("bin_bits", request.param[1])
+    """every digit width (1..5 passes) and launch shape (cluster size, cluster barrier on/off) of the counting sort
+    (soax_tune bin_bits / bin_cluster / bin_csync) must give the same unique result"""
+    for key, v in zip(("bin_bits", "bin_cluster", "bin_csync"), request.param):
+        gpu[1].soax_tune(key, v)
     yield request.param
-    gpu[1].soax_tune("bin_stage", 2)
-    gpu[1].soax_tune("bin_bits", 0)
+    for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1)):
+        gpu[1].soax_tune(key, v)
 
 
 @pytest.mark.parametrize("n,G", [(100003, 64), (4096, 64), (4097, 8), (50000, 2), (31, 64), (1, 64), (70000, 1), (8191, 64)])
@@ -305,12 +337,67 @@ def test_bin_permute_fused_drift_and_kinetic_config5_shape(gpu):
     host = inputs.make_r1(n, seed=7)
     src_after, sorted_soa, out = run_bin(gpu, host, G, drift_dt=DT, kinetic=True)
     drifted = oracle.drift(host, DT, 1)
-    check_r1(src_after, drifted)                                      # the fused drift updated src in place
-    check_bin(drifted, sorted_soa, out, G)
+    for name in host:                                                 # src is read only: the drift is applied on the way to dst
+        assert np.array_equal(bits(src_after[name]), bits(host[name])), name
+    check_bin(drifted, sorted_soa, out, G)                            # dst = the DRIFTED particles in cell order, bit for bit
     ke = float(out["kinetic"].item())
     oke = oracle.energy(drifted, oracle.KINETIC)
     assert abs(ke - oke) <= 1e-10 * oke
     assert np.array_equal(np.sort(sorted_soa["id"][0]), np.arange(n, dtype=np.int32))   # ids stay a permutation
+
+
+def test_bin_permute_wide_record_r2_with_drift(gpu):
+    """binning of the 13-array record R2 (double vel): the drift fused into the first pass uses the double-velocity fma;
+    every one of the 13 arrays is permuted.  Oracle: r2 drift, then the R1 binning oracle on the drifted positions."""
+    torch, B, Cn = gpu
+    n, G = 30011, 16
+    host = inputs.make_r2(n, seed=3)
+    host["acc"][:] = np.random.default_rng(2).normal(size=host["acc"].shape)
+    src, dst = to_device(Cn, Cn.R2, host), Cn.Soax(Cn.R2, n)
+    r = src.bin_permute(dst, G, drift_dt=DT, want_kinetic=True)
+    torch.cuda.synchronize()
+    drifted = oracle.drift(host, DT, 1)
+    as_r1 = {"id": np.zeros((1, n), np.int32), "pos": drifted["pos"], "vel": np.zeros((3, n), np.float32)}
+    exp = oracle.bin_r1(as_r1, G)
+    for k in ("counts", "offsets", "perm"):
+        assert np.array_equal(r[k].cpu().numpy().view(np.uint32), exp[k]), k
+    got = dst.download()
+    for name in host:
+        assert np.array_equal(bits(got[name]), bits(drifted[name][:, exp["perm"]])), name
+    assert np.array_equal(bits(src.download()["pos"]), bits(host["pos"]))             # src untouched
+    oke = oracle.energy(host, oracle.KINETIC)
+    assert abs(float(r["kinetic"].item()) - oke) <= 1e-10 * oke
+
+
+@pytest.mark.parametrize("want", ["none", "perm_only", "counts_only", "offsets_kinetic"])
+def test_bin_permute_optional_outputs(gpu, want):
+    """dev_counts / dev_offsets / dev_perm / dev_kinetic may each be NULL: the arrays are still permuted, and the outputs
+    that are asked for are the same as when all are asked for (the carried index / the sorted keys are skipped otherwise)."""
+    torch, B, Cn = gpu
+    n, G = 50021, 64
+    host = inputs.make_r1(n, seed=5)
+    src, dst = to_device(Cn, Cn.R1, host), Cn.Soax(Cn.R1, n)
+    exp = oracle.bin_r1(host, G)
+    want_sorted = oracle.permute_r1(host, exp["perm"])
+    i32 = lambda m: torch.full((m,), -1, dtype=torch.int32, device="cuda")           # noqa: E731
+    counts, offsets, perm, kin = i32(G ** 3), i32(G ** 3), i32(n), torch.zeros(1, dtype=torch.float64, device="cuda")
+    scratch = torch.empty(B.soax_scratch_bytes(src.layout, n, G), dtype=torch.uint8, device="cuda")
+    use = {"none": (), "perm_only": ("perm",), "counts_only": ("counts",), "offsets_kinetic": ("offsets", "kinetic")}[want]
+    B.soax_bin_permute(src.handle, dst.handle, G, 0.0, counts.data_ptr() if "counts" in use else None,
+                       offsets.data_ptr() if "offsets" in use else None, perm.data_ptr() if "perm" in use else None,
+                       kin.data_ptr() if "kinetic" in use else None, scratch.data_ptr(), scratch.numel(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    got = dst.download()
+    for name in want_sorted:
+        assert np.array_equal(bits(got[name]), bits(want_sorted[name])), name
+    for name, t in (("counts", counts), ("offsets", offsets), ("perm", perm)):
+        if name in use:
+            assert np.array_equal(t.cpu().numpy().view(np.uint32), exp[name]), name
+        else:
+            assert bool((t == -1).all()), name                                       # not asked for: not written
+    if "kinetic" in use:
+        oke = oracle.energy(host, oracle.KINETIC)
+        assert abs(float(kin.item()) - oke) <= 1e-10 * oke
 
 
 def test_bin_empty(gpu):

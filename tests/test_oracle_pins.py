@@ -321,6 +321,66 @@ def test_energy_compensated_sum_large_n_vs_fsum():
     assert abs(got / n - 1.5) < 0.01
 
 
+
+def _r2(pos, vel, acc=None, mass=None, charge=None, flags=None, ids=None):
+    pos = np.asarray(pos, np.float64).reshape(-1, 3)
+    vel = np.asarray(vel, np.float64).reshape(-1, 3)
+    n = pos.shape[0]
+    acc = np.zeros((n, 3)) if acc is None else np.asarray(acc, np.float64).reshape(-1, 3)
+    return {"id": (np.arange(n, dtype=np.int64) if ids is None else np.asarray(ids, np.int64))[None, :].copy(),
+            "pos": np.ascontiguousarray(pos.T), "vel": np.ascontiguousarray(vel.T), "acc": np.ascontiguousarray(acc.T),
+            "mass": (np.ones(n, np.float32) if mass is None else np.asarray(mass, np.float32))[None, :].copy(),
+            "charge": (np.ones(n, np.float32) if charge is None else np.asarray(charge, np.float32))[None, :].copy(),
+            "flags": (np.zeros(n, np.uint8) if flags is None else np.asarray(flags, np.uint8))[None, :].copy()}
+
+
+def test_energy_r2_hand_fixture(golden_dir):
+    """The same 4-particle dyadic fixture stored as the wide record R2 (double vel): 18.5 / 18.8125 with '=='.
+    acc, mass, charge, flags and id are filled with values that would change the sum if any were read instead of
+    vel / pos (a wrong member in soax_oracle_r2_energy fails here)."""
+    s1, exp = _load_energy_fixture(golden_dir)
+    s = _r2(s1["pos"].T, s1["vel"].T.astype(np.float64), acc=[[7, 7, 7]] * 4, mass=[3, 5, 9, 17], charge=[-1, 1, -1, 1],
+            flags=[1, 2, 3, 4], ids=[100, 200, 300, 400])
+    assert oracle.energy(s, oracle.KINETIC) == exp["expect_kinetic"] == 18.5
+    assert oracle.energy(s, oracle.KINETIC_PLUS_HARMONIC) == exp["expect_total"] == 18.8125
+    for order in ([3, 2, 1, 0], [2, 0, 3, 1]):
+        assert oracle.energy(inputs.take(s, np.array(order)), oracle.KINETIC_PLUS_HARMONIC) == 18.8125
+    assert oracle.energy(s, oracle.KINETIC_PLUS_HARMONIC, k=4.0) == 18.5 + 4.0 * 0.3125
+    assert oracle.energy(s, oracle.KINETIC_PLUS_HARMONIC, k=1.0, center=0.0) == 18.5 + 0.5 * (0.75 + 0.5 + 0.875 + 0.5)
+    # component order matters in the fma chain only through rounding; a dropped component changes the value:
+    t = _r2([[0.5, 0.5, 0.5]], [[1.0, 2.0, 4.0]])
+    assert oracle.energy(t, oracle.KINETIC) == 10.5
+    assert oracle.energy(_r2([[0.25, 0.5, 1.0]], [[0, 0, 0]]), oracle.KINETIC_PLUS_HARMONIC) == 0.5 * (0.0625 + 0.25)
+
+
+def test_energy_r2_terms_and_compensated_sum():
+    """Per-particle term of the double-velocity record restated with exact rationals and one rounding per IEEE
+    operation (bit for bit), general k and centre; the Neumaier sum within one ulp of the exact sum."""
+    n = 2000
+    s = inputs.make_r2(n, seed=21)
+    s["acc"][:] = np.random.default_rng(3).normal(size=(3, n))         # must not enter the sum
+    for kind, k, ctr in ((oracle.KINETIC, 1.0, 0.5), (oracle.KINETIC_PLUS_HARMONIC, 1.0, 0.5), (oracle.KINETIC_PLUS_HARMONIC, 2.5, 0.25)):
+        terms = []
+        for i in range(n):
+            v = [F(s["vel"][c, i]) for c in range(3)]
+            q = rn64(v[0] * v[0])
+            q = rn64(v[1] * v[1] + q)
+            q = rn64(v[2] * v[2] + q)
+            if kind == oracle.KINETIC_PLUS_HARMONIC:
+                for c in range(3):
+                    d = rn64(F(s["pos"][c, i]) - F(ctr))
+                    q = rn64(rn64(F(k) * d) * d + q)
+            terms.append(q / 2)
+        for i in range(0, n, 89):
+            assert oracle.energy(inputs.take(s, np.array([i])), kind, k, ctr) == float(terms[i])
+        exact = sum(terms, Fraction(0))
+        got = oracle.energy(s, kind, k, ctr)
+        assert abs(F(got) - exact) <= Fraction(math.ulp(got))
+    # double velocities are NOT rounded through float: a value with more than 24 significant bits keeps them
+    t = _r2([[0.5, 0.5, 0.5]], [[1.0 + 2.0 ** -40, 0.0, 0.0]])
+    assert oracle.energy(t, oracle.KINETIC) == float(rn64(F(1.0 + 2.0 ** -40) ** 2) / 2) != 0.5
+
+
 # ------------------------------------------------------------------------------ AoS <-> SoA (a6, a7; Q1)
 def test_r1_packed_layout_offsets():
     off = np.zeros(7, np.int64)
