@@ -41,7 +41,7 @@ def test_library_is_sm100a_and_uses_wide_and_bulk_accesses():
     assert "sm_100a" in text
     assert "LDG.E.NA.ENL2.256" in text or "LDG.E.ENL2.256" in text or ".256" in text
     assert "UBLKCP" in text
-    assert "DFMA" in text and "MATCH.ANY" in text
+    assert "DFMA" in text and "UCGABAR_ARV" in text and "VOTE" in text   # explicit fma; cluster barrier + ballots of the scatter
 
 
 def test_layout_registry_and_aos_image():
