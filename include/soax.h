@@ -208,12 +208,17 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
  *                          row moves.
  *   SOAX_REMOVE_STABLE     order-preserving compaction into dst (same layout, no aliasing, capacity >= survivors;
  *                          s is left untouched).
- * The result is unique and deterministic for any mask.  The survivor count is written to *host_new_n (HOST) and
- * becomes the live count of s (SWAP_LAST) or dst (STABLE).  Because the handle must know that count, this call
- * SYNCHRONISES `stream` once, after all its kernels have been enqueued (they read the count on the device).
- * dev_scratch: >= soax_remove_scratch_bytes(n) bytes, 256-byte aligned.
- * Errors: INVALID_ARG, ALLOC (scratch too small; STABLE: dst capacity < survivors -- dst then holds the
- * survivors that fit and its live count is unchanged), UNSUPPORTED (n >= 2^32), CUDA. */
+ * The result is unique and deterministic for any mask.  The call is ASYNCHRONOUS like every other: the kernels read the
+ * survivor count on the device, and the host learns it without a synchronisation in this call -- the stream copies it
+ * into a pinned word owned by the target handle (s for SWAP_LAST, dst for STABLE) and records an event; the first later
+ * call that needs that handle's live count on the host (soax_size, or any call that launches over its particles) waits for
+ * that one event, which completes after the two small counting kernels, not after the rows have moved.  host_new_n:
+ * optional HOST pointer (NULL allowed) that also receives the survivor count by an asynchronous copy on `stream`; it must be
+ * pinned memory for the copy to be asynchronous, and may be read after the caller has synchronised the stream.
+ * dev_scratch: >= soax_remove_scratch_bytes(n) bytes, 256-byte aligned; it must stay valid until the enqueued work is done.
+ * STABLE into a destination whose capacity is below the survivor count: dst receives the survivors that fit and its live
+ * count becomes its capacity; *host_new_n still reports the true count (a capacity >= n can never overflow).
+ * Errors: INVALID_ARG, ALLOC (scratch too small), UNSUPPORTED (n >= 2^32), CUDA. */
 typedef enum { SOAX_REMOVE_SWAP_LAST = 0, SOAX_REMOVE_STABLE = 1 } soax_remove_mode;
 size_t soax_remove_scratch_bytes(int64_t n);
 int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, void* dev_scratch, size_t scratch_bytes,
@@ -224,7 +229,7 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
  * soax_copy into it -- the paper's resize). */
 int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream);
 /* Bulk getElement (PAPER.md:304 `soax.getElement(i)`): rows dev_idx[0..m) (uint32, each < n, repeats allowed) as m
- * packed AoS records in dev_aos (16-byte aligned).  Indices are not range-checked. */
+ * packed AoS records in dev_aos (16-byte aligned).  An index >= n is not dereferenced: its record is all zero bytes. */
 int soax_get_elements(const soax_t* s, const uint32_t* dev_idx, int64_t m, void* dev_aos, void* stream);
 /* Copy the live particles of src into dst (same layout, capacity >= n); dst's live count becomes src's. */
 int soax_copy(soax_t* dst, const soax_t* src, void* stream);

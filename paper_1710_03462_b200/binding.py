@@ -243,11 +243,13 @@ def soax_remove_scratch_bytes(n: int) -> int:
     return lib().soax_remove_scratch_bytes(n)
 
 
-def soax_remove(s: int, dst: int | None, dev_kill: int, mode: int, dev_scratch: int, scratch_bytes: int, stream: int = 0) -> int:
-    """Returns the survivor count (the call synchronises the stream once)."""
-    new_n = _i64()
-    _check(lib().soax_remove(s, dst, dev_kill, mode, dev_scratch, scratch_bytes, C.byref(new_n), stream), "soax_remove")
-    return new_n.value
+def soax_remove(s: int, dst: int | None, dev_kill: int, mode: int, dev_scratch: int, scratch_bytes: int, stream: int = 0,
+                host_new_n: int | None = None) -> None:
+    """Asynchronous: everything is enqueued and the call returns.  The live count of the target handle (s for SWAP_LAST,
+    dst for STABLE) is learnt lazily by the first later call that needs it (soax_size waits for the one event that marks
+    the count ready).  host_new_n: optional address of a PINNED int64 that also receives the survivor count."""
+    ptr = C.cast(host_new_n, C.POINTER(_i64)) if host_new_n else None
+    _check(lib().soax_remove(s, dst, dev_kill, mode, dev_scratch, scratch_bytes, ptr, stream), "soax_remove")
 
 
 def soax_push_back_aos(s: int, dev_aos: int, m: int, stream: int = 0) -> None:

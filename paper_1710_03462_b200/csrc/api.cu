@@ -33,27 +33,95 @@ struct soax_layout {
     int (*energy)(void* const*, int64_t, int, double, double, void*, double*, cudaStream_t);
     int (*bin_permute)(const BinArgs&, cudaStream_t);
     size_t (*bin_scratch)(int64_t, int);
-    int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, int64_t*, int64_t, cudaStream_t);
-    int (*gather_rows)(void* const*, const uint32_t*, int64_t, void*, cudaStream_t);
+    int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t);
+    int (*gather_rows)(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
 };
 
-// A captured `nsteps`-launch step loop, kept with the container and replayed while the call is the same: small
+// A captured loop of `nlaunch` kernel launches, replayed while the call that made it is repeated unchanged: small
 // (L2-resident) particle sets are launch-bound, and a graph replays its kernel nodes back to back without a host
-// round trip per step.  Still one kernel launch and one full memory pass per step (Q14).
-struct StepGraph {
+// round trip per step.  Still one kernel launch and one full memory pass per step (Q14).  The key is the byte image of
+// EVERYTHING the captured launches depend on (every component pointer, counts, parameters, tuning): a freed container
+// whose address or slab is reused by a new one can therefore never replay the old graph.
+struct GraphCache {
     cudaGraphExec_t exec = nullptr;
-    soax_step_params params{};
-    int32_t nsteps = 0;
-    int64_t n = 0;
-    Tuning tune{};
+    std::string key;
+    ~GraphCache() {}  // the exec is destroyed explicitly (soax_free / soax_expr_free); at thread exit the context may be gone
 };
+
+// True if `st` can be captured now: any stream but the legacy default stream that is not already being captured.
+static bool capturable(cudaStream_t st) {
+    if (st == nullptr || st == cudaStreamLegacy) return false;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
+    return true;
+}
+
+// Replay the graph cached under `key`, capturing it first with nlaunch calls of enqueue(st) if the key changed.  Returns
+// SOAX_OK with *done = true if the graph ran; *done = false if capture is not possible (the caller then issues the
+// launches one by one).  `prepare` runs once before a capture (work that must not be captured, e.g. module loading).
+template <class Prepare, class Enqueue>
+static int replay_or_capture(GraphCache& g, const std::string& key, int32_t nlaunch, cudaStream_t st, Prepare&& prepare, Enqueue&& enqueue,
+                             bool* done) {
+    *done = false;
+    if (!g.exec || g.key != key) {
+        if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+        SOAX_TRY(prepare());
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            int rc = SOAX_OK;
+            for (int32_t i = 0; i < nlaunch && rc == SOAX_OK; ++i) rc = enqueue();
+            const cudaError_t e = cudaStreamEndCapture(st, &graph);
+            if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+            if (e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) g.exec = nullptr;
+            if (graph) cudaGraphDestroy(graph);
+        }
+        cudaGetLastError();
+        if (g.exec) g.key = key;
+    } else {
+        g_launches.fetch_add(nlaunch, std::memory_order_relaxed);  // the replay launches the same nlaunch kernels
+    }
+    if (!g.exec) return SOAX_OK;
+    SOAX_CUDA(cudaGraphLaunch(g.exec, st));
+    *done = true;
+    return SOAX_OK;
+}
+
+template <class T> static void key_add(std::string& k, const T& v) { k.append(reinterpret_cast<const char*>(&v), sizeof(T)); }
 
 struct soax_container {
     const soax_layout* layout;
     int64_t n, capacity;
     void* comp[kMaxComp];
-    StepGraph graph;
+    uint64_t serial;  // unique per soax_alloc: part of every graph key
+    GraphCache graph;
+    // A live count that a kernel is still computing (soax_remove): the stream copies it into `pin_n` (pinned host
+    // memory owned by the handle) and records `n_event`; the first later call that needs the count on the host waits for
+    // that one event -- the count is ready after two small kernels, long before the rows have moved.
+    mutable bool n_pending = false;
+    int64_t* pin_n = nullptr;
+    cudaEvent_t n_event = nullptr;
 };
+
+// live particle count of a handle, resolving a pending one
+static int64_t live(const soax_container* s) {
+    if (s->n_pending) {
+        cudaEventSynchronize(s->n_event);
+        int64_t m = *s->pin_n;
+        if (m > s->capacity) m = s->capacity;  // STABLE into too small a destination: it holds the survivors that fit
+        const_cast<soax_container*>(s)->n = m;
+        s->n_pending = false;
+    }
+    return s->n;
+}
+static void set_live(soax_container* s, int64_t n) { s->n = n; s->n_pending = false; }
+
+static std::string container_key(const soax_container* s) {
+    std::string k;
+    key_add(k, s->serial); key_add(k, s->layout); key_add(k, live(s)); key_add(k, s->capacity);
+    k.append(reinterpret_cast<const char*>(s->comp), sizeof(void*) * s->layout->ncomp);
+    key_add(k, g_tune);
+    return k;
+}
 
 namespace {
 
@@ -228,8 +296,10 @@ int soax_alloc(const soax_layout* l, int64_t n, int64_t capacity, void* dev_slab
     soax_container* s = new (std::nothrow) soax_container();
     if (!s) return SOAX_ERR_ALLOC;
     s->layout = l;
-    s->n = n;
+    set_live(s, n);
     s->capacity = capacity;
+    static std::atomic<uint64_t> next_serial{1};
+    s->serial = next_serial.fetch_add(1, std::memory_order_relaxed);
     carve(l, capacity, dev_slab, s->comp);
     *out = s;
     return SOAX_OK;
@@ -238,15 +308,17 @@ int soax_alloc(const soax_layout* l, int64_t n, int64_t capacity, void* dev_slab
 int soax_free(soax_t* s) {
     if (!s) return SOAX_ERR_INVALID_ARG;
     if (s->graph.exec) cudaGraphExecDestroy(s->graph.exec);
+    if (s->n_event) { cudaEventSynchronize(s->n_event); cudaEventDestroy(s->n_event); }  // a pending count copy targets pin_n
+    if (s->pin_n) cudaFreeHost(s->pin_n);
     delete s;
     return SOAX_OK;
 }
 
-int64_t soax_size(const soax_t* s) { return s ? s->n : (int64_t)SOAX_ERR_INVALID_ARG; }
+int64_t soax_size(const soax_t* s) { return s ? live(s) : (int64_t)SOAX_ERR_INVALID_ARG; }
 
 int soax_resize(soax_t* s, int64_t n) {
     if (!s || n < 0 || n > s->capacity) return SOAX_ERR_INVALID_ARG;
-    s->n = n;
+    set_live(s, n);
     return SOAX_OK;
 }
 
@@ -263,12 +335,12 @@ int soax_upload(soax_t* s, const void* const* host_comps, int64_t n, void* strea
         if (host_comps[c] && n > 0)
             SOAX_CUDA(cudaMemcpyAsync(s->comp[c], host_comps[c], (size_t)n * s->layout->csize[c], cudaMemcpyHostToDevice,
                                       (cudaStream_t)stream));
-    s->n = n;
+    set_live(s, n);
     return SOAX_OK;
 }
 
 int soax_download(const soax_t* s, void* const* host_comps, int64_t n, void* stream) {
-    if (!s || !host_comps || n < 0 || n > s->n) return SOAX_ERR_INVALID_ARG;
+    if (!s || !host_comps || n < 0 || n > live(s)) return SOAX_ERR_INVALID_ARG;
     for (int c = 0; c < s->layout->ncomp; ++c)
         if (host_comps[c] && n > 0)
             SOAX_CUDA(cudaMemcpyAsync(host_comps[c], s->comp[c], (size_t)n * s->layout->csize[c], cudaMemcpyDeviceToHost,
@@ -280,35 +352,15 @@ int soax_step(soax_t* s, const soax_step_params* p, int32_t nsteps, void* stream
     if (!s || !p || nsteps < 0) return SOAX_ERR_INVALID_ARG;
     if (!s->layout->step) return SOAX_ERR_UNSUPPORTED;  // run-time layout: no compiled kernel families
     cudaStream_t st = (cudaStream_t)stream;
-    // Graph replay needs a capturable stream (not the legacy default stream) that is not already being captured.
-    bool use_graph = g_tune.step_graph && nsteps >= 2 && s->n > 0 && st != nullptr && st != cudaStreamLegacy;
-    if (use_graph) {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+    auto one = [&] { return s->layout->step(s->comp, live(s), p, st); };
+    if (g_tune.step_graph && nsteps >= 2 && live(s) > 0 && capturable(st)) {
+        std::string key = container_key(s);
+        key_add(key, *p); key_add(key, nsteps);
+        bool done = false;
+        SOAX_TRY(replay_or_capture(s->graph, key, nsteps, st, [] { return SOAX_OK; }, one, &done));
+        if (done) return SOAX_OK;
     }
-    if (use_graph) {
-        StepGraph& g = s->graph;
-        const bool same = g.exec && g.nsteps == nsteps && g.n == s->n && std::memcmp(&g.params, p, sizeof(*p)) == 0 &&
-                          std::memcmp(&g.tune, &g_tune, sizeof(Tuning)) == 0;
-        if (!same) {
-            if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
-            cudaGraph_t graph = nullptr;
-            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-                int rc = SOAX_OK;
-                for (int32_t i = 0; i < nsteps && rc == SOAX_OK; ++i) rc = s->layout->step(s->comp, s->n, p, st);
-                const cudaError_t e = cudaStreamEndCapture(st, &graph);
-                if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
-                if (e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) g.exec = nullptr;
-                if (graph) cudaGraphDestroy(graph);
-            }
-            cudaGetLastError();
-            if (g.exec) { std::memcpy(&g.params, p, sizeof(*p)); g.nsteps = nsteps; g.n = s->n; g.tune = g_tune; }
-        } else {
-            g_launches.fetch_add(nsteps, std::memory_order_relaxed);  // the replay launches the same nsteps kernels
-        }
-        if (g.exec) { SOAX_CUDA(cudaGraphLaunch(g.exec, st)); return SOAX_OK; }
-    }
-    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(s->layout->step(s->comp, s->n, p, st));
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(one());
     return SOAX_OK;
 }
 
@@ -317,53 +369,30 @@ int soax_step_aos(const soax_layout* l, void* dev_aos, int64_t n, const soax_ste
     if (!l || !p || nsteps < 0 || n < 0 || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
     if (!l->step_aos) return SOAX_ERR_UNSUPPORTED;
     cudaStream_t st = (cudaStream_t)stream;
+    auto one = [&] { return l->step_aos(dev_aos, n, p, variant, st); };
     // Same graph replay as soax_step, so that the AoS baseline is timed under the same launch mechanism as the SoA
     // path.  There is no container to keep the graph with: one entry per host thread, keyed by the whole call.
-    struct AosGraph : StepGraph { const soax_layout* layout = nullptr; void* aos = nullptr; int32_t variant = 0;
-                                  ~AosGraph() { /* the context may be gone at thread exit: leak the exec */ } };
-    static thread_local AosGraph g;
-    bool use_graph = g_tune.step_graph && nsteps >= 2 && n > 0 && st != nullptr && st != cudaStreamLegacy;
-    if (use_graph) {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+    static thread_local GraphCache g;
+    if (g_tune.step_graph && nsteps >= 2 && n > 0 && capturable(st)) {
+        std::string key;
+        key_add(key, l); key_add(key, dev_aos); key_add(key, n); key_add(key, *p); key_add(key, nsteps); key_add(key, variant); key_add(key, g_tune);
+        bool done = false;
+        SOAX_TRY(replay_or_capture(g, key, nsteps, st, [] { return SOAX_OK; }, one, &done));
+        if (done) return SOAX_OK;
     }
-    if (use_graph) {
-        const bool same = g.exec && g.layout == l && g.aos == dev_aos && g.variant == variant && g.nsteps == nsteps && g.n == n &&
-                          std::memcmp(&g.params, p, sizeof(*p)) == 0 && std::memcmp(&g.tune, &g_tune, sizeof(Tuning)) == 0;
-        if (!same) {
-            if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
-            cudaGraph_t graph = nullptr;
-            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-                int rc = SOAX_OK;
-                for (int32_t i = 0; i < nsteps && rc == SOAX_OK; ++i) rc = l->step_aos(dev_aos, n, p, variant, st);
-                const cudaError_t e = cudaStreamEndCapture(st, &graph);
-                if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
-                if (e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) g.exec = nullptr;
-                if (graph) cudaGraphDestroy(graph);
-            }
-            cudaGetLastError();
-            if (g.exec) {
-                std::memcpy(&g.params, p, sizeof(*p));
-                g.nsteps = nsteps; g.n = n; g.tune = g_tune; g.layout = l; g.aos = dev_aos; g.variant = variant;
-            }
-        } else {
-            g_launches.fetch_add(nsteps, std::memory_order_relaxed);
-        }
-        if (g.exec) { SOAX_CUDA(cudaGraphLaunch(g.exec, st)); return SOAX_OK; }
-    }
-    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(l->step_aos(dev_aos, n, p, variant, st));
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(one());
     return SOAX_OK;
 }
 
 int soax_aos_to_soa(soax_t* dst, const void* dev_aos, int64_t n, void* stream) {
     if (!dst || n < 0 || n > dst->capacity || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
     if (!dst->layout->aos_to_soa) return SOAX_ERR_UNSUPPORTED;
-    dst->n = n;
+    set_live(dst, n);
     return n == 0 ? SOAX_OK : dst->layout->aos_to_soa(dst->comp, dev_aos, n, (cudaStream_t)stream);
 }
 
 int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream) {
-    if (!src || n < 0 || n > src->n || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
+    if (!src || n < 0 || n > live(src) || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
     if (!src->layout->soa_to_aos) return SOAX_ERR_UNSUPPORTED;
     return n == 0 ? SOAX_OK : src->layout->soa_to_aos(const_cast<void* const*>(src->comp), dev_aos, n, (cudaStream_t)stream);
 }
@@ -375,7 +404,7 @@ int soax_reduce_energy(const soax_t* s, int32_t kind, double k, double center, v
     if (!s || !dev_scratch || !dev_out || !aligned(dev_scratch, 8) || !aligned(dev_out, 8)) return SOAX_ERR_INVALID_ARG;
     if (scratch_bytes < kEnergyScratchBytes) return SOAX_ERR_ALLOC;
     if (!s->layout->energy) return SOAX_ERR_UNSUPPORTED;
-    return s->layout->energy(const_cast<void* const*>(s->comp), s->n, kind, k, center, dev_scratch, dev_out,
+    return s->layout->energy(const_cast<void* const*>(s->comp), live(s), kind, k, center, dev_scratch, dev_out,
                              (cudaStream_t)stream);
 }
 
@@ -390,17 +419,17 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
     if (!src || !dst || src == dst || src->layout != dst->layout || !dev_scratch || !aligned(dev_scratch, kAlign))
         return SOAX_ERR_INVALID_ARG;
     const int log2g = ilog2_exact(grid_dim);
-    if (log2g < 0 || dst->capacity < src->n) return SOAX_ERR_INVALID_ARG;
+    if (log2g < 0 || dst->capacity < live(src)) return SOAX_ERR_INVALID_ARG;
     if (!src->layout->bin_permute) return SOAX_ERR_UNSUPPORTED;
     for (int c = 0; c < src->layout->ncomp; ++c)
         if (src->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
-    if (src->n >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
-    const size_t need = src->layout->bin_scratch(src->n, log2g);
+    if (live(src) >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
+    const size_t need = src->layout->bin_scratch(live(src), log2g);
     if (need == 0) return SOAX_ERR_UNSUPPORTED;
     if (scratch_bytes < need) return SOAX_ERR_ALLOC;
-    BinArgs a{src->comp, dst->comp, src->n, log2g, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
+    BinArgs a{src->comp, dst->comp, live(src), log2g, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
               dev_scratch, scratch_bytes};
-    dst->n = src->n;
+    set_live(dst, live(src));
     return src->layout->bin_permute(a, (cudaStream_t)stream);
 }
 
@@ -409,9 +438,11 @@ size_t soax_remove_scratch_bytes(int64_t n) { return n < 0 ? 0 : remove_scratch_
 
 int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, void* dev_scratch, size_t scratch_bytes,
                 int64_t* host_new_n, void* stream) {
-    if (!s || !host_new_n || (s->n > 0 && (!dev_kill || !dev_scratch)) || !aligned(dev_scratch, kAlign)) return SOAX_ERR_INVALID_ARG;
+    if (!s) return SOAX_ERR_INVALID_ARG;
+    const int64_t n = live(s);
+    if ((n > 0 && (!dev_kill || !dev_scratch)) || !aligned(dev_scratch, kAlign)) return SOAX_ERR_INVALID_ARG;
     if (mode != SOAX_REMOVE_SWAP_LAST && mode != SOAX_REMOVE_STABLE) return SOAX_ERR_INVALID_ARG;
-    if (s->n >= ((int64_t)1 << 32) || !s->layout->remove) return SOAX_ERR_UNSUPPORTED;
+    if (n >= ((int64_t)1 << 32) || !s->layout->remove) return SOAX_ERR_UNSUPPORTED;
     if (mode == SOAX_REMOVE_SWAP_LAST) {
         if (dst) return SOAX_ERR_INVALID_ARG;  // in place
     } else {
@@ -419,42 +450,52 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
         for (int c = 0; c < s->layout->ncomp; ++c)
             if (s->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
     }
-    if (s->n > 0 && scratch_bytes < remove_scratch_bytes(s->n)) return SOAX_ERR_ALLOC;
-    int64_t m = 0;
-    const int rc = s->layout->remove(s->comp, dst ? dst->comp : nullptr, dev_kill, s->n, mode, dev_scratch, &m,
-                                     dst ? dst->capacity : 0, (cudaStream_t)stream);
-    *host_new_n = m;
-    if (rc != SOAX_OK) return rc;
-    if (mode == SOAX_REMOVE_SWAP_LAST) s->n = m; else dst->n = m;
+    if (n > 0 && scratch_bytes < remove_scratch_bytes(n)) return SOAX_ERR_ALLOC;
+    soax_container* target = mode == SOAX_REMOVE_SWAP_LAST ? s : dst;
+    if (n == 0) {
+        if (host_new_n) *host_new_n = 0;
+        set_live(target, 0);
+        return SOAX_OK;
+    }
+    if (!target->pin_n) {
+        SOAX_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&target->pin_n), sizeof(int64_t), cudaHostAllocMapped | cudaHostAllocPortable));
+        SOAX_CUDA(cudaEventCreateWithFlags(&target->n_event, cudaEventDisableTiming));
+    } else if (target->n_pending) {
+        live(target);  // an earlier pending count still targets pin_n: let it land before the word is reused
+    }
+    const int64_t* dev_m = nullptr;
+    SOAX_TRY(s->layout->remove(s->comp, dst ? dst->comp : nullptr, dev_kill, n, mode, dev_scratch, &dev_m, dst ? dst->capacity : 0,
+                               target->pin_n, host_new_n, target->n_event, (cudaStream_t)stream));
+    target->n_pending = true;
     return SOAX_OK;
 }
 
 int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream) {
     if (!s || m < 0 || (m > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
     if (!s->layout->aos_to_soa) return SOAX_ERR_UNSUPPORTED;
-    if (s->n + m > s->capacity) return SOAX_ERR_ALLOC;  // the caller owns the memory: regrow = soax_alloc a larger slab + soax_copy
+    if (live(s) + m > s->capacity) return SOAX_ERR_ALLOC;  // the caller owns the memory: regrow = soax_alloc a larger slab + soax_copy
     if (m == 0) return SOAX_OK;
     void* tail[kMaxComp];
-    for (int c = 0; c < s->layout->ncomp; ++c) tail[c] = static_cast<char*>(s->comp[c]) + (size_t)s->n * s->layout->csize[c];
+    for (int c = 0; c < s->layout->ncomp; ++c) tail[c] = static_cast<char*>(s->comp[c]) + (size_t)live(s) * s->layout->csize[c];
     SOAX_TRY(s->layout->aos_to_soa(tail, dev_aos, m, (cudaStream_t)stream));
-    s->n += m;
+    set_live(s, live(s) + m);
     return SOAX_OK;
 }
 
 int soax_get_elements(const soax_t* s, const uint32_t* dev_idx, int64_t m, void* dev_aos, void* stream) {
     if (!s || m < 0 || (m > 0 && (!dev_idx || !dev_aos)) || !aligned(dev_aos, 16) || !aligned(dev_idx, 4)) return SOAX_ERR_INVALID_ARG;
     if (!s->layout->gather_rows) return SOAX_ERR_UNSUPPORTED;
-    return s->layout->gather_rows(const_cast<void* const*>(s->comp), dev_idx, m, dev_aos, (cudaStream_t)stream);
+    return s->layout->gather_rows(const_cast<void* const*>(s->comp), live(s), dev_idx, m, dev_aos, (cudaStream_t)stream);
 }
 
 int soax_copy(soax_t* dst, const soax_t* src, void* stream) {
     if (!dst || !src || dst == src || dst->layout != src->layout) return SOAX_ERR_INVALID_ARG;
-    if (dst->capacity < src->n) return SOAX_ERR_ALLOC;
+    if (dst->capacity < live(src)) return SOAX_ERR_ALLOC;
     for (int c = 0; c < src->layout->ncomp; ++c)
-        if (src->n > 0)
-            SOAX_CUDA(cudaMemcpyAsync(dst->comp[c], src->comp[c], (size_t)src->n * src->layout->csize[c], cudaMemcpyDeviceToDevice,
+        if (live(src) > 0)
+            SOAX_CUDA(cudaMemcpyAsync(dst->comp[c], src->comp[c], (size_t)live(src) * src->layout->csize[c], cudaMemcpyDeviceToDevice,
                                       (cudaStream_t)stream));
-    dst->n = src->n;
+    set_live(dst, live(src));
     return SOAX_OK;
 }
 
@@ -462,13 +503,7 @@ int soax_copy(soax_t* dst, const soax_t* src, void* stream) {
 struct soax_expr {
     CompiledExpr* impl;
     const soax_layout* layout;
-    // captured nsteps-launch loop, replayed while the call is the same (as soax_step does; see StepGraph)
-    cudaGraphExec_t exec = nullptr;
-    const soax_container* g_s = nullptr;
-    void* g_comp0 = nullptr;
-    int64_t g_n = 0;
-    int32_t g_nsteps = 0, g_nscalars = 0, g_block = 0;
-    double g_scalars[16] = {};
+    GraphCache graph;  // captured nsteps-launch loop, replayed while the call is the same (as soax_step does)
 };
 
 static int expr_compile_any(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars, bool is_sum,
@@ -505,53 +540,32 @@ int soax_expr_sum(const soax_t* s, soax_expr* e, const double* scalars, int32_t 
         return SOAX_ERR_INVALID_ARG;
     if (s->layout != e->layout) return SOAX_ERR_INVALID_ARG;
     if (scratch_bytes < kEnergyScratchBytes) return SOAX_ERR_ALLOC;
-    return expr_sum(e->impl, s->layout, const_cast<void* const*>(s->comp), s->n, scalars, nscalars, static_cast<double*>(dev_scratch),
+    return expr_sum(e->impl, s->layout, const_cast<void* const*>(s->comp), live(s), scalars, nscalars, static_cast<double*>(dev_scratch),
                     dev_out, (cudaStream_t)stream);
 }
 
 int soax_expr_run(soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, int32_t nsteps, void* stream) {
-    if (!s || !e || nsteps < 0 || nscalars < 0 || nscalars > 16) return SOAX_ERR_INVALID_ARG;
+    if (!s || !e || nsteps < 0 || nscalars < 0 || nscalars > 16 || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
     if (s->layout != e->layout) return SOAX_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    bool use_graph = g_tune.step_graph && nsteps >= 2 && s->n > 0 && st != nullptr && st != cudaStreamLegacy;
-    if (use_graph) {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+    auto one = [&] { return expr_run(e->impl, s->layout, s->comp, live(s), scalars, nscalars, st); };
+    if (g_tune.step_graph && nsteps >= 2 && live(s) > 0 && capturable(st)) {
+        std::string key = container_key(s);  // every component pointer: a new container at a recycled address never matches
+        key_add(key, nsteps); key_add(key, nscalars);
+        if (nscalars) key.append(reinterpret_cast<const char*>(scalars), sizeof(double) * nscalars);
+        bool done = false;
+        // the first launch loads the generated code: do it (with n = 0) outside the capture
+        SOAX_TRY(replay_or_capture(e->graph, key, nsteps, st,
+                                   [&] { return expr_run(e->impl, s->layout, s->comp, 0, scalars, nscalars, st); }, one, &done));
+        if (done) return SOAX_OK;
     }
-    if (use_graph) {
-        const bool same = e->exec && e->g_s == s && e->g_comp0 == s->comp[0] && e->g_n == s->n && e->g_nsteps == nsteps &&
-                          e->g_nscalars == nscalars && e->g_block == g_tune.step_block &&
-                          (nscalars == 0 || std::memcmp(e->g_scalars, scalars, sizeof(double) * nscalars) == 0);
-        if (!same) {
-            if (e->exec) { cudaGraphExecDestroy(e->exec); e->exec = nullptr; }
-            // the first launch loads the generated code: do it outside the capture
-            SOAX_TRY(expr_run(e->impl, s->layout, s->comp, 0, scalars, nscalars, st));
-            cudaGraph_t graph = nullptr;
-            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-                int rc = SOAX_OK;
-                for (int32_t i = 0; i < nsteps && rc == SOAX_OK; ++i) rc = expr_run(e->impl, s->layout, s->comp, s->n, scalars, nscalars, st);
-                const cudaError_t err = cudaStreamEndCapture(st, &graph);
-                if (rc != SOAX_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
-                if (err == cudaSuccess && graph && cudaGraphInstantiate(&e->exec, graph, 0) != cudaSuccess) e->exec = nullptr;
-                if (graph) cudaGraphDestroy(graph);
-            }
-            cudaGetLastError();
-            if (e->exec) {
-                e->g_s = s; e->g_comp0 = s->comp[0]; e->g_n = s->n; e->g_nsteps = nsteps; e->g_nscalars = nscalars; e->g_block = g_tune.step_block;
-                if (nscalars) std::memcpy(e->g_scalars, scalars, sizeof(double) * nscalars);
-            }
-        } else {
-            g_launches.fetch_add(nsteps, std::memory_order_relaxed);
-        }
-        if (e->exec) { SOAX_CUDA(cudaGraphLaunch(e->exec, st)); return SOAX_OK; }
-    }
-    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(expr_run(e->impl, s->layout, s->comp, s->n, scalars, nscalars, st));
+    for (int32_t i = 0; i < nsteps; ++i) SOAX_TRY(one());
     return SOAX_OK;
 }
 
 int soax_expr_free(soax_expr* e) {
     if (!e) return SOAX_ERR_INVALID_ARG;
-    if (e->exec) cudaGraphExecDestroy(e->exec);
+    if (e->graph.exec) cudaGraphExecDestroy(e->graph.exec);
     expr_free(e->impl);
     delete e;
     return SOAX_OK;

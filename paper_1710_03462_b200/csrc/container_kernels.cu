@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restri
 // ---- pass 2 (one CTA): exclusive scan of the tile counts in place; info[0] = K = #flagged, info[1] = h = #flagged
 // below m = n - K (the holes of SWAP_LAST) ------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024) kill_scan_kernel(uint32_t* __restrict__ tile_count, int64_t ntiles, const uint8_t* __restrict__ kill,
-                                                         int64_t n, uint64_t* __restrict__ info) {
+                                                         int64_t n, uint64_t* __restrict__ info, int64_t* __restrict__ host_count) {
     __shared__ uint32_t warp_sum[32];
     __shared__ uint32_t carry_sm;
     __shared__ uint32_t cnt_sm;
@@ -105,6 +105,9 @@ __global__ void __launch_bounds__(1024) kill_scan_kernel(uint32_t* __restrict__ 
     if (threadIdx.x == 0) {
         info[0] = K;
         info[1] = (tm < ntiles ? tile_count[tm] : (uint32_t)K) + cnt_sm;
+        info[2] = (uint64_t)m;  // the survivor count
+        *host_count = m;        // mapped pinned host memory owned by the handle: the host reads it after the count event
+        __threadfence_system();
     }
 }
 
@@ -236,7 +239,7 @@ __global__ void __launch_bounds__(256, 2) compact_kernel(Ptrs<L::ncomp> src, Ptr
 // ---- bulk getElement: rows idx[0..m) as packed AoS records ----------------------------------------------------------------
 constexpr int kGTile = 256;
 template <class L>
-__global__ void __launch_bounds__(kGTile) gather_rows_kernel(Ptrs<L::ncomp> a, const uint32_t* __restrict__ idx, int64_t m, unsigned char* aos) {
+__global__ void __launch_bounds__(kGTile) gather_rows_kernel(Ptrs<L::ncomp> a, int64_t n, const uint32_t* __restrict__ idx, int64_t m, unsigned char* aos) {
     constexpr int S = L::aos_stride;
     extern __shared__ __align__(128) unsigned char sm[];
     const int64_t ntiles = (m + kGTile - 1) / kGTile;
@@ -246,6 +249,9 @@ __global__ void __launch_bounds__(kGTile) gather_rows_kernel(Ptrs<L::ncomp> a, c
         if ((int)threadIdx.x < cnt) {
             const uint32_t row = idx[t0 + threadIdx.x];
             unsigned char* rec = sm + threadIdx.x * S;
+            if ((int64_t)row >= n) {  // out of range: never dereferenced, the record is zero bytes
+                for (int b = 0; b < S; ++b) rec[b] = 0;
+            } else {
             // all the (random) loads of a group of components first, then the stores into the packed record, whose
             // fields may be misaligned (Q1): byte images
             constexpr int kGroup = 16;
@@ -264,6 +270,7 @@ __global__ void __launch_bounds__(kGTile) gather_rows_kernel(Ptrs<L::ncomp> a, c
                     memcpy(rec + L::aos_offset(C), v.template get<C>(), sizeof(T));
                 });
             });
+            }
         }
         __syncthreads();
         if (cnt == kGTile) {  // a full tile leaves as one bulk store
@@ -292,7 +299,7 @@ struct RemovePlan {
         auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1, kAlign); return at; };
         tile_count = take((size_t)ntiles * 4);
         seg_count = take((size_t)ntiles * kSegsPerTile * 4);
-        info = take(2 * sizeof(uint64_t));
+        info = take(3 * sizeof(uint64_t));
         holes = take(((size_t)n / 2 + 1) * 4);  // #holes = #movers <= min(K, n - K) <= n / 2
         movers = take(((size_t)n / 2 + 1) * 4);
         total = o;
@@ -301,9 +308,8 @@ struct RemovePlan {
 size_t remove_scratch_bytes(int64_t n) { return RemovePlan(n).total; }
 
 template <class L>
-int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch, int64_t* host_new_n,
-                 int64_t dst_capacity, cudaStream_t st) {
-    if (n == 0) { *host_new_n = 0; return SOAX_OK; }
+int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch, const int64_t** dev_count,
+                 int64_t dst_capacity, int64_t* pin_n, int64_t* host_new_n, cudaEvent_t count_ready, cudaStream_t st) {
     const RemovePlan plan(n);
     char* sc = static_cast<char*>(scratch);
     uint32_t* tile_count = reinterpret_cast<uint32_t*>(sc + plan.tile_count);
@@ -314,12 +320,14 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
     kill_count_kernel<<<(unsigned)plan.ntiles, 256, 0, st>>>(kill, n, tile_count, seg_count);
     const unsigned seg_blocks = (unsigned)(((n + kSeg - 1) / kSeg + 7) / 8);  // 8 warps = 8 segments per CTA
     SOAX_TRY(launched());
-    kill_scan_kernel<<<1, 1024, 0, st>>>(tile_count, plan.ntiles, kill, n, info);
+    kill_scan_kernel<<<1, 1024, 0, st>>>(tile_count, plan.ntiles, kill, n, info, pin_n);
     SOAX_TRY(launched());
-    // Nothing below waits for the count: the kernels read it from `info` on the device, and the one synchronisation
-    // of this call (the host needs the new size for the handle) comes after everything has been enqueued.
-    uint64_t host_info[2] = {0, 0};
-    SOAX_CUDA(cudaMemcpyAsync(host_info, info, sizeof host_info, cudaMemcpyDeviceToHost, st));
+    // Nothing waits for the count, neither here nor on the device: the data kernels read it from `info`, and the scan
+    // kernel itself stores it into the handle's mapped pinned word (no copy node in the stream); `count_ready` lets the
+    // handle pick it up later.
+    *dev_count = reinterpret_cast<const int64_t*>(info + 2);
+    if (host_new_n) SOAX_CUDA(cudaMemcpyAsync(host_new_n, info + 2, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    SOAX_CUDA(cudaEventRecord(count_ready, st));
     if (mode == SOAX_REMOVE_SWAP_LAST) {
         holes_movers_kernel<<<seg_blocks, 256, 0, st>>>(kill, n, info, tile_count, seg_count, holes, movers);
         SOAX_TRY(launched());
@@ -330,26 +338,22 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
         compact_kernel<L><<<seg_blocks, 256, 0, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, tile_count, seg_count, dst_capacity);
         SOAX_TRY(launched());
     }
-    SOAX_CUDA(cudaStreamSynchronize(st));
-    const int64_t m = n - (int64_t)host_info[0];
-    *host_new_n = m;
-    if (mode == SOAX_REMOVE_STABLE && m > dst_capacity) return SOAX_ERR_ALLOC;
     return SOAX_OK;
 }
 
 template <class L>
-int gather_rows_entry(void* const* comps, const uint32_t* idx, int64_t m, void* aos, cudaStream_t st) {
+int gather_rows_entry(void* const* comps, int64_t n, const uint32_t* idx, int64_t m, void* aos, cudaStream_t st) {
     if (m == 0) return SOAX_OK;
     constexpr int smem = kGTile * L::aos_stride;
     const int64_t ntiles = (m + kGTile - 1) / kGTile;
     const int64_t cap = (int64_t)kSMs * 8;
-    gather_rows_kernel<L><<<(unsigned)(ntiles < cap ? ntiles : cap), kGTile, smem, st>>>(make_ptrs<L>(comps), idx, m, static_cast<unsigned char*>(aos));
+    gather_rows_kernel<L><<<(unsigned)(ntiles < cap ? ntiles : cap), kGTile, smem, st>>>(make_ptrs<L>(comps), n, idx, m, static_cast<unsigned char*>(aos));
     return launched();
 }
 
 #define X(L)                                                                                                                  \
-    template int remove_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, int, void*, int64_t*, int64_t, cudaStream_t); \
-    template int gather_rows_entry<L>(void* const*, const uint32_t*, int64_t, void*, cudaStream_t);
+    template int remove_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t); \
+    template int gather_rows_entry<L>(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
 SOAX_FOR_EACH_LAYOUT(X)
 #undef X
 

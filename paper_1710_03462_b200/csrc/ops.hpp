@@ -43,9 +43,12 @@ template <class L> int bin_permute_entry(const BinArgs& a, cudaStream_t st);
 template <class L> size_t bin_scratch_bytes(int64_t n, int log2g);
 
 // NEXT-3 (container_kernels.cu)
+// Enqueues everything and returns: the survivor count is copied (asynchronously) into pin_n (pinned host memory) and, if
+// not null, into host_new_n; count_ready is recorded right after those copies.  *dev_count = its device location.
 template <class L> int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch,
-                                    int64_t* host_new_n, int64_t dst_capacity, cudaStream_t st);
-template <class L> int gather_rows_entry(void* const* comps, const uint32_t* idx, int64_t m, void* aos, cudaStream_t st);
+                                    const int64_t** dev_count, int64_t dst_capacity, int64_t* pin_n, int64_t* host_new_n,
+                                    cudaEvent_t count_ready, cudaStream_t st);
+template <class L> int gather_rows_entry(void* const* comps, int64_t n, const uint32_t* idx, int64_t m, void* aos, cudaStream_t st);
 size_t remove_scratch_bytes(int64_t n);
 
 constexpr int kEnergyBlocks = 1184;  // 148 SMs x 8 CTAs: fixed, so the reduction tree is fixed

@@ -76,9 +76,16 @@ def test_remove_wide_record_and_errors(gpu):
     assert np.array_equal(image(s), oracle.remove_swap_last(base, 89, kill))
     small = Cn.Soax(Cn.R2, 0, capacity=10)
     s2 = device(Cn, Cn.R2, host)
-    with pytest.raises(B.SoaxError) as ei:
-        s2.remove(kd, stable=True, dst=small)
-    assert ei.value.status == B.SOAX_ERR_ALLOC
+    # too small a destination: it receives the survivors that fit, its live count is its capacity, and the pinned host
+    # word still reports the true survivor count (soax_remove never synchronises, so it cannot answer ALLOC itself)
+    true_m = torch.zeros(1, dtype=torch.int64).pin_memory()
+    scratch = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
+    B.soax_remove(s2.handle, small.handle, kd.data_ptr(), B.SOAX_REMOVE_STABLE, scratch.data_ptr(), scratch.numel(),
+                  torch.cuda.current_stream().cuda_stream, host_new_n=true_m.data_ptr())
+    assert small.n == 10
+    torch.cuda.synchronize()
+    assert int(true_m[0]) == int((kill == 0).sum()) > 10
+    assert np.array_equal(image(small), oracle.remove_stable(base, 89, kill)[:10 * 89])
     with pytest.raises(B.SoaxError):
         B.soax_remove(s2.handle, s2.handle, kd.data_ptr(), B.SOAX_REMOVE_STABLE, kd.data_ptr(), 1 << 20)   # dst aliases s
     e = Cn.Soax(Cn.R2, 0, capacity=4)
@@ -135,3 +142,43 @@ def test_every_call_accepts_an_empty_container(gpu):
             s.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, 1e-3, nsteps=2)
         torch.cuda.synchronize()
         assert all(len(v[0]) == 0 for v in s.download().values())
+
+
+def test_remove_is_asynchronous_and_the_count_is_learnt_lazily(gpu):
+    """soax_remove enqueues and returns (no call synchronises).  Several removals are queued back to back on a
+    side stream without reading any count; every later call that needs a live count picks it up by itself, and the chain
+    equals the oracle's chain."""
+    torch, B, Cn = gpu
+    n = 70001
+    host = inputs.make_r1(n, seed=8)
+    rng = np.random.default_rng(4)
+    k1 = (rng.random(n) < 0.3).astype(np.uint8)
+    base = oracle.r1_soa_to_aos(host)
+    after1 = oracle.remove_swap_last(base, 40, k1)
+    n1 = after1.size // 40
+    k2 = (rng.random(n) < 0.5).astype(np.uint8)                      # only its first n1 bytes are read by the second removal
+    after2 = oracle.remove_stable(after1, 40, k2[:n1])
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = device(Cn, Cn.R1, host)
+        d = Cn.Soax(Cn.R1, 0, capacity=n)
+        kd1, kd2 = torch.from_numpy(k1).cuda(), torch.from_numpy(k2).cuda()
+        s.remove_async(kd1)                                          # in place; s.n now pending
+        s.step(B.SOAX_STEP_DRIFT, 0.0, nsteps=1)                     # needs the count: resolves it by itself (dt = 0: no change)
+        s.remove_async(kd2, stable=True, dst=d)                      # d.n pending
+        e = d.energy(B.SOAX_ENERGY_KINETIC)                          # needs d's count
+        assert s.n == n1 and d.n == after2.size // 40
+        assert np.array_equal(image(s), after1) and np.array_equal(image(d), after2)
+        oke = oracle.energy(oracle.r1_aos_to_soa(after2), oracle.KINETIC)
+        assert abs(e - oke) <= 1e-10 * oke
+
+
+def test_get_elements_out_of_range_rows_are_zero_records(gpu):
+    torch, B, Cn = gpu
+    n = 1000
+    host = inputs.make_r1(n, seed=1)
+    s = device(Cn, Cn.R1, host)
+    idx = np.array([0, 999, 1000, 5, 2 ** 31 - 1, 17], np.uint32)
+    got = s.get_elements(torch.from_numpy(idx.view(np.int32)).cuda()).cpu().numpy().reshape(-1, 40)
+    base = oracle.r1_soa_to_aos(host).reshape(-1, 40)
+    for j, i in enumerate(idx):
+        assert np.array_equal(got[j], base[i] if i < n else np.zeros(40, np.uint8)), (j, i)
