@@ -246,8 +246,14 @@ int soax_copy(soax_t* dst, const soax_t* src, void* stream);
  *                                      statement over its components c = 0, 1, ...; every other un-indexed
  *                                      multi-component field in it must have the same dimension and is read as its
  *                                      component c (scalar fields are read as they are)
- *   expr    := + - * / unary-  < <= > >= == !=  &  ( )  numbers  scalar names  field reads  and the calls
- *              fma(a,b,c) sqrt(x) abs(x) min(a,b) max(a,b) floor(x) wrap(x) float(x) double(x) select(cond,a,b)
+ *   expr    := + - * / unary-  < <= > >= == !=  &  |  ( )  numbers  scalar names  field reads  and the calls
+ *              fma(a,b,c) sqrt(x) abs(x) min(a,b) max(a,b) floor(x) wrap(x) float(x) double(x) select(cond,a,b) cell(G)
+ * Precedence, lowest first: comparisons, '|', '&', + -, * /, unary -.  NOTE that '&' and '|' bind TIGHTER than comparisons
+ * (Python's rule, not C's): `flags & 1 != 0` means `(flags & 1) != 0`, and conditions are joined WITH parentheses,
+ * `(pos[0] < a) | (pos[0] >= b)`.  '&' takes two integers of the same type (or an integer literal) or two
+ * conditions; '|' takes two conditions.  A binary operation on two integer LITERALS is evaluated in double (`1/2` is 0.5).
+ * cell(G), G a literal power of two <= 64, is the int32 cell index of the particle on the G^3 grid, (i0*G + i1)*G + i2 with
+ * i_c = (int32)(pos_c*G) clamped into [0, G-1] -- bit-equal to soax_bin_permute's (a10); it needs a field pos of 3 doubles.
  * Semantics: statements run in order for each particle and later statements see earlier assignments; typing is
  * C's: float op float is float, anything with a double is double, an assignment rounds to the target's type
  * (`a += b` is `a = (T)(a + b)`); named scalars and literals with a '.' or exponent are double, integer literals
@@ -275,6 +281,15 @@ int soax_expr_compile_sum(const soax_layout* layout, const char* expression, con
                           int32_t nscalars, soax_expr** out);
 int soax_expr_sum(const soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* dev_scratch,
                   size_t scratch_bytes, double* dev_out, void* stream);
+/* User-written MASKS (what soax_remove consumes; PAPER.md:175 removal, 304-307): `condition` is ONE condition of the same
+ * language -- a comparison, or comparisons joined by '&' and '|' -- e.g. "(flags & 1) != 0" or, for the particles that left
+ * the cell range [lo, hi) of a slab decomposition, "(double(cell(64)) < lo) | (double(cell(64)) >= hi)".  soax_expr_mask
+ * writes one byte per live particle into dev_mask (n bytes, 4-byte aligned): 1 where the condition holds, else 0, with the
+ * access shape of the other generated kernels (4 particles per thread, one 32-bit store of 4 mask bytes).  Asynchronous.
+ * A mask program cannot be passed to soax_expr_run / soax_expr_sum, nor the other kinds to soax_expr_mask (INVALID_ARG). */
+int soax_expr_compile_mask(const soax_layout* layout, const char* condition, const char* const* scalar_names,
+                           int32_t nscalars, soax_expr** out);
+int soax_expr_mask(const soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, uint8_t* dev_mask, void* stream);
 /* Message of the last failed soax_expr_compile on the calling thread ("" if none). */
 const char* soax_expr_error(void);
 /* The generated CUDA source (owned by the handle), for inspection. */

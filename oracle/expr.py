@@ -12,6 +12,10 @@ plain definition of what such a program computes, following the language rules s
     the type of the target; `a += b` is `a = (T)(a + b)`;
   * a dim-3 field without index expands the statement over c = 0, 1, 2;
   * integer fields can only be compared, masked with '&' or converted with float()/double();
+  * conditions (comparison results) can be joined with '&' and '|' (both operands parenthesised comparisons: '&' and '|'
+    bind tighter than comparisons, as in Python); cell(G) is the int32 cell index (i0*G + i1)*G + i2 of the particle on a
+    G^3 grid, i_c = trunc(pos_c*G) clamped into [0, G-1] (SURVEY.md 8(c) "BINNING" + the clamp stated in include/soax.h);
+  * a MASK program is one condition; its value per particle is a byte, 1 where it holds (mask());
   * nothing is contracted: the only fused multiply-adds are the fma() calls, evaluated with std::fma/std::fmaf
     (oracle.fma); min/max are C's fmin/fmax; wrap(x) = x - floor(x) with a result of exactly 1 mapped to 0 (Q3).
 
@@ -124,9 +128,14 @@ class _Eval:
             return -v
         if isinstance(node, ast.BinOp):
             a, b = self.ev(node.left), self.ev(node.right)
+            is_cond = lambda x: isinstance(x, np.ndarray) and x.dtype == bool      # noqa: E731
+            if isinstance(node.op, (ast.BitAnd, ast.BitOr)) and is_cond(a) and is_cond(b):
+                return np.logical_and(a, b) if isinstance(node.op, ast.BitAnd) else np.logical_or(a, b)
+            if isinstance(node.op, ast.BitOr):
+                raise ExprError("'|' joins two conditions")
             if isinstance(node.op, ast.BitAnd):
                 if not (_is_int(a) and _is_int(b)):
-                    raise ExprError("'&' needs integer operands")
+                    raise ExprError("'&' needs integer operands or two conditions")
                 dt = next(x.dtype for x in (a, b) if isinstance(x, np.ndarray)) if any(isinstance(x, np.ndarray) for x in (a, b)) else np.int64
                 av, bv = (np.asarray(x.v, dtype=dt) if isinstance(x, _IntLit) else x for x in (a, b))
                 return np.bitwise_and(av, bv)
@@ -162,8 +171,22 @@ class _Eval:
         if isinstance(node, ast.Call):
             if not isinstance(node.func, ast.Name) or node.keywords:
                 raise ExprError("unsupported call")
+            if node.func.id == "cell":
+                return self.cell(node.args)
             return self.call(node.func.id, [self.ev(a) for a in node.args])
         raise ExprError(f"unsupported syntax: {ast.dump(node)}")
+
+    def cell(self, args):
+        """a10: i_c = (int32)(pos_c * G) (exact product, truncation), clamped into the grid; cell = (i0*G + i1)*G + i2."""
+        if len(args) != 1 or not isinstance(args[0], ast.Constant) or not isinstance(args[0].value, int) or isinstance(args[0].value, bool):
+            raise ExprError("cell(G): G must be an integer literal")
+        G = args[0].value
+        if G < 1 or G > 64 or G & (G - 1):
+            raise ExprError("cell(G): G must be a power of two, 1 <= G <= 64")
+        if "pos" not in self.f or self.dims["pos"] != 3 or self.f["pos"][0].dtype != np.float64:
+            raise ExprError("cell(G) needs a field pos of three doubles")
+        i = [np.clip(np.trunc(self.f["pos"][c] * float(G)), 0, G - 1).astype(np.int32) for c in range(3)]
+        return (i[0] * np.int32(G) + i[1]) * np.int32(G) + i[2]
 
     def call(self, fn: str, a: list):
         r = self._call(fn, a)
@@ -277,3 +300,19 @@ def total(fields: dict, expression: str, scalars: dict | None = None) -> float:
         raise ExprError("the summed expression must be a floating-point value")
     terms = np.broadcast_to(v.astype(np.float64), (n,))
     return math.fsum(terms.tolist())
+
+
+def mask(fields: dict, condition: str, scalars: dict | None = None) -> np.ndarray:
+    """The mask programs of soax_expr_compile_mask: one condition, evaluated per particle as in `run`; returns uint8, 1 where
+    it holds."""
+    n = next(iter(fields.values())).shape[1]
+    state = {k: [np.array(v[c]) for c in range(v.shape[0])] for k, v in fields.items()}
+    dims = {k: v.shape[0] for k, v in fields.items()}
+    try:
+        tree = ast.parse(condition.strip().rstrip(";"), mode="eval")
+    except SyntaxError as e:
+        raise ExprError(str(e)) from e
+    v = _Eval(state, dims, dict(scalars or {}), n).ev(tree.body)
+    if not (isinstance(v, np.ndarray) and v.dtype == bool):
+        raise ExprError("the mask expression must be a condition")
+    return np.broadcast_to(v, (n,)).astype(np.uint8)

@@ -74,6 +74,8 @@ SIGNATURES = {
     "soax_expr_compile": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
     "soax_expr_compile_sum": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
     "soax_expr_sum": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _vp, _sz, _vp, _vp]),
+    "soax_expr_compile_mask": (C.c_int, [_vp, C.c_char_p, C.POINTER(C.c_char_p), _i32, C.POINTER(_vp)]),
+    "soax_expr_mask": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _vp, _vp]),
     "soax_expr_run": (C.c_int, [_vp, _vp, C.POINTER(_f64), _i32, _i32, _vp]),
     "soax_expr_free": (C.c_int, [_vp]),
     "soax_expr_error": (C.c_char_p, []),
@@ -285,6 +287,22 @@ def soax_expr_compile_sum(layout: int, expression: str, scalar_names: Sequence[s
         e.args = (f"{e.args[0]}: {lib().soax_expr_error().decode()}",)
         raise e
     return out.value
+
+
+def soax_expr_compile_mask(layout: int, condition: str, scalar_names: Sequence[str] = ()) -> int:
+    names = (C.c_char_p * max(len(scalar_names), 1))(*[n.encode() for n in scalar_names])
+    out = _vp()
+    status = lib().soax_expr_compile_mask(layout, condition.encode(), names, len(scalar_names), C.byref(out))
+    if status != SOAX_OK:
+        e = SoaxError(status, "soax_expr_compile_mask")
+        e.args = (f"{e.args[0]}: {lib().soax_expr_error().decode()}",)
+        raise e
+    return out.value
+
+
+def soax_expr_mask(s: int, e: int, scalars: Sequence[float], dev_mask: int, stream: int = 0) -> None:
+    arr = (_f64 * max(len(scalars), 1))(*[float(x) for x in scalars])
+    _check(lib().soax_expr_mask(s, e, arr, len(scalars), dev_mask, stream), "soax_expr_mask")
 
 
 def soax_expr_sum(s: int, e: int, scalars: Sequence[float], dev_scratch: int, scratch_bytes: int, dev_out: int, stream: int = 0) -> None:

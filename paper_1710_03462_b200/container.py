@@ -242,6 +242,36 @@ class SumProgram:
         return float(self.sum_async(s, **scalars).item())
 
 
+class MaskProgram:
+    """A user-written condition compiled into a kernel that writes one byte per particle (soax_expr_compile_mask): the kill
+    mask soax_remove consumes, produced on the device (e.g. "(flags & 1) != 0", or the particles that left a cell range)."""
+
+    def __init__(self, fields, condition: str, scalar_names=(), dynamic: bool = False):
+        self.fields, self.condition, self.scalar_names = tuple(fields), condition, tuple(scalar_names)
+        self.layout = (B.soax_layout_define_dynamic if dynamic else B.soax_layout_define)(self.fields)
+        self.handle = B.soax_expr_compile_mask(self.layout, condition, self.scalar_names)
+        self.bytes_read, self.bytes_written = B.soax_expr_traffic(self.handle)
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h:
+            try:
+                B.soax_expr_free(h)
+            except Exception:
+                pass
+
+    @property
+    def cuda_source(self) -> str:
+        return B.soax_expr_cuda_source(self.handle)
+
+    def mask(self, s: Soax, out: torch.Tensor | None = None, **scalars) -> torch.Tensor:
+        n = s.n
+        out = torch.empty(max(n, 4), dtype=torch.uint8, device=s.slab.device) if out is None else out
+        assert out.dtype == torch.uint8 and out.numel() >= n
+        B.soax_expr_mask(s.handle, self.handle, [scalars[k] for k in self.scalar_names], out.data_ptr(), _stream())
+        return out[:n]
+
+
 def aos_step(fields, aos: torch.Tensor, n: int, kind: int, dt: float, nsteps: int = 1, variant: int = 0, k: float = 1.0,
              center: float = 0.5) -> None:
     layout = B.soax_layout_define(fields)

@@ -506,7 +506,7 @@ struct soax_expr {
     GraphCache graph;  // captured nsteps-launch loop, replayed while the call is the same (as soax_step does)
 };
 
-static int expr_compile_any(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars, bool is_sum,
+static int expr_compile_any(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars, int kind,
                             soax_expr** out) {
     if (!l || !source || !out || nscalars < 0 || nscalars > 16 || (nscalars > 0 && !scalar_names)) return SOAX_ERR_INVALID_ARG;
     ExprLayoutInfo info{};
@@ -515,7 +515,7 @@ static int expr_compile_any(const soax_layout* l, const char* source, const char
     for (int f = 0; f < l->nfields; ++f) { info.fname[f] = l->fname[f]; info.fdim[f] = l->fdim[f]; info.fbegin[f] = l->fbegin[f]; }
     for (int c = 0; c < l->ncomp; ++c) { info.cdtype[c] = l->cdtype[c]; info.csize[c] = l->csize[c]; }
     CompiledExpr* impl = nullptr;
-    SOAX_TRY(expr_compile(info, l, source, scalar_names, nscalars, is_sum, &impl));
+    SOAX_TRY(expr_compile(info, l, source, scalar_names, nscalars, kind, &impl));
     soax_expr* e = new (std::nothrow) soax_expr();
     if (!e) { expr_free(impl); return SOAX_ERR_ALLOC; }
     e->impl = impl;
@@ -526,12 +526,25 @@ static int expr_compile_any(const soax_layout* l, const char* source, const char
 
 int soax_expr_compile(const soax_layout* l, const char* source, const char* const* scalar_names, int32_t nscalars,
                       soax_expr** out) {
-    return expr_compile_any(l, source, scalar_names, nscalars, false, out);
+    return expr_compile_any(l, source, scalar_names, nscalars, 0, out);
 }
 
 int soax_expr_compile_sum(const soax_layout* l, const char* expression, const char* const* scalar_names, int32_t nscalars,
                           soax_expr** out) {
-    return expr_compile_any(l, expression, scalar_names, nscalars, true, out);
+    return expr_compile_any(l, expression, scalar_names, nscalars, 1, out);
+}
+
+int soax_expr_compile_mask(const soax_layout* l, const char* condition, const char* const* scalar_names, int32_t nscalars,
+                           soax_expr** out) {
+    return expr_compile_any(l, condition, scalar_names, nscalars, 2, out);
+}
+
+int soax_expr_mask(const soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, uint8_t* dev_mask, void* stream) {
+    if (!s || !e || nscalars < 0 || nscalars > 16 || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
+    if (s->layout != e->layout) return SOAX_ERR_INVALID_ARG;
+    const int64_t n = live(s);
+    if (n > 0 && (!dev_mask || !aligned(dev_mask, 4))) return SOAX_ERR_INVALID_ARG;
+    return expr_mask(e->impl, s->layout, const_cast<void* const*>(s->comp), n, scalars, nscalars, dev_mask, (cudaStream_t)stream);
 }
 
 int soax_expr_sum(const soax_t* s, soax_expr* e, const double* scalars, int32_t nscalars, void* dev_scratch, size_t scratch_bytes,

@@ -99,7 +99,7 @@ std::vector<Tok> tokenize(const std::string& s) {
             for (const char* op : two)
                 if (s.compare(i, 2, op) == 0) { t.text = op; i += 2; found = true; break; }
             if (!found) {
-                if (!std::strchr("+-*/()[],;=<>&", ch)) throw ParseError{std::string("unexpected character '") + ch + "'", i};
+                if (!std::strchr("+-*/()[],;=<>&|", ch)) throw ParseError{std::string("unexpected character '") + ch + "'", i};
                 t.text = std::string(1, ch);
                 ++i;
             }
@@ -127,6 +127,7 @@ struct Program {
     std::vector<bool> touched;
     std::string body;              // statements over the locals, one particle
     bool is_sum = false;           // the program is ONE expression whose per-particle value is summed in double
+    bool is_mask = false;          // the program is ONE condition whose per-particle truth value is written as a byte
 };
 
 std::string hex_double(double v) {
@@ -156,6 +157,15 @@ class Parser {
         if (v.ty == T_ILIT) v = to_float(v, T_F64, 0);
         if (!is_float(v.ty)) fail("the summed expression must be a floating-point value (use float()/double())");
         P_.body += "        acc += (double)" + v.code + ";\n";
+    }
+
+    // a mask program: one condition (a comparison, or comparisons joined by '&' and '|'), stored as one byte per particle
+    void mask_expression() {
+        Val v = expr();
+        if (is_op(";")) next();
+        if (peek().kind != Tok::END) fail("a mask program is a single condition");
+        if (v.ty != T_BOOL) fail("the mask expression must be a condition (a comparison, or comparisons joined by '&' / '|')");
+        P_.body += "        mk[j] = " + v.code + " ? (unsigned char)1 : (unsigned char)0;\n";
     }
 
   private:
@@ -256,12 +266,24 @@ class Parser {
     }
 
     // ---- expressions: comparison < additive < multiplicative < unary < primary ------------------------------------------
+    // precedence (lowest first, Python's): comparison, '|', '&', additive, multiplicative, unary.  '&' and '|' bind TIGHTER
+    // than comparisons, so conditions are joined as (a < b) & (c >= d) -- with the parentheses.
     Val expr() {
-        Val a = bitand_();
+        Val a = bitor_();
         while (is_op("<") || is_op("<=") || is_op(">") || is_op(">=") || is_op("==") || is_op("!=")) {
             const Tok op = next();
-            Val b = bitand_();
+            Val b = bitor_();
             a = compare(op.text, a, b, op.pos);
+        }
+        return a;
+    }
+    Val bitor_() {
+        Val a = bitand_();
+        while (is_op("|")) {
+            const Tok op = next();
+            Val b = bitand_();
+            if (a.ty != T_BOOL || b.ty != T_BOOL) throw ParseError{"'|' joins two conditions (parenthesised comparisons)", op.pos};
+            a = Val{"(" + a.code + " || " + b.code + ")", T_BOOL};
         }
         return a;
     }
@@ -270,7 +292,8 @@ class Parser {
         while (is_op("&")) {
             const Tok op = next();
             Val b = additive();
-            if (!is_int(a.ty) || !is_int(b.ty)) throw ParseError{"'&' needs integer operands", op.pos};
+            if (a.ty == T_BOOL && b.ty == T_BOOL) { a = Val{"(" + a.code + " && " + b.code + ")", T_BOOL}; continue; }
+            if (!is_int(a.ty) || !is_int(b.ty)) throw ParseError{"'&' needs integer operands or two conditions", op.pos};
             const int ty = a.ty == T_ILIT ? b.ty : a.ty;
             if (a.ty != T_ILIT && b.ty != T_ILIT && a.ty != b.ty) throw ParseError{"'&' between different integer types", op.pos};
             a = Val{"((" + std::string(c_name(ty)) + ")(" + a.code + " & " + b.code + "))", ty == T_ILIT ? T_I64 : ty};
@@ -380,6 +403,18 @@ class Parser {
             if (v.ty == T_ILIT) return to_float(v, ty, fn.pos);
             return Val{"((" + std::string(c_name(ty)) + ")" + v.code + ")", ty};
         }
+        if (n == "cell") {  // a10: the particle's cell index on a G^3 grid, bit-equal to soax_bin_permute's
+            expect("(");
+            if (peek().kind != Tok::INT) fail("cell(G): G must be an integer literal");
+            const long long G = next().ival;
+            expect(")");
+            if (G < 1 || G > 64 || (G & (G - 1)) != 0) throw ParseError{"cell(G): G must be a power of two, 1 <= G <= 64", fn.pos};
+            const int f = find_field("pos");
+            if (f < 0 || P_.L->fdim[f] != 3 || P_.L->cdtype[P_.L->fbegin[f]] != T_F64) throw ParseError{"cell(G) needs a field pos of three doubles", fn.pos};
+            const int c0 = P_.L->fbegin[f];
+            for (int c = 0; c < 3; ++c) mark_read(c0 + c);
+            return Val{"soax_cell(" + local(c0) + ", " + local(c0 + 1) + ", " + local(c0 + 2) + ", " + std::to_string(G) + ")", T_I32};
+        }
         if (n == "select") {
             std::vector<Val> a = call_args(3, fn);
             if (a[0].ty != T_BOOL) throw ParseError{"select(cond, a, b): cond must be a comparison", fn.pos};
@@ -462,6 +497,14 @@ __device__ __forceinline__ double soax_wrap01(double x) {
     else w = x - floor(x);
     return w >= 1.0 ? 0.0 : w;
 }
+// a10: cell index on a G^3 grid, x slowest (Q11); pos*G is exact for G a power of two (Q16); truncation toward zero; an index
+// outside the grid (a position outside [0,1): a precondition violation) is clamped into it, as soax_bin_permute does
+__device__ __forceinline__ int soax_cell(double x0, double x1, double x2, int G) {
+    const int i0 = min(max((int)(x0 * (double)G), 0), G - 1);
+    const int i1 = min(max((int)(x1 * (double)G), 0), G - 1);
+    const int i2 = min(max((int)(x2 * (double)G), 0), G - 1);
+    return (i0 * G + i1) * G + i2;
+}
 __device__ __forceinline__ float soax_wrap01f(float x) {
     float w;
     if (x >= -1.0f && x < 2.0f) w = x + (x < 0.0f ? 1.0f : (x >= 1.0f ? -1.0f : 0.0f));
@@ -475,7 +518,8 @@ std::string generate(const Program& P) {
     std::string s = "// generated by soax_expr_compile -- one fused pass, 4 particles per thread\n";
     s += kPrelude;
     s += "struct Args { void* p[" + std::to_string(L.ncomp) + "]; double s[" + std::to_string(P.scalar_names.empty() ? 1 : P.scalar_names.size()) + "]; };\n";
-    s += std::string("template <int P> __device__ __forceinline__ ") + (P.is_sum ? "double" : "void") + " group(const Args& a, long long i0) {\n";
+    s += std::string("template <int P> __device__ __forceinline__ ") + (P.is_sum ? "double" : "void") + " group(const Args& a, long long i0" +
+         (P.is_mask ? ", unsigned char* mask" : "") + ") {\n";
     for (int c = 0; c < L.ncomp; ++c) {
         if (!P.touched[c]) continue;
         const std::string T = c_name(L.cdtype[c]), v = "v" + std::to_string(c);
@@ -483,6 +527,7 @@ std::string generate(const Program& P) {
         else s += "    Vec<" + T + ", P> " + v + ";\n";
     }
     if (P.is_sum) s += "    double acc = 0.0;\n";
+    if (P.is_mask) s += "    unsigned char mk[P];\n";
     s += "#pragma unroll\n    for (int j = 0; j < P; ++j) {\n";
     for (int c = 0; c < L.ncomp; ++c)
         if (P.touched[c]) s += "        " + std::string(c_name(L.cdtype[c])) + "& x" + std::to_string(c) + " = v" + std::to_string(c) + ".v[j];\n";
@@ -494,8 +539,21 @@ std::string generate(const Program& P) {
             s += "    st_vec<" + T + ", P>(static_cast<" + T + "*>(a.p[" + std::to_string(c) + "]) + i0, v" + std::to_string(c) + ");\n";
         }
     if (P.is_sum) s += "    return acc;\n";
+    if (P.is_mask)  // four mask bytes leave as one 32-bit store (mask + i0 is 4-byte aligned: i0 is a multiple of 4)
+        s += "    if constexpr (P == 4) *reinterpret_cast<unsigned*>(mask + i0) = mk[0] | (mk[1] << 8) | (mk[2] << 16) | ((unsigned)mk[3] << 24);\n"
+             "    else mask[i0] = mk[0];\n";
     s += "}\n";
-    if (!P.is_sum) {
+    if (P.is_mask) {
+        s += R"K(extern "C" __global__ void __launch_bounds__(512) soax_expr_kernel(const Args a, const long long n, unsigned char* mask) {
+    const long long ngroups = n / 4;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long g = tid; g < ngroups; g += stride) group<4>(a, g * 4, mask);
+    const long long t = ngroups * 4 + tid;
+    if (t < n) group<1>(a, t, mask);
+}
+)K";
+    } else if (!P.is_sum) {
         s += R"K(extern "C" __global__ void __launch_bounds__(512) soax_expr_kernel(const Args a, const long long n) {
     const long long ngroups = n / 4;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -632,7 +690,7 @@ struct CompiledExpr {
     const void* layout_key = nullptr;
     int ncomp = 0, nscalars = 0;
     int bytes_read = 0, bytes_written = 0;
-    bool is_sum = false;
+    bool is_sum = false, is_mask = false;
     std::string source, cuda_source;
     std::vector<char> cubin;
     std::mutex mu;
@@ -640,13 +698,21 @@ struct CompiledExpr {
     cudaKernel_t kernel = nullptr;
 };
 
-int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* source, const char* const* scalar_names,
-                 int nscalars, bool is_sum, CompiledExpr** out) {
+static bool is_identifier(const char* s) {
+    if (!((*s >= 'a' && *s <= 'z') || (*s >= 'A' && *s <= 'Z') || *s == '_')) return false;
+    for (; *s; ++s)
+        if (!((*s >= 'a' && *s <= 'z') || (*s >= 'A' && *s <= 'Z') || (*s >= '0' && *s <= '9') || *s == '_')) return false;
+    return true;
+}
+
+static int expr_compile_impl(const ExprLayoutInfo& L, const void* layout_key, const char* source, const char* const* scalar_names,
+                             int nscalars, int kind, CompiledExpr** out) {
+    const bool is_sum = kind == 1, is_mask = kind == 2;
     g_expr_error.clear();
     Program P;
     P.L = &L;
     for (int k = 0; k < nscalars; ++k) {
-        if (!scalar_names[k] || !*scalar_names[k]) { g_expr_error = "empty scalar name"; return SOAX_ERR_INVALID_ARG; }
+        if (!scalar_names[k] || !is_identifier(scalar_names[k])) { g_expr_error = "a scalar name must be an identifier"; return SOAX_ERR_INVALID_ARG; }
         for (int f = 0; f < L.nfields; ++f)
             if (std::strcmp(L.fname[f], scalar_names[k]) == 0) { g_expr_error = std::string("scalar '") + scalar_names[k] + "' has the name of a field"; return SOAX_ERR_INVALID_ARG; }
         P.scalar_names.push_back(scalar_names[k]);
@@ -656,8 +722,10 @@ int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* so
     P.touched.assign(L.ncomp, false);
     try {
         P.is_sum = is_sum;
+        P.is_mask = is_mask;
         Parser parser(source, P);
         if (is_sum) parser.sum_expression();
+        else if (is_mask) parser.mask_expression();
         else parser.program();
     } catch (const ParseError& e) {
         char where[64];
@@ -667,18 +735,20 @@ int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* so
     }
     bool any = false;
     for (int c = 0; c < L.ncomp; ++c) any |= P.assigned[c];
-    if (!any && !is_sum) { g_expr_error = "the program assigns nothing"; return SOAX_ERR_INVALID_ARG; }
+    if (!any && !is_sum && !is_mask) { g_expr_error = "the program assigns nothing"; return SOAX_ERR_INVALID_ARG; }
     std::unique_ptr<CompiledExpr> E(new (std::nothrow) CompiledExpr());
     if (!E) return SOAX_ERR_ALLOC;
     E->layout_key = layout_key;
     E->ncomp = L.ncomp;
     E->nscalars = nscalars;
     E->is_sum = is_sum;
+    E->is_mask = is_mask;
     E->source = source;
     for (int c = 0; c < L.ncomp; ++c) {
         if (P.read_first[c]) E->bytes_read += L.csize[c];
         if (P.assigned[c]) E->bytes_written += L.csize[c];
     }
+    if (is_mask) E->bytes_written += 1;
     try {
         E->cuda_source = generate(P);
     } catch (const ParseError& e) {
@@ -690,9 +760,23 @@ int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* so
     return SOAX_OK;
 }
 
+// No C++ exception may cross the C boundary: anything the parser or the standard library throws becomes a status.
+int expr_compile(const ExprLayoutInfo& L, const void* layout_key, const char* source, const char* const* scalar_names,
+                 int nscalars, int kind, CompiledExpr** out) {
+    try {
+        return expr_compile_impl(L, layout_key, source, scalar_names, nscalars, kind, out);
+    } catch (const std::bad_alloc&) {
+        g_expr_error = "out of host memory";
+        return SOAX_ERR_ALLOC;
+    } catch (...) {
+        g_expr_error = "internal error while compiling the program";
+        return SOAX_ERR_INVALID_ARG;
+    }
+}
+
 int expr_run(CompiledExpr* E, const void* layout_key, void* const* comps, int64_t n, const double* scalars, int nscalars,
              cudaStream_t st) {
-    if (E->layout_key != layout_key || E->is_sum) return SOAX_ERR_INVALID_ARG;
+    if (E->layout_key != layout_key || E->is_sum || E->is_mask) return SOAX_ERR_INVALID_ARG;
     if (nscalars != E->nscalars || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
     {
         std::lock_guard<std::mutex> lock(E->mu);
@@ -738,6 +822,31 @@ int expr_sum(CompiledExpr* E, const void* layout_key, void* const* comps, int64_
     SOAX_CUDA(cudaLaunchKernel(reinterpret_cast<const void*>(E->kernel), dim3(kEnergyBlocks), dim3(256), params, 0, st));
     SOAX_TRY(launched());
     return sum_partials(partial, kEnergyBlocks, out, st);
+}
+
+// A mask program: one byte per live particle (1 where the condition holds), same launch shape as expr_run.
+int expr_mask(CompiledExpr* E, const void* layout_key, void* const* comps, int64_t n, const double* scalars, int nscalars,
+              unsigned char* mask, cudaStream_t st) {
+    if (E->layout_key != layout_key || !E->is_mask) return SOAX_ERR_INVALID_ARG;
+    if (nscalars != E->nscalars || (nscalars > 0 && !scalars)) return SOAX_ERR_INVALID_ARG;
+    {
+        std::lock_guard<std::mutex> lock(E->mu);
+        if (!E->kernel) {
+            SOAX_CUDA(cudaLibraryLoadData(&E->lib, E->cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0));
+            SOAX_CUDA(cudaLibraryGetKernel(&E->kernel, E->lib, "soax_expr_kernel"));
+        }
+    }
+    if (n == 0) return SOAX_OK;
+    std::vector<unsigned char> args((size_t)E->ncomp * sizeof(void*) + (size_t)(nscalars > 0 ? nscalars : 1) * sizeof(double), 0);
+    std::memcpy(args.data(), comps, (size_t)E->ncomp * sizeof(void*));
+    if (nscalars > 0) std::memcpy(args.data() + (size_t)E->ncomp * sizeof(void*), scalars, (size_t)nscalars * sizeof(double));
+    long long nn = n;
+    void* params[] = {args.data(), &nn, &mask};
+    const int block = g_tune.step_block;
+    const int64_t threads = n / 4 > n % 4 ? n / 4 : n % 4;
+    const int64_t blocks = (threads + block - 1) / block;
+    SOAX_CUDA(cudaLaunchKernel(reinterpret_cast<const void*>(E->kernel), dim3((unsigned)(blocks < 1 ? 1 : blocks)), dim3((unsigned)block), params, 0, st));
+    return launched();
 }
 
 void expr_free(CompiledExpr* E) {

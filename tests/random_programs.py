@@ -62,3 +62,26 @@ def program(seed: int) -> str:
             rhs = _expr(rng, 3)
             stmts.append(f"{rng.choice(TARGETS)} {op} " + (f"(abs({rhs}) + 1)" if op == "/=" else rhs))   # no division by zero
     return "; ".join(stmts)
+
+
+def _cond(rng, depth):
+    """a random condition over R2: comparisons of float expressions, integer tests, cell tests, joined by & and |"""
+    if depth > 0 and rng.random() < 0.6:
+        return f"({_cond(rng, depth - 1)}) {rng.choice('&|')} ({_cond(rng, depth - 1)})"
+    kind = rng.randrange(6)
+    if kind < 2:
+        return f"{_expr(rng, 2)} {rng.choice(['<', '<=', '>', '>=', '==', '!='])} {_expr(rng, 2)}"
+    if kind == 2:
+        return f"(flags & {rng.choice([1, 2, 4, 64, 255])}) {rng.choice(['!=', '=='])} {rng.choice([0, 0, 4])}"
+    if kind == 3:
+        G = rng.choice([1, 2, 8, 64])
+        return f"cell({G}) {rng.choice(['<', '>=', '==', '!='])} {rng.randrange(max(1, G ** 3))}"
+    if kind == 4:
+        G = rng.choice([4, 16, 64])
+        return f"double(cell({G})) {rng.choice(['<', '>='])} {rng.choice(['a * 1000', 'lo', '0.5 * lo'])}"
+    return f"id {rng.choice(['<', '>=', '!='])} {rng.randrange(600)}"
+
+
+def condition(seed: int) -> str:
+    """one mask program (soax_expr_compile_mask) over R2 with the scalars a, b, lo"""
+    return _cond(random.Random(10_000 + seed), 2)

@@ -250,3 +250,66 @@ def test_random_programs_compile_and_the_oracle_evaluates_them(compiler):
         if seed < 20:
             out = oexpr.run(host, src, {"a": 0.75, "b": -1.5})
             assert all(np.isfinite(out[k]).all() for k in ("pos", "vel", "acc", "mass", "charge")), src
+
+
+# ------------------------------------------------------------------------------------------- masks (NEXT-3 feed)
+def test_mask_oracle_hand_values_cell_and_joins(golden_dir):
+    """Pins for oexpr.mask / cell() / '&' '|' on conditions: the 6-particle binning fixture (cells 4,1,4,3,1,7
+    on a 2^3 grid), the already pinned cell index of oracle.bin_r1 on random positions, hand-written flag tests, and the
+    clamp of cell() for a position outside the box."""
+    pos = np.array([[.75, .25, .25], [.25, .25, .75], [.75, .25, .40], [.10, .90, .90], [.25, .25, .60], [.99, .99, .99]]).T.copy()
+    f = {"id": np.arange(6, dtype=np.int32)[None], "pos": pos, "vel": np.zeros((3, 6), np.float32)}
+    assert oexpr.mask(f, "cell(2) == 4").tolist() == [1, 0, 1, 0, 0, 0]
+    assert oexpr.mask(f, "(cell(2) < 2) | (cell(2) >= 7)").tolist() == [0, 1, 0, 0, 1, 1]
+    assert oexpr.mask(f, "(cell(2) >= 2) & (cell(2) < 7)").tolist() == [1, 0, 1, 1, 0, 0]
+    assert oexpr.mask(f, "(double(cell(2)) < lo) | (double(cell(2)) >= hi)", {"lo": 2, "hi": 7}).tolist() == [0, 1, 0, 0, 1, 1]
+    assert oexpr.mask(f, "cell(1) == 0").tolist() == [1] * 6
+    assert oexpr.mask(f, "(pos[0] > 0.5) & (id != 5)").tolist() == [1, 0, 1, 0, 0, 0]
+    assert oexpr.mask(f, "((pos[0] > 0.5) & (id != 5)) | (id == 1)").tolist() == [1, 1, 1, 0, 0, 0]
+    h = inputs.make_r1(20000, seed=5)
+    for G in (1, 2, 8, 64):
+        cell = oracle.bin_r1(h, G, want_perm=False)["cell"]            # pinned by the fixture + brute force in test_oracle_pins
+        for k in (0, G ** 3 // 2, G ** 3 - 1):
+            assert np.array_equal(oexpr.mask(h, f"cell({G}) == {k}"), (cell == k).astype(np.uint8))
+            assert np.array_equal(oexpr.mask(h, f"double(cell({G})) >= t", {"t": k}), (cell >= k).astype(np.uint8))
+    out = {"id": np.zeros((1, 3), np.int32), "pos": np.array([[-0.25, 0.5, 1.5], [0.5, 0.5, 0.5], [0.5, 0.5, 0.5]]), "vel": np.zeros((3, 3), np.float32)}
+    assert [int(m) for m in (oexpr.mask(out, "cell(4) == 10"), oexpr.mask(out, "cell(4) == 42"), oexpr.mask(out, "cell(4) == 58"))[0:1][0]] == [1, 0, 0]
+    assert oexpr.mask(out, "cell(4) == 42").tolist() == [0, 1, 0] and oexpr.mask(out, "cell(4) == 58").tolist() == [0, 0, 1]   # clamped to i0 = 0 / 3
+    r2 = inputs.make_r2(1000, seed=2)
+    assert np.array_equal(oexpr.mask(r2, "(flags & 1) != 0"), (r2["flags"][0] & 1).astype(np.uint8))
+    assert np.array_equal(oexpr.mask(r2, "((flags & 6) == 6) | (mass < 1)"),
+                          (((r2["flags"][0] & 6) == 6) | (r2["mass"][0] < np.float32(1))).astype(np.uint8))
+    for bad in ("pos[0]", "flags & 1", "(pos[0] < 1) | 3", "cell(3) == 0", "cell(pos) == 0", "(pos[0] < 1) < 2"):
+        with pytest.raises(oexpr.ExprError):
+            oexpr.mask(r2, bad)
+
+
+def test_mask_program_compiles_and_rejects(compiler):
+    from tests.random_programs import condition
+    B, Cn = compiler
+    L1, L2 = B.soax_layout_define(Cn.R1), B.soax_layout_define(Cn.R2)
+    e = B.soax_expr_compile_mask(L1, "(double(cell(64)) < lo) | (double(cell(64)) >= hi)", ["lo", "hi"])
+    src = B.soax_expr_cuda_source(e)
+    assert src.count("__global__") == 1 and "soax_cell(" in src and "st_vec<" not in src.split("struct Args")[1]
+    assert B.soax_expr_traffic(e) == (24, 1)                          # reads pos only, writes one byte per particle
+    B.soax_expr_free(e)
+    e = B.soax_expr_compile_mask(L2, "(flags & 1) != 0", [])
+    assert B.soax_expr_traffic(e) == (1, 1)
+    B.soax_expr_free(e)
+    B.soax_expr_free(B.soax_expr_compile_mask(L2, "flags & 1 != 0", []))   # '&' binds tighter than '!=' (Python's rule): (flags & 1) != 0
+    assert np.array_equal(oexpr.mask(inputs.make_r2(100, seed=1), "flags & 1 != 0"), oexpr.mask(inputs.make_r2(100, seed=1), "(flags & 1) != 0"))
+    for bad, msg in (("pos[0]", "must be a condition"), ("(pos[0] < 1) | 3", "joins two conditions"),
+                     ("cell(3) == 1", "power of two"), ("pos[0] < 1; pos[1] < 2", "single condition"), ("vel[0] = 1.0", "")):
+        with pytest.raises(B.SoaxError) as ei:
+            B.soax_expr_compile_mask(L2, bad, [])
+        assert ei.value.status == B.SOAX_ERR_INVALID_ARG and msg in str(ei.value), (bad, str(ei.value))
+    with pytest.raises(B.SoaxError):
+        B.soax_expr_compile_mask(B.soax_layout_define(Cn.B6(0)), "cell(8) == 0", [])     # pos is float there: no cell()
+    with pytest.raises(B.SoaxError):
+        B.soax_expr_compile(L2, "mass = 1.0", ["not an identifier"])
+    host = inputs.make_r2(777, seed=4)
+    for seed in range(24):                                            # the first of the random conditions of the GPU parity test
+        src = condition(seed)
+        B.soax_expr_free(B.soax_expr_compile_mask(L2, src, ["a", "b", "lo"]))
+        m = oexpr.mask(host, src, {"a": 0.75, "b": -1.5, "lo": 3000.0})
+        assert m.dtype == np.uint8 and set(np.unique(m)) <= {0, 1}
