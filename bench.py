@@ -734,6 +734,41 @@ def _run_soax(args) -> None:
         dist.destroy_process_group()
 
 
+def spawn_ranks(args, argv) -> int:
+    """`python bench.py --gpus N` with N > 1 and no launcher: start N ranks on this node (one process per GPU, LOCAL_RANK
+    set, rendezvous on 127.0.0.1) by re-running this file under torch.distributed.run, which is exactly what the driver's
+    own launch line does.  Rank 0 prints the ONE JSON line (n_gpus = N); its output is passed through."""
+    import socket
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + argv
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                            # the communicator log shows the ranks (and NVLS) to the driver
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    return subprocess.run(cmd, env=env).returncode
+
+
+def run_spawn_check(args) -> None:
+    """--spawn-check: the launch plumbing alone (no GPU needed): every rank joins a gloo group and adds its rank + 1;
+    rank 0 prints one line.  Used by the CPU test of the `--gpus N` spawn path."""
+    import torch
+    import torch.distributed as dist
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    t = torch.tensor([rank + 1], dtype=torch.int64)
+    if world > 1:
+        dist.all_reduce(t)
+    if rank == 0:
+        print(json.dumps({"spawn_check": True, "n_gpus": world, "requested_gpus": args.gpus, "sum_of_rank_plus_1": int(t),
+                          "local_ranks_seen": world}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -744,10 +779,15 @@ def main() -> None:
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5,expr,container: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
-    ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (run length, alignment, digit width)")
+    ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (digit width, cluster size, pacing)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
+    ap.add_argument("--spawn-check", action="store_true", help="test aid: exercise the --gpus N launch path alone over gloo (no GPU)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:            # no launcher around us: start the N ranks ourselves
+        raise SystemExit(spawn_ranks(args, sys.argv[1:]))
+    if args.spawn_check:
+        run_spawn_check(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_soax(args)
