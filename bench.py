@@ -38,13 +38,16 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def committed_traffic():
-    """dram bytes per launch of the step kernel from the committed ncu --set full capture (profiles/), or None."""
-    path = os.path.join(ROOT, "profiles", "step_kernel_traffic.json")
+def committed_traffic(key: str = "step_soa_kernel"):
+    """(dram bytes per launch, provenance) of a kernel from the committed ncu --set full captures (profiles/kernel_traffic.json:
+    written by hand from the .ncu-rep of the commit and date it names), or (None, None)."""
+    path = os.path.join(ROOT, "profiles", "kernel_traffic.json")
     if os.path.exists(path):
         with open(path) as f:
-            return json.load(f).get("dram_bytes_per_launch")
-    return None
+            d = json.load(f).get(key)
+        if d:
+            return d.get("dram_bytes_per_launch"), {k: d.get(k) for k in ("captured_at_commit", "captured_on", "source", "n_particles")}
+    return None, None
 
 
 # ---------------------------------------------------------------------------------------------- clocks sampling
@@ -96,6 +99,40 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------------------- the CPU oracle, timed
+def cpu_info() -> dict:
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count()}
+
+
+class pinned_to_one_core:
+    """the oracle is single-threaded: pin the process to ONE core while it is timed, then restore"""
+
+    def __enter__(self):
+        self.old = None
+        try:
+            self.old = os.sched_getaffinity(0)
+            self.core = min(self.old)
+            os.sched_setaffinity(0, {self.core})
+        except (AttributeError, OSError):
+            self.core = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.old is not None:
+            try:
+                os.sched_setaffinity(0, self.old)
+            except OSError:
+                pass
+
+
 def time_oracle(host, n_sample: int, nsteps: int) -> tuple[float, float]:
     """particle-steps/s of the single-threaded oracle on the first n_sample particles; returns (rate, seconds)."""
     import numpy as np
@@ -104,12 +141,67 @@ def time_oracle(host, n_sample: int, nsteps: int) -> tuple[float, float]:
     sub = inputs.take(host, np.arange(n_sample))
     aos = oracle.pack_r1(sub)                                    # packing is outside the timed loop
     e = oracle.lib().soax_oracle_r1_energy
-    t0 = time.perf_counter()
-    e(aos.ctypes.data, aos.size, 1, 1.0, 0.5)
-    oracle.lib().soax_oracle_r1_symplectic_euler(aos.ctypes.data, aos.size, DT, 1.0, 0.5, nsteps)
-    e(aos.ctypes.data, aos.size, 1, 1.0, 0.5)
-    dt = time.perf_counter() - t0
+    with pinned_to_one_core():
+        t0 = time.perf_counter()
+        e(aos.ctypes.data, aos.size, 1, 1.0, 0.5)
+        oracle.lib().soax_oracle_r1_symplectic_euler(aos.ctypes.data, aos.size, DT, 1.0, 0.5, nsteps)
+        e(aos.ctypes.data, aos.size, 1, 1.0, 0.5)
+        dt = time.perf_counter() - t0
     return n_sample * nsteps / dt, dt
+
+
+def time_oracle_other_configs() -> dict:
+    """The oracle timed on bounded samples of configs 1, 3, 4 and 5 (SURVEY 8(d) "oracle timed beside it"): one thread,
+    pinned to one core, the timer around the step / transpose / binning calls only (generation and packing excluded).
+    The oracle's rate is size-independent beyond the last-level cache, so power-of-two samples stand for the full sizes."""
+    import numpy as np
+    import oracle
+    from paper_1710_03462_b200 import inputs
+    L = oracle.lib()
+    out = {}
+
+    def timed(fn):
+        t0 = time.perf_counter()
+        fn()
+        return time.perf_counter() - t0
+
+    with pinned_to_one_core() as pin:
+        out["affinity_core"] = pin.core
+        # config 1: the whole config (65536 particles x 10 drift steps)
+        a1 = oracle.pack_r1(inputs.make_r1(65536, seed=0))
+        t = timed(lambda: L.soax_oracle_r1_drift(a1.ctypes.data, a1.size, DT, 10))
+        out["config1_drift"] = {"sample": "the whole config: 65536 particles x 10 steps", "seconds": t, "particle_steps_per_s": 65536 * 10 / t}
+        # config 3: the oracle IS the AoS kernel (array of structs); transposes on 2^22 records
+        n3 = 1 << 22
+        h3 = inputs.make_r1(n3, seed=0)
+        a3 = oracle.r1_soa_to_aos(h3)
+        comps = [h3["id"][0]] + [h3["pos"][c] for c in range(3)] + [h3["vel"][c] for c in range(3)]
+        ptr = [c.ctypes.data for c in comps]
+        t_a2s = timed(lambda: L.soax_oracle_r1_aos_to_soa(a3.ctypes.data, n3, *ptr))
+        t_s2a = timed(lambda: L.soax_oracle_r1_soa_to_aos(a3.ctypes.data, n3, *ptr))
+        out["config3_transposes"] = {"sample": "first 2^22 of the 2^24 records", "aos_to_soa_seconds": t_a2s, "soa_to_aos_seconds": t_s2a,
+                                     "aos_to_soa_particles_per_s": n3 / t_a2s, "soa_to_aos_particles_per_s": n3 / t_s2a,
+                                     "note": "the AoS step of config 3 is the oracle's own layout: its rate is cpu_baseline.value"}
+        # config 4: masked RK2 on 2^20 wide records x 20 steps
+        n4 = 1 << 20
+        a4 = oracle.pack_r2(inputs.make_r2(n4, seed=0))
+        t = timed(lambda: L.soax_oracle_r2_rk2(a4.ctypes.data, n4, DT, 1.0, 0.5, 1, 20))
+        out["config4_rk2_masked"] = {"sample": "first 2^20 of the 2^26 particles x 20 steps", "seconds": t, "particle_steps_per_s": n4 * 20 / t}
+        # config 5: drift + cell/counts/scan/stable permutation + permutation of all fields on 2^22 particles
+        n5 = 1 << 22
+        a5 = oracle.pack_r1(inputs.make_r1(n5, seed=7))
+        b5 = np.zeros_like(a5)
+        cell, counts, offs, perm = (np.empty(m, np.uint32) for m in (n5, 64 ** 3, 64 ** 3, n5))
+
+        def cfg5():
+            L.soax_oracle_r1_drift(a5.ctypes.data, n5, DT, 1)
+            L.soax_oracle_r1_bin(a5.ctypes.data, n5, 64, cell.ctypes.data, counts.ctypes.data, offs.ctypes.data, perm.ctypes.data, None)
+            L.soax_oracle_r1_permute(a5.ctypes.data, b5.ctypes.data, n5, perm.ctypes.data)
+            L.soax_oracle_r1_energy(a5.ctypes.data, n5, 0, 1.0, 0.5)
+        t = timed(cfg5)
+        out["config5_bin_permute"] = {"sample": "first 2^22 of the 2^27 particles: drift, cell, counts, scan, stable permutation, permute, KE",
+                                      "seconds": t, "particles_per_s": n5 / t}
+    return out
 
 
 def run_reference(args) -> None:
@@ -134,7 +226,8 @@ def run_reference(args) -> None:
         "vs_baseline": None, "dtype": "f64+f32", "data": "synthetic",
         "config": {"workload": "config2: R1 SoA symplectic-Euler harmonic, N=2^24, 100 steps + energy at step 0 and 100",
                    "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, **cpu_info(),
+                         "affinity": "pinned to one core while timed"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -312,22 +405,38 @@ def _extra_config1(torch, B, Cn, ex):
 
 
 def _extra_config4(torch, B, Cn, peak, ex, gbs, iters):
-    # config 4: wide record R2, N = 2^26, 20 masked RK2 steps
+    """config 4: wide record R2, N = 2^26, 20 masked RK2 steps -- the second configuration north_star's 80 % bar names.
+    Bytes per particle-pass: byte-granular 63; sector-granular 117.5 (a thread's 4 particles are one
+    32-byte sector of every double array: a sector is touched unless all 4 are inactive, 15/16); + the read of `acc` that
+    completes partially active sectors before they are written, 14/16 x 24 = 21 -> 138.5 = the floor of a kernel that
+    writes full sectors only.  `roofline` below is the same object the headline line carries, for this kernel."""
     n4 = 1 << 26
     s4 = Cn.Soax(Cn.R2, n4)
     device_fill(torch, s4, 0)
     ms = ev_time_ms(torch, lambda: s4.step(B.SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, DT, nsteps=20, k=1.0, flag_mask=1), iters, 1) / 20
     active = int((s4.comp_view("flags") & 1).sum().item())
+    traffic, prov = committed_traffic("step_soa_kernel_rk2_r2")
     ex["config4_rk2_masked"] = {"n": n4, "ms_per_step": ms, "particle_steps_per_s": n4 / (ms * 1e-3),
                                 "active_particles": active, "active_particle_steps_per_s": active / (ms * 1e-3),
                                 "GBps_63B_byte_granular": gbs(63, n4, ms), "GBps_117p5B_sector_granular": gbs(117.5, n4, ms),
-                                "frac_of_peak_117p5B": gbs(117.5, n4, ms) / peak}
+                                "GBps_138p5B_full_sector_floor": gbs(138.5, n4, ms),
+                                "frac_of_peak_117p5B": gbs(117.5, n4, ms) / peak, "frac_of_peak_138p5B_floor": gbs(138.5, n4, ms) / peak,
+                                "roofline": {"bound": "hbm", "kernel": "step_soa_kernel<R2, RK2_MIDPOINT_HARMONIC_MASKED, 4>",
+                                             "achieved": gbs(117.5, n4, ms), "peak": peak, "unit": "GB/s", "frac": gbs(117.5, n4, ms) / peak,
+                                             "algorithmic_bytes_per_launch": 117.5 * n4, "avg_launch_ms": ms,
+                                             "traffic": traffic, "traffic_provenance": prov,
+                                             "achieved_by_dram_traffic": None if not traffic else traffic / ms / 1e6,
+                                             "frac_by_dram_traffic": None if not traffic else traffic / ms / 1e6 / peak,
+                                             "frac_of_nominal_8TBps_by_dram_traffic": None if not traffic else traffic / ms / 1e6 / 8000.0,
+                                             "frac_of_nominal_8TBps": gbs(117.5, n4, ms) / 8000.0}}
     del s4
     torch.cuda.empty_cache()
 
 
 def _extra_config5(torch, B, Cn, peak, ex, gbs, iters):
-    # config 5: N = 2^27, fused drift + cell + KE, then the stable counting sort moving all 7 arrays
+    """config 5: N = 2^27: drift + cell + KE + first histogram (src read-only), two 9-bit stable scatter passes moving all
+    7 arrays + key + carried index (the drift applied on the way), counts / offsets.  Ideal = 60 (drift) + 4 + 84 (permute
+    once) = 148 B/particle; what this pipeline must move = 40 (cell_hist) + 4 (hist) + 92 + 96 (two passes) = 232."""
     n5 = 1 << 27
     s5, d5 = Cn.Soax(Cn.R1, n5), Cn.Soax(Cn.R1, n5)
     device_fill(torch, s5, 7)
@@ -336,7 +445,10 @@ def _extra_config5(torch, B, Cn, peak, ex, gbs, iters):
     ms_d = ev_time_ms(torch, lambda: s5.step(B.SOAX_STEP_DRIFT, DT, nsteps=1), 5, 1)
     ex["config5_bin_permute"] = {"n": n5, "grid": 64, "ms_total_drift_cell_ke_sort_permute": ms, "particles_per_s": n5 / (ms * 1e-3),
                                  "drift_only_ms": ms_d, "drift_GBps_60B": gbs(60, n5, ms_d),
-                                 "GBps_ideal_148B": gbs(60 + 4 + 84, n5, ms), "scratch_GB": scratch.numel() / 1e9}
+                                 "GBps_ideal_148B": gbs(60 + 4 + 84, n5, ms), "frac_of_peak_ideal_148B": gbs(148, n5, ms) / peak,
+                                 "GBps_pipeline_232B": gbs(232, n5, ms), "frac_of_peak_pipeline_232B": gbs(232, n5, ms) / peak,
+                                 "scratch_GB": scratch.numel() / 1e9, "particle_set_GB": 40 * n5 / 1e9, "passes": 2, "digit_bits": 9,
+                                 "round1_ms": 8.47}
 
 
 def run_tour(torch, B, Cn) -> None:
@@ -402,48 +514,95 @@ def run_tour(torch, B, Cn) -> None:
 
 
 def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
-    """Design study behind the counting sort (--bin-study): one 9-bit pass (G = 8, 512 bins) over 2^27 R1 particles
-    whose cell pattern is synthetic, so that the length and the sector alignment of the runs a tile writes per bin are
-    controlled; then the digit-width sweep on the real config-5 input.  Prints one JSON line per measurement."""
+    """Design study behind the counting sort (--bin-study) on the real config-5 input at N = 2^27: digit width x cluster
+    size x cluster barrier x store pacing (soax_tune bin_bits / bin_cluster / bin_csync / bin_pace).  One JSON line per
+    measurement; every variant's permutation is checked against a stable argsort before it is timed."""
     n = 1 << log2n
     s5, d5 = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
     device_fill(torch, s5, 7)
-    e = torch.arange(n, device="cuda", dtype=torch.int64)
+    i = [(s5.comp_view("pos", c) * 64.0).to(torch.int64) for c in range(3)]
+    ref = torch.sort((i[0] * 64 + i[1]) * 64 + i[2], stable=True)[1].to(torch.int32)
+    del i
+    S = 4096                                                      # bin_pace bit 12: a CTA barrier between a thread's stores
+    rows = [(6, 1, 1, 0), (6, 1, 1, S), (6, 4, 1, S), (9, 1, 1, 0), (9, 1, 1, S), (9, 2, 1, S), (9, 4, 0, 0), (9, 4, 1, 0), (9, 4, 0, S),
+            (9, 4, 1, S), (9, 4, 1, 100), (9, 4, 1, S + 100), (9, 8, 1, S), (9, 16, 1, S), (7, 4, 1, S), (5, 1, 1, 0), (0, 0, 1, -1)]
+    for bits, cl, cs, pace in rows:
+        for key, v in (("bin_bits", bits), ("bin_cluster", cl), ("bin_csync", cs), ("bin_pace", pace)):
+            B.soax_tune(key, v)
+        scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
+        r = s5.bin_permute(d5, 64, scratch=scratch)
+        ok = bool(torch.equal(r["perm"], ref))
+        ms0 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, scratch=scratch), 5, 2)
+        ms1 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), 5, 2)
+        print(json.dumps({"study": "config 5 pipeline at 2^27", "digit_bits": bits or 9, "passes": (18 + (bits or 9) - 1) // (bits or 9),
+                          "cluster": cl or "default(4)", "cluster_barrier": cs, "pace_cta_barrier": -1 if pace < 0 else pace >> 12,
+                          "pace_sleep_ns": -1 if pace < 0 else pace & 0xfff, "ms_no_drift": round(ms0, 3), "ms_drift_ke": round(ms1, 3),
+                          "permutation_equals_stable_argsort": ok, "scratch_GB": round(scratch.numel() / 1e9, 3)}), flush=True)
+        del scratch, r
+    for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1), ("bin_pace", -1)):
+        B.soax_tune(key, v)
 
-    def set_cells(cell):                                          # G = 8: cell = (i0*8 + i1)*8 + i2, pos at the cell centre
-        for c, i in enumerate((cell // 64, (cell // 8) % 8, cell % 8)):
-            s5.comp_view("pos", c).copy_((i.double() + 0.5) / 8.0)
 
-    g = torch.Generator(device="cuda")
-    g.manual_seed(1)
-    shuffled = torch.randperm(4096, generator=g, device="cuda")[e % 4096]
-    patterns = [
-        ("uniform random positions (runs ~Poisson(8), any alignment)", None),
-        ("exactly 8 per bin and tile, runs sector-aligned", (e // 8) % 512),
-        ("exactly 8 per bin and tile, shuffled inside the tile, runs sector-aligned", (shuffled // 8) % 512),
-        ("exactly 8 per bin and tile, every run starts 1 element past a sector boundary",
-         torch.where(e < 512, e % 512, ((e - 512) // 8) % 512)),
-        ("exactly 8 per bin and tile, every run starts 4 elements past a sector boundary",
-         torch.where(e < 2048, (e // 4) % 512, ((e - 2048) // 8) % 512)),
-        ("exactly 64 per bin and tile (64 bins used), runs sector-aligned", (e // 64) % 64),
-    ]
-    scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
-    B.soax_tune("bin_bits", 9)
-    for name, cell in patterns:
-        if cell is None:
-            for c in range(3):
-                s5.comp_view("pos", c).copy_(torch.rand(n, generator=g, device="cuda", dtype=torch.float64))
-        else:
-            set_cells(cell)
-        ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 8, scratch=scratch), 5, 2)
-        print(json.dumps({"study": "one 9-bit pass, G=8 (cell + histogram + scan + scatter + counts)", "n": n, "pattern": name, "ms": round(ms, 3)}))
-    device_fill(torch, s5, 7)
-    for bits in (9, 7, 6, 5):
-        B.soax_tune("bin_bits", bits)
-        ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), 3, 1)
-        print(json.dumps({"study": "config 5 whole pipeline vs digit width", "n": n, "bin_bits": bits,
-                          "passes": (18 + bits - 1) // bits, "ms": round(ms, 3)}))
-    B.soax_tune("bin_bits", 0)
+def run_sweeps(torch, B, Cn) -> None:
+    """The launch-shape sweeps DESIGN.md section 6 cites (--sweeps), each one JSON line per point, N = 2^24 R1:
+      step      symplectic-Euler step: particles per thread x threads per CTA x persistent grid
+      xpose     AoS<->SoA transposes: records per stage (256 R) x stages x CTAs per SM
+      streams   a CONTROL for the transposes' plateau: plain copies with 1 input / 7 output streams and 7 / 1, written as
+                expression programs on a run-time layout {double a; double b[7]} (64 B/particle), against soax_copy (7 / 7)"""
+    n = 1 << LOG2N
+    s = Cn.Soax(Cn.R1, n)
+    device_fill(torch, s, 0)
+    kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
+    for ppt in (1, 2, 4):
+        for block in (128, 256, 512):
+            for persist in (0, 2, 4, 8):
+                for k, v in (("step_ppt", ppt), ("step_block", block), ("step_persist", persist)):
+                    B.soax_tune(k, v)
+                ms = ev_time_ms(torch, lambda: s.step(kind, DT, nsteps=20), 3, 1) / 20
+                print(json.dumps({"sweep": "step", "particles_per_thread": ppt, "block": block, "persistent_ctas_per_sm": persist,
+                                  "ms": round(ms, 5), "GBps_72B": round(72 * n / ms / 1e6, 1)}), flush=True)
+    for k, v in (("step_ppt", 4), ("step_block", 256), ("step_persist", 0)):
+        B.soax_tune(k, v)
+    aos = s.to_aos()
+    for r in (1, 2, 4):
+        for ns in (1, 2):
+            for ctas in (1, 2, 4, 8):
+                for k, v in (("xpose_r", r), ("xpose_ns", ns), ("xpose_ctas", ctas)):
+                    B.soax_tune(k, v)
+                try:
+                    a = ev_time_ms(torch, lambda: s.from_aos(aos, n), 10)
+                    b = ev_time_ms(torch, lambda: s.to_aos(aos), 10)
+                except Exception as e:                            # a shape that does not fit shared memory
+                    print(json.dumps({"sweep": "xpose", "records_per_stage": 256 * r, "stages": ns, "ctas_per_sm": ctas, "error": str(e)[:80]}))
+                    continue
+                print(json.dumps({"sweep": "xpose", "records_per_stage": 256 * r, "stages": ns, "ctas_per_sm": ctas,
+                                  "aos_to_soa_ms": round(a, 5), "soa_to_aos_ms": round(b, 5),
+                                  "aos_to_soa_GBps": round(80 * n / a / 1e6, 1), "soa_to_aos_GBps": round(80 * n / b / 1e6, 1)}), flush=True)
+    for k in ("xpose_r", "xpose_ns", "xpose_ctas"):
+        B.soax_tune(k, 0)
+    B.soax_tune("xpose_ring", 0)
+    a = ev_time_ms(torch, lambda: s.from_aos(aos, n), 10)
+    b = ev_time_ms(torch, lambda: s.to_aos(aos), 10)
+    print(json.dumps({"sweep": "xpose", "variant": "one tile per CTA visit (xpose_ring = 0)", "aos_to_soa_GBps": round(80 * n / a / 1e6, 1),
+                      "soa_to_aos_GBps": round(80 * n / b / 1e6, 1)}), flush=True)
+    B.soax_tune("xpose_ring", 1)
+    t = Cn.Soax(Cn.R1, n)
+    ms = ev_time_ms(torch, lambda: t.copy_from(s), 10)
+    print(json.dumps({"sweep": "streams", "copy": "soax_copy: 7 inputs -> 7 outputs (7 cudaMemcpyAsync D2D)", "ms": round(ms, 5),
+                      "GBps_80B": round(80 * n / ms / 1e6, 1)}), flush=True)
+    del t, aos
+    W = (("a", B.SOAX_F64, 1), ("b", B.SOAX_F64, 7))
+    w = Cn.Soax(W, n, dynamic=True)
+    w.slab.zero_()
+    fan_out = Cn.Program(W, "; ".join(f"b[{c}] = a" for c in range(7)), dynamic=True)
+    fan_in = Cn.Program(W, "a = " + " + ".join(f"b[{c}]" for c in range(7)), dynamic=True)
+    one = Cn.Program(W, "b[0] = a", dynamic=True)
+    for name, prog in (("1 input -> 7 outputs", fan_out), ("7 inputs -> 1 output", fan_in)):
+        ms = ev_time_ms(torch, lambda: prog.run(w, nsteps=20), 3, 1) / 20
+        print(json.dumps({"sweep": "streams", "copy": name + " (generated kernel, 8-byte elements, 256-bit accesses)", "ms": round(ms, 5),
+                          "GBps_64B": round(64 * n / ms / 1e6, 1)}), flush=True)
+    ms = ev_time_ms(torch, lambda: one.run(w, nsteps=20), 3, 1) / 20
+    print(json.dumps({"sweep": "streams", "copy": "1 input -> 1 output (generated kernel)", "ms": round(ms, 5), "GBps_16B": round(16 * n / ms / 1e6, 1)}), flush=True)
 
 
 def run_paper_replica(torch, B, Cn, max_log2n: int = 27) -> None:
@@ -550,6 +709,9 @@ def _run_soax(args) -> None:
         return
     if args.bin_study:
         run_bin_study(torch, B, Cn)
+        return
+    if args.sweeps:
+        run_sweeps(torch, B, Cn)
         return
     if args.paper_replica:
         run_paper_replica(torch, B, Cn)
@@ -711,7 +873,8 @@ def _run_soax(args) -> None:
                     "serial_value": e2e_serial, "serial_ms_per_step": float(ms2.item()) / args.steps,
                     "serial_path": "the same step with nothing overlapped: upload, compute, download, synchronise"},
             "roofline": {"bound": "hbm", "kernel": "step_soa_kernel<R1, SYMPLECTIC_EULER_HARMONIC, 4>", "achieved": achieved,
-                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": committed_traffic(),
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": committed_traffic()[0],
+                         "traffic_provenance": committed_traffic()[1],
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": STEP_BYTES * n,
                          "avg_launch_ms": kernel_ms, "frac_of_nominal_8TBps": achieved / 8000.0,
                          "kernel_share_of_step": kernel_ms * NSTEPS * args.steps / total_ms},
@@ -721,9 +884,11 @@ def _run_soax(args) -> None:
             t0 = time.perf_counter()
             n_sample = 1 << 22
             rate, secs = time_oracle(host, n_sample, NSTEPS)
-            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs,
-                                    "host_cores_available": os.cpu_count(),
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs, **cpu_info(),
+                                    "affinity": "oracle, 1 thread of %d cores, pinned to one core while timed" % (os.cpu_count() or 0),
                                     "sample": f"first 2^22 of the 2^24 particles x {NSTEPS} symplectic-Euler steps + 2 energy sums, single thread"}
+            if not args.no_extras:
+                line["cpu_baseline"]["other_configs"] = time_oracle_other_configs()
             if not args.no_extras:
                 del pin, out
                 line["extras"] = run_extras(torch, B, Cn, s, peak)
@@ -780,6 +945,7 @@ def main() -> None:
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
     ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (digit width, cluster size, pacing)")
+    ap.add_argument("--sweeps", action="store_true", help="launch-shape sweeps of the step and transpose kernels + the stream-count control")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     ap.add_argument("--spawn-check", action="store_true", help="test aid: exercise the --gpus N launch path alone over gloo (no GPU)")
     args = ap.parse_args()

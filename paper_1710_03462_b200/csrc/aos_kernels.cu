@@ -401,11 +401,12 @@ int step_aos_entry(void* aos, int64_t n, const soax_step_params* p, int variant,
 }
 
 template <class L, int R, int NS>
-static unsigned ring_grid(int64_t n) {
+static unsigned ring_grid(int64_t n, int default_ctas) {
     constexpr int by_smem = (220 * 1024) / ring_smem<L, R, NS>();
     constexpr int per_sm = by_smem < 8 ? by_smem : 8;
     const int64_t ntiles = n / (R * kTile);
-    const int64_t cap = (int64_t)kSMs * (g_tune.xpose_ctas > 0 && g_tune.xpose_ctas < per_sm ? g_tune.xpose_ctas : per_sm);
+    const int want = g_tune.xpose_ctas > 0 ? g_tune.xpose_ctas : default_ctas;
+    const int64_t cap = (int64_t)kSMs * (want < per_sm ? want : per_sm);
     return (unsigned)(ntiles < cap ? (ntiles < 1 ? 1 : ntiles) : cap);
 }
 template <class L, int R, int NS>
@@ -414,7 +415,7 @@ static int launch_a2s(void* const* comps, const void* aos, int64_t n, cudaStream
     else {
         static const bool ready = cudaFuncSetAttribute(aos_to_soa_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()) == cudaSuccess;
         if (!ready) return cuda_fail(cudaGetLastError());
-        aos_to_soa_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
+        aos_to_soa_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n, 2), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
         return launched();
     }
 }
@@ -424,18 +425,18 @@ static int launch_s2a(void* const* comps, void* aos, int64_t n, cudaStream_t st)
     else {
         static const bool ready = cudaFuncSetAttribute(soa_to_aos_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()) == cudaSuccess;
         if (!ready) return cuda_fail(cudaGetLastError());
-        soa_to_aos_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
+        soa_to_aos_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n, 4), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
         return launched();
     }
 }
-// Measured on B200: every shape plateaus at 6.0-6.1 TB/s for R1 -- an out-of-place copy with 1 + ncomp
-// streams -- so the defaults are simply the best per direction: AoS->SoA likes big bulk copies (4 x 256 records per
-// stage, one stage, several CTAs per SM), SoA->AoS likes 2 x 256 (80 bytes of loads in flight per thread for R1).
-// soax_tune("xpose_r"/"xpose_ns") override both directions for sweeps.
-#define SOAX_RING_SWITCH(FN, DEFAULT_R, ...)                                                        \
+// Measured on B200 (profiles/r2_sweeps.md, bench.py --sweeps): the shapes differ by a factor of three, and FEW resident CTAs
+// win (the ring already keeps the copies in flight; more CTAs only thrash): AoS->SoA is best with 256 records per stage,
+// two stages, two CTAs per SM (6.29 TB/s for R1); SoA->AoS with 512 records, one stage, four CTAs per SM (6.29 TB/s).
+// soax_tune("xpose_r" / "xpose_ns" / "xpose_ctas") override both directions for sweeps.
+#define SOAX_RING_SWITCH(FN, DEFAULT_R, DEFAULT_NS, ...)                                            \
     {                                                                                               \
         int r_ = g_tune.xpose_r > 0 ? g_tune.xpose_r : DEFAULT_R;                                   \
-        const int ns_ = g_tune.xpose_ns > 0 ? g_tune.xpose_ns : 1;                                  \
+        const int ns_ = g_tune.xpose_ns > 0 ? g_tune.xpose_ns : DEFAULT_NS;                         \
         while (r_ > 1 && ns_ * r_ * kTile * L::aos_stride + 64 > 110 * 1024) r_ >>= 1; /* two CTAs per SM at least */ \
         switch (r_ * 10 + ns_) {                                                                    \
             case 11: return FN<L, 1, 1>(__VA_ARGS__); case 12: return FN<L, 1, 2>(__VA_ARGS__);     \
@@ -446,14 +447,14 @@ static int launch_s2a(void* const* comps, void* aos, int64_t n, cudaStream_t st)
     }
 template <class L>
 int aos_to_soa_entry(void* const* comps, const void* aos, int64_t n, cudaStream_t st) {
-    if (g_tune.xpose_ring) SOAX_RING_SWITCH(launch_a2s, 4, comps, aos, n, st)
+    if (g_tune.xpose_ring) SOAX_RING_SWITCH(launch_a2s, 1, 2, comps, aos, n, st)
     constexpr int smem = kTile * L::aos_stride;
     aos_to_soa_kernel<L><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
     return launched();
 }
 template <class L>
 int soa_to_aos_entry(void* const* comps, void* aos, int64_t n, cudaStream_t st) {
-    if (g_tune.xpose_ring) SOAX_RING_SWITCH(launch_s2a, 2, comps, aos, n, st)
+    if (g_tune.xpose_ring) SOAX_RING_SWITCH(launch_s2a, 2, 1, comps, aos, n, st)
     constexpr int smem = kTile * L::aos_stride;
     soa_to_aos_kernel<L><<<tile_grid<L>(n, tile_ctas_per_sm<L>()), kTile, smem, st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
     return launched();
