@@ -167,6 +167,16 @@ int soax_step_aos(const soax_layout* layout, void* dev_aos, int64_t n, const soa
 int soax_aos_to_soa(soax_t* dst, const void* dev_aos, int64_t n, void* stream);
 int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream);
 
+/* NEXT-4 ("MPI transfer of particle objects"): the merge of sorted runs of packed AoS records into the component
+ * arrays of dst, written as a SEGMENTED GATHER: row j of dst (0 <= j < n) is record  dev_seg_src[i] + (j - dev_seg_dst[i])  of
+ * dev_aos, where i is the LAST of the nseg segments with dev_seg_dst[i] <= j.  dev_seg_dst must start at 0 and be
+ * non-decreasing (an empty segment repeats the next start); both tables are uint32 device arrays built by the caller from
+ * counts (paper_1710_03462_b200/dist.py builds them from the all-gathered per-cell counts, so that `world` runs that are
+ * each sorted by cell merge into one set sorted by (cell, run, position): one pass of 40 B read + 40 B written per particle
+ * instead of a transpose plus a full sort).  Source records are not range-checked.  dst's live count becomes n. */
+int soax_gather_segments_aos(soax_t* dst, const void* dev_aos, const uint32_t* dev_seg_dst, const uint32_t* dev_seg_src,
+                             int64_t nseg, int64_t n, void* stream);
+
 /* ---- a8: energy reduction in double -----------------------------------------------------------------------
  *   per particle  q = v0*v0; q = fma(v1,v1,q); q = fma(v2,v2,q)            (v_c = (double)vel_c)
  *   [+ HARMONIC:  d_c = pos_c - center; q = fma(k*d_c, d_c, q), c = 0,1,2]

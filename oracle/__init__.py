@@ -215,3 +215,19 @@ def get_elements(aos_bytes: np.ndarray, stride: int, idx: np.ndarray) -> np.ndar
     out = np.empty(i.size * stride, np.uint8)
     lib().soax_oracle_get_elements(_p(a), stride, _p(i), i.size, _p(out))
     return out
+
+
+def gather_segments(aos_bytes: np.ndarray, stride: int, seg_dst: np.ndarray, seg_src: np.ndarray, n: int) -> np.ndarray:
+    """NEXT-4, the merge of sorted runs written as a segmented gather of packed records (include/soax.h
+    soax_gather_segments_aos): output row j comes from input row seg_src[i] + (j - seg_dst[i]) where i is the LAST
+    segment with seg_dst[i] <= j.  Plain definition, one row at a time."""
+    a = np.ascontiguousarray(aos_bytes, np.uint8).reshape(-1, stride)
+    seg_dst = np.asarray(seg_dst, np.int64)
+    seg_src = np.asarray(seg_src, np.int64)
+    out = np.empty((n, stride), np.uint8)
+    i = 0
+    for j in range(n):
+        while i + 1 < seg_dst.size and seg_dst[i + 1] <= j:
+            i += 1
+        out[j] = a[seg_src[i] + (j - seg_dst[i])]
+    return out.reshape(-1)

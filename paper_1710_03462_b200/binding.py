@@ -66,6 +66,7 @@ SIGNATURES = {
     "soax_reduce_energy": (C.c_int, [_vp, _i32, _f64, _f64, _vp, _sz, _vp, _vp]),
     "soax_scratch_bytes": (_sz, [_vp, _i64, _i32]),
     "soax_bin_permute": (C.c_int, [_vp, _vp, _i32, _f64, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "soax_gather_segments_aos": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _i64, _vp]),
     "soax_remove_scratch_bytes": (_sz, [_i64]),
     "soax_remove": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _sz, C.POINTER(_i64), _vp]),
     "soax_push_back_aos": (C.c_int, [_vp, _vp, _i64, _vp]),
@@ -260,6 +261,10 @@ def soax_push_back_aos(s: int, dev_aos: int, m: int, stream: int = 0) -> None:
 
 def soax_get_elements(s: int, dev_idx: int, m: int, dev_aos: int, stream: int = 0) -> None:
     _check(lib().soax_get_elements(s, dev_idx, m, dev_aos, stream), "soax_get_elements")
+
+
+def soax_gather_segments_aos(dst: int, dev_aos: int, dev_seg_dst: int, dev_seg_src: int, nseg: int, n: int, stream: int = 0) -> None:
+    _check(lib().soax_gather_segments_aos(dst, dev_aos, dev_seg_dst, dev_seg_src, nseg, n, stream), "soax_gather_segments_aos")
 
 
 def soax_copy(dst: int, src: int, stream: int = 0) -> None:

@@ -180,6 +180,11 @@ class Soax:
         B.soax_get_elements(self.handle, idx.data_ptr(), m, aos.data_ptr(), _stream())
         return aos[:m * stride]
 
+    def from_aos_segments(self, aos: torch.Tensor, seg_dst: torch.Tensor, seg_src: torch.Tensor, n: int) -> None:
+        """merge of sorted runs of AoS records as a segmented gather (soax_gather_segments_aos); tables: int32/uint32 device"""
+        assert seg_dst.dtype in (torch.int32, torch.uint32) and seg_src.dtype == seg_dst.dtype and seg_dst.numel() == seg_src.numel()
+        B.soax_gather_segments_aos(self.handle, aos.data_ptr(), seg_dst.data_ptr(), seg_src.data_ptr(), seg_dst.numel(), n, _stream())
+
     def copy_from(self, src: "Soax") -> None:
         B.soax_copy(self.handle, src.handle, _stream())
 

@@ -460,7 +460,51 @@ int soa_to_aos_entry(void* const* comps, void* aos, int64_t n, cudaStream_t st) 
     return launched();
 }
 
+// ---- NEXT-4: merge of sorted runs as a SEGMENTED GATHER of packed records into the component arrays -------------------------
+// Output row j comes from input record seg_src[i] + (j - seg_dst[i]), i = the last segment with seg_dst[i] <= j (binary
+// search; the tables are small and stay in cache).  Consecutive rows of a segment read consecutive records, so the AoS
+// side is read in whole sectors (through L1, like the thread-per-record AoS kernel), the SoA side is written coalesced.
+template <class L>
+__global__ void __launch_bounds__(256) gather_segments_kernel(Ptrs<L::ncomp> dst, const unsigned char* __restrict__ aos,
+                                                              const uint32_t* __restrict__ seg_dst, const uint32_t* __restrict__ seg_src,
+                                                              int64_t nseg, int64_t n) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    int64_t lo = 0, hi = nseg;  // first segment with seg_dst > j
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if ((int64_t)seg_dst[mid] <= j) lo = mid + 1; else hi = mid;
+    }
+    const int64_t i = lo - 1;
+    const unsigned char* rec = aos + ((int64_t)seg_src[i] + (j - (int64_t)seg_dst[i])) * L::aos_stride;
+    constexpr int kGroup = 16;
+    constexpr int kGroups = (L::ncomp + kGroup - 1) / kGroup;
+    for_each_int<kGroups>([&](auto gi) {
+        constexpr int G0 = decltype(gi)::value * kGroup;
+        constexpr int GN = L::ncomp - G0 < kGroup ? L::ncomp - G0 : kGroup;
+        CompRegs<L, G0, 1, std::make_integer_sequence<int, GN>> v;
+        for_each_int<GN>([&](auto ci) {
+            constexpr int C = G0 + decltype(ci)::value;
+            using T = typename L::template comp_type<C>;
+            v.template get<C>()[0] = ld_piecewise<T, comp_align<L, C>()>(rec + L::aos_offset(C));
+        });
+        for_each_int<GN>([&](auto ci) {
+            constexpr int C = G0 + decltype(ci)::value;
+            comp_ptr<L, C>(dst)[j] = v.template get<C>()[0];
+        });
+    });
+}
+template <class L>
+int gather_segments_entry(void* const* comps, const void* aos, const uint32_t* seg_dst, const uint32_t* seg_src, int64_t nseg, int64_t n,
+                          cudaStream_t st) {
+    if (n == 0) return SOAX_OK;
+    gather_segments_kernel<L><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), seg_dst,
+                                                                         seg_src, nseg, n);
+    return launched();
+}
+
 #define X(L)                                                                                         \
+    template int gather_segments_entry<L>(void* const*, const void*, const uint32_t*, const uint32_t*, int64_t, int64_t, cudaStream_t); \
     template int step_aos_entry<L>(void*, int64_t, const soax_step_params*, int, cudaStream_t);      \
     template int aos_to_soa_entry<L>(void* const*, const void*, int64_t, cudaStream_t);              \
     template int soa_to_aos_entry<L>(void* const*, void*, int64_t, cudaStream_t);

@@ -30,6 +30,7 @@ struct soax_layout {
     int (*step_aos)(void*, int64_t, const soax_step_params*, int, cudaStream_t);
     int (*aos_to_soa)(void* const*, const void*, int64_t, cudaStream_t);
     int (*soa_to_aos)(void* const*, void*, int64_t, cudaStream_t);
+    int (*gather_segments)(void* const*, const void*, const uint32_t*, const uint32_t*, int64_t, int64_t, cudaStream_t);
     int (*energy)(void* const*, int64_t, int, double, double, void*, double*, cudaStream_t);
     int (*bin_permute)(const BinArgs&, cudaStream_t);
     size_t (*bin_scratch)(int64_t, int);
@@ -146,6 +147,7 @@ soax_layout describe(const char* name) {
     d.step_aos = &step_aos_entry<L>;
     d.aos_to_soa = &aos_to_soa_entry<L>;
     d.soa_to_aos = &soa_to_aos_entry<L>;
+    d.gather_segments = &gather_segments_entry<L>;
     d.energy = &energy_entry<L>;
     d.bin_permute = &bin_permute_entry<L>;
     d.bin_scratch = &bin_scratch_bytes<L>;
@@ -395,6 +397,16 @@ int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream) {
     if (!src || n < 0 || n > live(src) || (n > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
     if (!src->layout->soa_to_aos) return SOAX_ERR_UNSUPPORTED;
     return n == 0 ? SOAX_OK : src->layout->soa_to_aos(const_cast<void* const*>(src->comp), dev_aos, n, (cudaStream_t)stream);
+}
+
+int soax_gather_segments_aos(soax_t* dst, const void* dev_aos, const uint32_t* dev_seg_dst, const uint32_t* dev_seg_src, int64_t nseg,
+                             int64_t n, void* stream) {
+    if (!dst || n < 0 || nseg < 0 || n > dst->capacity || n >= ((int64_t)1 << 32)) return SOAX_ERR_INVALID_ARG;
+    if (n > 0 && (!dev_aos || !dev_seg_dst || !dev_seg_src || nseg == 0 || !aligned(dev_aos, 16) || !aligned(dev_seg_dst, 4) || !aligned(dev_seg_src, 4)))
+        return SOAX_ERR_INVALID_ARG;
+    if (!dst->layout->gather_segments) return SOAX_ERR_UNSUPPORTED;
+    set_live(dst, n);
+    return dst->layout->gather_segments(dst->comp, dev_aos, dev_seg_dst, dev_seg_src, nseg, n, (cudaStream_t)stream);
 }
 
 size_t soax_energy_scratch_bytes(void) { return kEnergyScratchBytes; }

@@ -32,6 +32,8 @@ template <class L> int step_entry(void* const* comps, int64_t n, const soax_step
 template <class L> int step_aos_entry(void* aos, int64_t n, const soax_step_params* p, int variant, cudaStream_t st);
 template <class L> int aos_to_soa_entry(void* const* comps, const void* aos, int64_t n, cudaStream_t st);
 template <class L> int soa_to_aos_entry(void* const* comps, void* aos, int64_t n, cudaStream_t st);
+template <class L> int gather_segments_entry(void* const* comps, const void* aos, const uint32_t* seg_dst, const uint32_t* seg_src, int64_t nseg,
+                                             int64_t n, cudaStream_t st);
 template <class L> int energy_entry(void* const* comps, int64_t n, int kind, double k, double ctr, void* scratch,
                                     double* out, cudaStream_t st);
 struct BinArgs {

@@ -16,8 +16,9 @@ the paper itself runs on one processor).  Three places need an exch
         3. because the local set is sorted by cell, what goes to rank r is ONE contiguous slice of every array:
            soax_soa_to_aos packs the sorted set into 40-byte records and a single all_to_all_single (NCCL over
            NVLink 5 / NVSwitch: every peer is one hop away, so the flat all-to-all is the right shape) moves them;
-        4. the received records are `world` sorted runs in rank order: soax_aos_to_soa + one more local
-           soax_bin_permute merges them.  Stability makes the result unique: within a cell, particles are ordered by
+        4. the received records are `world` sorted runs in rank order whose per-cell counts are already known (the
+           all-gather): the merge is ONE segmented gather (soax_gather_segments_aos: 40 B read + 40 B written per particle)
+           instead of a transpose plus a second full sort.  Stability makes the result unique: within a cell, particles are ordered by
            (source rank, source index), i.e. exactly the stable sort of the rank-major concatenation of all inputs.
   * per-step migration (`migrate`): after an integration step the particles whose cell left this rank's range
     [bounds[rank], bounds[rank+1]) are flagged ON THE DEVICE (a mask program, soax_expr_mask), copied out in order
@@ -143,8 +144,10 @@ class Engine(Protocol):
     def local_sort(self) -> tuple[torch.Tensor, torch.Tensor]:
         """-> (per-cell counts of this rank [ncell], the rank's particles sorted by cell as packed records [n*stride] uint8)"""
 
-    def merge(self, records: torch.Tensor, n: int) -> object:
-        """records: n packed records (sorted runs in rank order) -> the final local container, stably sorted by cell"""
+    def merge(self, records: torch.Tensor, n: int, run_counts: torch.Tensor, lo: int) -> object:
+        """records: n packed records = `world` runs in rank order, each sorted by cell; run_counts [world, hi - lo]: the
+        number of records of every cell of this rank's range [lo, hi) in every run -> the final local container, stably
+        sorted by cell"""
 
 
 class SoaxEngine:
@@ -165,12 +168,22 @@ class SoaxEngine:
         self.kinetic = r["kinetic"]
         return r["counts"].to(torch.int64), tmp.to_aos()
 
-    def merge(self, records: torch.Tensor, n: int):
-        tmp = self._Cn.Soax(self.src.fields, 0, capacity=max(n, 1))
-        tmp.from_aos(records, n)
+    def merge(self, records: torch.Tensor, n: int, run_counts: torch.Tensor, lo: int):
+        """The runs are sorted and their per-cell counts are known, so the merge is ONE segmented gather (80 B/particle):
+        segment (cell c, run q) goes to [sum of the counts before it in (cell, run) order) and comes from run q's slice
+        of cell c.  The two tables are built from counts with torch (plumbing); the records move in libsoax.so."""
+        cnt = run_counts.to(records.device)                          # [world, m]
+        run_start = torch.cumsum(cnt.sum(1), 0) - cnt.sum(1)
+        src_start = run_start[:, None] + torch.cumsum(cnt, 1) - cnt
+        flat = cnt.t().reshape(-1)
+        seg_dst = (torch.cumsum(flat, 0) - flat).to(torch.int32)
+        seg_src = src_start.t().reshape(-1).to(torch.int32)
         out = self._Cn.Soax(self.src.fields, 0, capacity=max(n, 1))
-        r = tmp.bin_permute(out, self.grid_dim)
-        return out, r["counts"], r["offsets"]
+        out.from_aos_segments(records, seg_dst, seg_src, n)
+        counts = torch.zeros(self.ncell, dtype=torch.int64, device=records.device)
+        counts[lo:lo + cnt.shape[1]] = cnt.sum(0)
+        offsets = torch.cumsum(counts, 0) - counts
+        return out, counts.to(torch.int32), offsets.to(torch.int32)
 
     # ---- migration (every device step is a libsoax.so call) ----------------------------------------------------------------
     def _mask(self, cond: str):
@@ -212,9 +225,11 @@ def _ship(engine: Engine, counts: torch.Tensor, records: torch.Tensor, group, bo
 def bin_exchange(engine: Engine, group=None):
     """One binning step across the group (see the module docstring).  Returns (engine.merge(...) result, bounds, n_local):
     this rank then owns the cells [bounds[rank], bounds[rank+1]).  One host round trip (the split sizes)."""
+    rank = dist.get_rank(group)
     counts, records = engine.local_sort()
-    recv, n_recv, bounds, _ = _ship(engine, counts, records, group, None)
-    return engine.merge(recv, sum(n_recv)), bounds, sum(n_recv)
+    recv, n_recv, bounds, all_counts = _ship(engine, counts, records, group, None)
+    lo, hi = bounds[rank], bounds[rank + 1]
+    return engine.merge(recv, sum(n_recv), all_counts[:, lo:hi], lo), bounds, sum(n_recv)
 
 
 def migrate(engine: SoaxEngine, s, bounds: Sequence[int], group=None) -> int:

@@ -65,3 +65,24 @@ def test_get_elements_is_row_indexing():
     idx = np.array([3, 3, 49, 0, 17], np.uint32)
     assert np.array_equal(oracle.get_elements(a.reshape(-1), 24, idx).reshape(-1, 24), a[idx])
     assert oracle.get_elements(a.reshape(-1), 24, np.zeros(0, np.uint32)).size == 0
+
+
+def test_gather_segments_is_the_merge_of_sorted_runs():
+    """oracle.gather_segments pinned by hand and by what it is for: with the tables built from per-run per-cell counts it
+    reproduces the stable sort (by cell) of the concatenation of runs that are each sorted by cell."""
+    rows = np.arange(10 * 3, dtype=np.uint8).reshape(10, 3)          # 10 records of 3 bytes: record r = (3r, 3r+1, 3r+2)
+    out = oracle.gather_segments(rows.reshape(-1), 3, [0, 2, 2, 5], [7, 0, 4, 1], 6).reshape(-1, 3)
+    assert out[:, 0].tolist() == [21, 24, 12, 15, 18, 3]             # rows 7,8 | (empty) | 4,5,6 | 1
+    rng = np.random.default_rng(0)
+    world, ncell = 3, 17
+    runs = [np.sort(rng.integers(0, ncell, rng.integers(0, 60))) for _ in range(world)]       # each run sorted by cell
+    cells = np.concatenate(runs)
+    recs = np.stack([cells.astype(np.uint8), np.arange(cells.size, dtype=np.uint8)], axis=1)   # (cell, position in the concatenation)
+    cnt = np.stack([np.bincount(r, minlength=ncell) for r in runs])                          # [world, ncell]
+    run_start = np.concatenate([[0], np.cumsum([r.size for r in runs])[:-1]])
+    src_start = run_start[:, None] + np.cumsum(cnt, axis=1) - cnt                             # first record of (run q, cell c)
+    flat = cnt.T.reshape(-1)                                                                 # (cell, run) order = destination order
+    seg_dst = np.cumsum(flat) - flat
+    got = oracle.gather_segments(recs.reshape(-1), 2, seg_dst, src_start.T.reshape(-1), cells.size).reshape(-1, 2)
+    order = np.argsort(cells, kind="stable")
+    assert np.array_equal(got, recs[order])

@@ -90,8 +90,9 @@ class OracleEngine:                                                # stands in f
         b, srt = sort_by_cell(self.host)
         return torch.from_numpy(b["counts"].astype(np.int64)), torch.from_numpy(oracle.r1_soa_to_aos(srt))
 
-    def merge(self, records, n):
+    def merge(self, records, n, run_counts, lo):
         b, srt = sort_by_cell(oracle.r1_aos_to_soa(records[:n * 40].numpy()))
+        assert np.array_equal(run_counts.sum(0).numpy(), b["counts"][lo:lo + run_counts.shape[1]])
         return srt, b["counts"]
 
     def take_leavers(self, s, lo, hi):

@@ -182,3 +182,32 @@ def test_get_elements_out_of_range_rows_are_zero_records(gpu):
     base = oracle.r1_soa_to_aos(host).reshape(-1, 40)
     for j, i in enumerate(idx):
         assert np.array_equal(got[j], base[i] if i < n else np.zeros(40, np.uint8)), (j, i)
+
+
+@pytest.mark.parametrize("world,n_each", [(3, 4001), (8, 700), (1, 5000), (2, 0)])
+def test_gather_segments_merges_sorted_runs(gpu, world, n_each):
+    """soax_gather_segments_aos against oracle.gather_segments, on the tables of a `world`-run merge by cell (G = 8)."""
+    torch, B, Cn = gpu
+    G = 8
+    rng = np.random.default_rng(world)
+    runs, cnts = [], []
+    for q in range(world):
+        h = inputs.make_r1(n_each + 13 * q if n_each else 0, seed=20 + q)
+        b = oracle.bin_r1(h, G)
+        runs.append(oracle.r1_soa_to_aos(oracle.permute_r1(h, b["perm"])))
+        cnts.append(b["counts"].astype(np.int64))
+    recs = np.concatenate(runs) if runs else np.zeros(0, np.uint8)
+    n = recs.size // 40
+    cnt = np.stack(cnts)
+    sizes = cnt.sum(1)
+    src_start = (np.cumsum(sizes) - sizes)[:, None] + np.cumsum(cnt, 1) - cnt
+    flat = cnt.T.reshape(-1)
+    seg_dst, seg_src = (np.cumsum(flat) - flat).astype(np.int32), src_start.T.reshape(-1).astype(np.int32)
+    want = oracle.gather_segments(recs, 40, seg_dst, seg_src, n)
+    d = Cn.Soax(Cn.R1, 0, capacity=max(n, 1))
+    d.from_aos_segments(torch.from_numpy(np.concatenate([recs, np.zeros(16, np.uint8)])).cuda(), torch.from_numpy(seg_dst).cuda(),
+                        torch.from_numpy(seg_src).cuda(), n)
+    assert d.n == n and np.array_equal(image(d), want)
+    if n:                                                             # and it IS the stable sort by cell of the concatenation
+        whole = oracle.r1_aos_to_soa(recs)
+        assert np.array_equal(want, oracle.r1_soa_to_aos(oracle.permute_r1(whole, oracle.bin_r1(whole, G)["perm"])))
