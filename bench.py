@@ -268,7 +268,7 @@ def device_fill(torch, s, seed: int) -> None:
         s.comp_view("flags").copy_(torch.randint(0, 256, (n,), generator=g, device="cuda", dtype=torch.uint8))
 
 
-def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5", "expr", "container"), iters: int = 3) -> dict:
+def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config1", "config4", "config5", "expr", "container", "exchange"), iters: int = 3) -> dict:
     """The other section-8(a) rows, each timed alone with CUDA events (N=1, rank 0): reported beside the headline."""
     ex = {}
     n = s.n
@@ -287,7 +287,78 @@ def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config
         _extra_expr(torch, B, Cn, s, peak, ex, gbs)
     if "container" in which:
         _extra_container(torch, B, Cn, s, peak, ex, gbs)
+    if "exchange" in which:
+        _extra_exchange(torch, B, Cn, s, peak, ex, gbs)
     return ex
+
+
+def _extra_exchange(torch, B, Cn, s, peak, ex, gbs):
+    """NEXT-4 on ONE GPU: the device-side pieces of the cross-GPU exchange, timed alone (no multi-GPU number exists).
+    (1) The merge of 8 received runs (2^24 R1 records in all, each run sorted by cell on a 64^3 grid): one segmented gather
+    (soax_gather_segments_aos, 80 B/particle) against what round 1 did (soax_aos_to_soa + a second soax_bin_permute).
+    (2) One migration step's local work at ~1 % leavers: two mask programs, the stable copy-out of the leavers, the
+    overwrite-with-last removal, and the sort of the leavers."""
+    n, G, world = s.n, 64, 8
+    sizes = [n // world] * world
+    runs, cnts = [], []
+    for q in range(world):
+        part = Cn.Soax(Cn.R1, sizes[q])
+        for name, dt, dim in Cn.R1:
+            for c in range(dim):
+                part.comp_view(name, c).copy_(s.comp_view(name, c)[q * sizes[q]:(q + 1) * sizes[q]])
+        srt = Cn.Soax(Cn.R1, sizes[q])
+        r = part.bin_permute(srt, G)
+        runs.append(srt.to_aos())
+        cnts.append(r["counts"].to(torch.int64))
+        del part, srt, r
+    recs = torch.cat(runs)
+    del runs
+    cnt = torch.stack(cnts)
+    run_start = torch.cumsum(cnt.sum(1), 0) - cnt.sum(1)
+    src_start = run_start[:, None] + torch.cumsum(cnt, 1) - cnt
+    flat = cnt.t().reshape(-1)
+    seg_dst, seg_src = (torch.cumsum(flat, 0) - flat).to(torch.int32), src_start.t().reshape(-1).to(torch.int32)
+    out, tmp = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
+    scratch = torch.empty(B.soax_scratch_bytes(out.layout, n, G), dtype=torch.uint8, device="cuda")
+    ms_new = ev_time_ms(torch, lambda: out.from_aos_segments(recs, seg_dst, seg_src, n), 10)
+
+    def old():
+        tmp.from_aos(recs, n)
+        tmp.bin_permute(out, G, scratch=scratch)
+    ms_old = ev_time_ms(torch, old, 5)
+    ref = Cn.Soax(Cn.R1, n)
+    old()
+    ref.copy_from(out)
+    out.from_aos_segments(recs, seg_dst, seg_src, n)
+    same = all(torch.equal(out.comp_view(name, c), ref.comp_view(name, c)) for name, dt, dim in Cn.R1 for c in range(dim))
+    del tmp, ref, scratch, recs
+    # (2) migration, local part: this GPU owns cells [lo, hi) = the middle 98 % of the cell range after a drift
+    lo, hi = int(0.01 * G ** 3), int(0.99 * G ** 3)
+    cond_leave = f"(double(cell({G})) < lo) | (double(cell({G})) >= hi)"
+    cond_stay = f"(double(cell({G})) >= lo) & (double(cell({G})) < hi)"
+    leave, stay = Cn.MaskProgram(Cn.R1, cond_leave, ["lo", "hi"]), Cn.MaskProgram(Cn.R1, cond_stay, ["lo", "hi"])
+    work, gone = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, 0, capacity=n)
+    m1, m2 = torch.empty(n, dtype=torch.uint8, device="cuda"), torch.empty(n, dtype=torch.uint8, device="cuda")
+    rs = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
+    rs2 = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
+
+    work.copy_from(s)
+    ms_masks = ev_time_ms(torch, lambda: (leave.mask(work, out=m1, lo=lo, hi=hi), stay.mask(work, out=m2, lo=lo, hi=hi)), 10)
+    ms_out = ev_time_ms(torch, lambda: work.remove_async(m2, stable=True, dst=gone, scratch=rs), 10)
+    n_gone = gone.n
+    ms_copy = ev_time_ms(torch, lambda: work.copy_from(s), 10)
+
+    def refresh_and_remove():                                   # the in-place removal changes `work`: every run starts from a fresh copy
+        work.copy_from(s)
+        work.remove_async(m1, scratch=rs2)
+    ms_swap = ev_time_ms(torch, refresh_and_remove, 10) - ms_copy
+    ms_mig = ms_masks + ms_out + ms_swap
+    ex["next4_exchange_local_work"] = {
+        "n": n, "runs": world, "merge_segmented_gather_ms": ms_new, "merge_segmented_gather_GBps_80B": gbs(80, n, ms_new),
+        "merge_round1_transpose_plus_sort_ms": ms_old, "merge_speedup": ms_old / ms_new, "merge_results_identical": bool(same),
+        "migration_local_ms": ms_mig, "migration_masks_ms": ms_masks, "migration_copy_out_leavers_ms": ms_out,
+        "migration_overwrite_with_last_ms": ms_swap, "migration_leavers": n_gone, "migration_particles_per_s": n / (ms_mig * 1e-3),
+        "note": "device-side pieces of the multi-GPU exchange on one GPU; the collectives themselves are unmeasured on hardware"}
 
 
 def _extra_container(torch, B, Cn, s, peak, ex, gbs):
@@ -472,6 +543,15 @@ def run_tour(torch, B, Cn) -> None:
     idx = torch.randint(0, n, (1 << 20,), device="cuda", dtype=torch.int32)
     s.get_elements(idx)                                                        # NEXT-3: bulk getElement
     del d
+    mask = Cn.MaskProgram(Cn.R1, "(double(cell(64)) < lo) | (double(cell(64)) >= hi)", ["lo", "hi"])
+    for _ in range(2):
+        mask.mask(s, lo=2621.0, hi=259522.0)                                   # NEXT-3/4: the kill mask written on the device
+    seg = torch.tensor([0, n // 2], dtype=torch.int32, device="cuda")
+    g = Cn.Soax(Cn.R1, n)
+    tmp_aos = s.to_aos()
+    for _ in range(2):
+        g.from_aos_segments(tmp_aos, seg, torch.tensor([n // 2, 0], dtype=torch.int32, device="cuda"), n)   # NEXT-4: merge of runs
+    del g, tmp_aos
     aos = s.to_aos()
     for _ in range(2):
         s.to_aos(aos)                                                          # a7  (config 3)
