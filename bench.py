@@ -605,7 +605,7 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
     del i
     S = 4096                                                      # bin_pace bit 12: a CTA barrier between a thread's stores
     rows = [(6, 1, 1, 0), (6, 1, 1, S), (6, 4, 1, S), (9, 1, 1, 0), (9, 1, 1, S), (9, 2, 1, S), (9, 4, 0, 0), (9, 4, 1, 0), (9, 4, 0, S),
-            (9, 4, 1, S), (9, 4, 1, 100), (9, 4, 1, S + 100), (9, 8, 1, S), (9, 16, 1, S), (7, 4, 1, S), (5, 1, 1, 0), (0, 0, 1, -1)]
+            (9, 4, 1, S), (9, 4, 1, 2 * S), (9, 4, 1, 100), (9, 4, 1, S + 100), (9, 8, 1, S), (9, 16, 1, S), (7, 4, 1, S), (5, 1, 1, 0), (0, 0, 1, -1)]
     for bits, cl, cs, pace in rows:
         for key, v in (("bin_bits", bits), ("bin_cluster", cl), ("bin_csync", cs), ("bin_pace", pace)):
             B.soax_tune(key, v)
@@ -615,8 +615,8 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
         ms0 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, scratch=scratch), 5, 2)
         ms1 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), 5, 2)
         print(json.dumps({"study": "config 5 pipeline at 2^27", "digit_bits": bits or 9, "passes": (18 + (bits or 9) - 1) // (bits or 9),
-                          "cluster": cl or "default(4)", "cluster_barrier": cs, "pace_cta_barrier": -1 if pace < 0 else pace >> 12,
-                          "pace_sleep_ns": -1 if pace < 0 else pace & 0xfff, "ms_no_drift": round(ms0, 3), "ms_drift_ke": round(ms1, 3),
+                          "cluster": cl or "default(4)", "cluster_barrier": cs, "pace_barrier": "default(cluster)" if pace < 0 else ("none", "cta", "cluster")[pace >> 12],
+                          "pace_sleep_ns": 0 if pace < 0 else pace & 0xfff, "ms_no_drift": round(ms0, 3), "ms_drift_ke": round(ms1, 3),
                           "permutation_equals_stable_argsort": ok, "scratch_GB": round(scratch.numel() / 1e9, 3)}), flush=True)
         del scratch, r
     for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1), ("bin_pace", -1)):

@@ -254,10 +254,13 @@ __device__ __forceinline__ void cluster_sync_relaxed() {
 
 // Pacing of the scatter stores (measured, profiles/r2_bin_study.md): a thread has kItems stores per array; issued back to
 // back they reach the L2 out of step with the stores of the neighbouring CTAs that complete the same sectors.  Between
-// two stores of a thread the CTA therefore optionally meets at a barrier and/or sleeps a few tens of nanoseconds.
+// two stores of a thread the CTA (pace_sync 1) or the whole cluster (2, the default with clusters) therefore meets at a
+// barrier, so that at any moment the cluster writes ONE window of ~64 neighbouring bins; a sleep of a few tens of
+// nanoseconds can be added for studies.
 __device__ __forceinline__ void pace(int k, int pace_sync, int pace_ns) {
     if (k == 0) return;
-    if (pace_sync) __syncthreads();
+    if (pace_sync == 1) __syncthreads();
+    if (pace_sync == 2) cluster_sync_relaxed();
     if (pace_ns) __nanosleep(pace_ns);
 }
 
@@ -400,13 +403,17 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
     __syncthreads();     // inv complete, counters dead: stage 1 joins the ring
     fill_load(std::integral_constant<int, 1>{});
 
-    // ---- output slots: thread t owns slots t, t + 512, ... of the tile-sorted order --------------------------------
+    // ---- output slots: thread t owns slots t, t + 512, ... of the tile-sorted order, so that in its k-th store the whole CTA
+    // (and, in step with it, the other CTAs of the cluster) writes ONE window of 512 consecutive slots = the runs of ~64
+    // neighbouring bins.  Few runs open at a time is what lets the L2 merge their pieces: giving every warp its own 256
+    // consecutive slots instead (16 windows open per CTA) was measured 25 % slower (profiles/r2_bin_study.md).
+#define SLOT(k) (tid + (k) * kSortThreads)
     uint32_t gdest[kItems], srcp[kItems / 2];  // source elements packed two per register
     {
         uint32_t kv[kItems];
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
-            const int j = tid + k * kSortThreads;
+            const int j = SLOT(k);
             uint32_t s = 0;
             kv[k] = 0;
             gdest[k] = 0;
@@ -422,7 +429,7 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
 #pragma unroll
             for (int k = 0; k < kItems; ++k) {
                 pace(k, g.pace_sync, g.pace_ns);
-                if (tid + k * kSortThreads < cnt) g.key_out[gdest[k]] = kv[k];
+                if (SLOT(k) < cnt) g.key_out[gdest[k]] = kv[k];
             }
         }
         if constexpr (!HAS_IDX) {
@@ -431,7 +438,7 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
 #pragma unroll
                 for (int k = 0; k < kItems; ++k) {
                     pace(k, g.pace_sync, g.pace_ns);
-                    if (tid + k * kSortThreads < cnt) g.idx_out[gdest[k]] = (uint32_t)(tile0 + ((srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu));
+                    if (SLOT(k) < cnt) g.idx_out[gdest[k]] = (uint32_t)(tile0 + ((srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu));
                 }
             }
         }
@@ -458,13 +465,13 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
 #pragma unroll
                 for (int k = 0; k < kItems; ++k) {
                     const uint32_t s = (srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
-                    if (tid + k * kSortThreads < cnt) v[k] = drift1<V>(g.dt, vb[s], sb[s]);
+                    if (SLOT(k) < cnt) v[k] = drift1<V>(g.dt, vb[s], sb[s]);
                 }
             } else {
 #pragma unroll
                 for (int k = 0; k < kItems; ++k) {
                     const uint32_t s = (srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
-                    if (tid + k * kSortThreads < cnt) v[k] = sb[s];
+                    if (SLOT(k) < cnt) v[k] = sb[s];
                 }
             }
             if (g.csync) cluster_sync_relaxed();
@@ -474,7 +481,7 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
 #pragma unroll
             for (int k = 0; k < kItems; ++k) {
                 pace(k, g.pace_sync, g.pace_ns);
-                if (tid + k * kSortThreads < cnt) gout[gdest[k]] = v[k];
+                if (SLOT(k) < cnt) gout[gdest[k]] = v[k];
             }
             __syncthreads();  // the stage can take the next load
             fill_load(std::integral_constant<int, m + kRingStages>{});
@@ -483,6 +490,7 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
         else body(comp_ptr<L, (a >= kFirstComp ? a - kFirstComp : 0)>(src), comp_ptr<L, (a >= kFirstComp ? a - kFirstComp : 0)>(dst));
     };
     for_each_int<kArrays - 1>([&](auto i) { move(std::integral_constant<int, decltype(i)::value + 1>{}); });
+#undef SLOT
 }
 
 // ---- counts / offsets from the sorted keys: off[c] = first sorted slot whose key is >= c (binary search) -------------
@@ -655,7 +663,8 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
             const int want_cluster = g_tune.bin_cluster > 0 ? g_tune.bin_cluster : 4;
             const int cluster = (g_tune.bin_cluster > 0 || w >= 8) ? want_cluster : 1;
             g.csync = cluster > 1 && g_tune.bin_csync != 0;
-            g.pace_sync = g_tune.bin_pace >= 0 ? (g_tune.bin_pace >> 12) & 1 : (cluster > 1);
+            g.pace_sync = g_tune.bin_pace >= 0 ? (g_tune.bin_pace >> 12) & 3 : (cluster > 1 ? 2 : 0);
+            if (g.pace_sync == 2 && cluster == 1) g.pace_sync = 1;
             g.pace_ns = g_tune.bin_pace >= 0 ? g_tune.bin_pace & 0xfff : 0;
             if (pass == 0) {
                 if constexpr (has_vel) {
