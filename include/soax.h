@@ -195,9 +195,12 @@ int soax_reduce_energy(const soax_t* s, int32_t kind, double k, double center, v
  * The permutation is unique and the result is deterministic for any particle distribution.
  * grid_dim G: power of two, 1 <= G <= 64 (G^3 <= 2^18 cells).  src is read only; dst: same layout,
  * capacity >= n, must not alias src; its live count becomes n.  dev_counts, dev_offsets: G^3 uint32 each;
- * dev_perm: n uint32; any of the three may be NULL.  dev_scratch: >= soax_scratch_bytes(layout, n, G) bytes,
- * 256-byte aligned.  Optional fusions (one call = config 5's whole pipeline): if drift_dt != 0 a DRIFT step
- * with that dt is applied to src IN PLACE first, inside the same pass that computes the cell indices; if
+ * dev_perm: n uint32; any of the three may be NULL (a NULL dev_perm means no source index is carried through the passes;
+ * NULL counts and offsets mean the sorted keys are not written).  dev_scratch: >= soax_scratch_bytes(layout, n, G) bytes,
+ * 256-byte aligned.  Optional fusions (one call = config 5's whole pipeline): if drift_dt != 0 the particles are
+ * DRIFTED by that dt on their way to dst -- dst = the drifted particles in cell order, binned by their drifted positions;
+ * src is READ ONLY and keeps the pre-drift state (the drift is computed once for the keys and once more, with the same
+ * fma, while the position arrays move: no pass over memory exists only to write positions back; Q22); if
  * dev_kinetic != NULL it receives sum_i 0.5*|vel_i|^2 as in soax_reduce_energy(KINETIC).
  * Errors: INVALID_ARG, UNSUPPORTED (no pos[3] double field, n >= 2^32), ALLOC (scratch too small), CUDA.
  * Positions outside [0,1) are a precondition violation: their cell index is clamped into the grid. */
@@ -315,8 +318,11 @@ int soax_last_cuda_error(void);
 /* Number of kernels this library has launched since load (or since the last soax_reset_launch_count). */
 int64_t soax_launch_count(void);
 void soax_reset_launch_count(void);
-/* Launch-shape knobs for benchmarking sweeps ("step_ppt", "step_block", "step_persist", ...); unknown keys
- * return INVALID_ARG.  Not needed for normal use: defaults are the measured best. */
+/* Launch-shape knobs for benchmarking sweeps ("step_ppt", "step_block", "step_persist", "xpose_*", "bin_bits", "bin_cluster",
+ * "bin_csync", "bin_pace", ...); unknown keys return INVALID_ARG.  Not needed for normal use: defaults are the measured
+ * best.  The knobs are process-global and NOT thread-safe: set them before the first call that launches work and do not
+ * change them while another thread is inside the library (captured step graphs are keyed on the knobs and re-captured
+ * when they change; soax_scratch_bytes follows "bin_bits", so query it after setting that knob). */
 int soax_tune(const char* key, int64_t value);
 
 #if defined(__GNUC__)

@@ -33,9 +33,24 @@ def _deps_mtime() -> float:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Returns the path of an up-to-date libsoax.so, compiling it if needed.  Safe under several processes at once (ranks
+    of one torchrun importing the binding together): the check-and-compile runs under an exclusive file lock, so one
+    process compiles and the others wait and then find the library fresh; the link goes to a temporary name + os.replace."""
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps_mtime():
         return LIB
+    import fcntl
     os.makedirs(OBJ, exist_ok=True)
+    with open(os.path.join(OBJ, ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps_mtime():
+                return LIB                                        # another process built it while we waited
+            return _build_locked(verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose: bool) -> str:
     nvcc = _nvcc()
 
     def compile_one(src: str) -> str:

@@ -413,8 +413,7 @@ template <class L, int R, int NS>
 static int launch_a2s(void* const* comps, const void* aos, int64_t n, cudaStream_t st) {
     if constexpr (ring_smem<L, R, NS>() > 220 * 1024) return SOAX_ERR_UNSUPPORTED;
     else {
-        static const bool ready = cudaFuncSetAttribute(aos_to_soa_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()) == cudaSuccess;
-        if (!ready) return cuda_fail(cudaGetLastError());
+        SOAX_CUDA(cudaFuncSetAttribute(aos_to_soa_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()));  // per device, cheap: set on every call
         aos_to_soa_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n, 2), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<const unsigned char*>(aos), n);
         return launched();
     }
@@ -423,8 +422,7 @@ template <class L, int R, int NS>
 static int launch_s2a(void* const* comps, void* aos, int64_t n, cudaStream_t st) {
     if constexpr (ring_smem<L, R, NS>() > 220 * 1024) return SOAX_ERR_UNSUPPORTED;
     else {
-        static const bool ready = cudaFuncSetAttribute(soa_to_aos_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()) == cudaSuccess;
-        if (!ready) return cuda_fail(cudaGetLastError());
+        SOAX_CUDA(cudaFuncSetAttribute(soa_to_aos_ring_kernel<L, R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, ring_smem<L, R, NS>()));  // per device, cheap: set on every call
         soa_to_aos_ring_kernel<L, R, NS><<<ring_grid<L, R, NS>(n, 4), kTile, ring_smem<L, R, NS>(), st>>>(make_ptrs<L>(comps), static_cast<unsigned char*>(aos), n);
         return launched();
     }
