@@ -637,6 +637,7 @@ int soax_tune(const char* key, int64_t value) {
     else if (!std::strcmp(key, "xpose_ctas")) { if (v < 0 || v > 8) return SOAX_ERR_INVALID_ARG; g_tune.xpose_ctas = v; }
     else if (!std::strcmp(key, "bin_bits")) { if (v < 0 || v > 9) return SOAX_ERR_INVALID_ARG; g_tune.bin_bits = v; }
     else if (!std::strcmp(key, "bin_cluster")) { if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8 && v != 16) return SOAX_ERR_INVALID_ARG; g_tune.bin_cluster = v; }
+    else if (!std::strcmp(key, "bin_pace_every")) { if (v < 0 || v > 8) return SOAX_ERR_INVALID_ARG; g_tune.bin_pace_every = v; }
     else if (!std::strcmp(key, "bin_pace")) { if (v < -1 || v > 16383) return SOAX_ERR_INVALID_ARG; g_tune.bin_pace = v; }
     else if (!std::strcmp(key, "bin_csync")) { if (v < 0 || v > 1) return SOAX_ERR_INVALID_ARG; g_tune.bin_csync = v; }
     else return SOAX_ERR_INVALID_ARG;

@@ -7,13 +7,15 @@
 // of the field arrays is ever made (a per-array gather would read one 32-byte sector per 4- or 8-byte item).
 //   cell_hist   [drift +] cell index [+ kinetic energy] and the first digit's per-tile histogram     36 B read, 4 B written
 //   colscan_*   exclusive scan of the [tile][digit] table in digit-major order                      (small)
-//   scatter     every array of the tile (keys, carried indices, each component array) arrives in shared memory as ONE
-//               bulk asynchronous copy (TMA) into a 3-stage ring; stable in-tile ranks come from warp ballots and
-//               per-warp running counters; output slot j reads ring[inv[j]] and writes its global slot, consecutive
-//               threads writing consecutive slots of a bin's run.  The first pass applies the requested DRIFT to the
-//               positions on their way through the ring (src is never written).
+//   scatter     every UNIT of the tile (the key + carried index, each 8-byte component, each PAIR of 4-byte components)
+//               arrives in shared memory by bulk asynchronous copy (TMA) into a 3-stage ring; stable in-tile ranks come
+//               from warp ballots and per-warp running counters; output slot j reads ring[inv[j]] and writes its global
+//               slot, consecutive threads writing consecutive slots of a bin's run.  Between the passes the records live
+//               in a PAIRED scratch format (4-byte arrays two by two as 8-byte elements: 6 streams instead of 9 for R1);
+//               the first pass reads the caller's SoA and applies the requested DRIFT to the positions on their way
+//               through the ring (src is never written), the last pass writes the caller's SoA.
 //   tile_hist   per-tile histogram of the next digit (later passes)                                  4 B read
-//   cell_bounds counts / offsets from the sorted keys by binary search per cell                      (small)
+//   cell_bounds counts / offsets from the sorted positions by binary search per cell                 (small)
 // A 512-bin pass leaves runs of only ~8 elements per tile and bin, whose ragged ends are partial 32-byte sectors; the
 // L2 turns a partial-sector write into a DRAM read-modify-write unless the rest of the sector arrives within about a
 // microsecond (measured, profiles/r2_bin_study.md).  Wide-digit passes are therefore launched in THREAD-BLOCK CLUSTERS
@@ -106,27 +108,36 @@ __global__ void __launch_bounds__(kCellThreads) cell_hist_kernel(Ptrs<L::ncomp> 
 }
 
 // ---- per-tile digit histogram (passes after the first) -----------------------------------------------------------
-__global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t* __restrict__ keys, int64_t n, int shift, uint32_t mask,
+// `stride` = 1: plain keys; 2: the (key, index) pairs of the paired format (the key is the first word of each pair).
+__global__ void __launch_bounds__(kSortThreads) tile_hist_kernel(const uint32_t* __restrict__ keys, int stride, int64_t n, int shift, uint32_t mask,
                                                                  uint32_t* __restrict__ hist) {
     __shared__ uint32_t h[kRadix];
-    if (threadIdx.x < kRadix) h[threadIdx.x] = 0;
+    for (int i = threadIdx.x; i < kRadix; i += kSortThreads) h[i] = 0;
     __syncthreads();
     const int64_t tile0 = (int64_t)blockIdx.x * kTileN;
-    if (tile0 + kTileN <= n) {  // full tile: two 128-bit loads per thread (the histogram does not care about order)
+    if (tile0 + kTileN <= n && stride == 1) {  // full tile: two 128-bit loads per thread (the histogram does not care about order)
         const uint4* k4 = reinterpret_cast<const uint4*>(keys + tile0);
         const uint4 a = k4[threadIdx.x], b = k4[threadIdx.x + kSortThreads];
         const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
 #pragma unroll
         for (int k = 0; k < 8; ++k) atomicAdd(&h[(w[k] >> shift) & mask], 1u);
+    } else if (tile0 + kTileN <= n) {  // full tile of pairs: four 128-bit loads per thread, the keys are words 0 and 2
+        const uint4* k4 = reinterpret_cast<const uint4*>(keys + 2 * tile0);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint4 a = k4[threadIdx.x + q * kSortThreads];
+            atomicAdd(&h[(a.x >> shift) & mask], 1u);
+            atomicAdd(&h[(a.z >> shift) & mask], 1u);
+        }
     } else {
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             const int64_t e = tile0 + k * kSortThreads + threadIdx.x;
-            if (e < n) atomicAdd(&h[(keys[e] >> shift) & mask], 1u);
+            if (e < n) atomicAdd(&h[(keys[e * stride] >> shift) & mask], 1u);
         }
     }
     __syncthreads();
-    if (threadIdx.x <= mask) hist[(int64_t)blockIdx.x * (mask + 1) + threadIdx.x] = h[threadIdx.x];  // row of mask+1 bins
+    for (int i = threadIdx.x; i <= (int)mask; i += kSortThreads) hist[(int64_t)blockIdx.x * (mask + 1) + i] = h[i];  // row of mask+1 bins
 }
 
 // ---- exclusive scan of hist[tile][digit] in (digit-major, tile-minor) order ----------------------------------------
@@ -209,39 +220,90 @@ __global__ void __launch_bounds__(kRadix) colscan_apply_kernel(uint32_t* __restr
     }
 }
 
-// ---- the order in which the arrays of a tile pass through the 3-stage ring, fixed at compile time -------------------
-// Array ids: 0 = keys, 1 = carried source indices (HAS_IDX), then the component arrays.  Arrays are LOADED in `load`
-// order and MOVED (written to their destination) in `move` order; the two differ only under DRIFT, where the position
-// component c needs the velocity component c in shared memory at the same time: vel_c is loaded just before pos_c and
-// moved just after it.  Load k >= 3 goes into the stage freed by move k - 3.
+// ---- units: what moves through the ring as ONE element stream ---------------------------------------------------------------
+// Between the passes the records live in a PAIRED format of this file's own choosing: 4-byte arrays travel two by two as
+// 8-byte elements -- (key, carried source index), and the 4-byte components in declaration order, e.g. R1: (id, vel0),
+// (vel1, vel2) -- so that a tile of R1 is 6 element streams instead of 9: a third fewer array moves (each costs a dozen
+// barriers) and a third fewer ragged run ends.  Unit 0 is the key [+ index]; a unit is a single component (any size) or a
+// pair of 4-byte components.  The first pass reads plain SoA (a pair = two bulk copies into the two halves of a stage) and
+// the last pass writes plain SoA (a pair = two 4-byte stores), so the format never leaves the scratch buffer.
+template <class L, bool HAS_IDX>
+struct Units {
+    static constexpr int kMax = 1 + L::ncomp;
+    int n = 1;
+    int a[kMax] = {}, b[kMax] = {}, bytes[kMax] = {};       // components of the unit (b = -1: single), element bytes when paired
+    int unit_of[L::ncomp > 0 ? L::ncomp : 1] = {}, half_of[L::ncomp > 0 ? L::ncomp : 1] = {};
+    constexpr Units() {
+        a[0] = b[0] = -1;
+        bytes[0] = HAS_IDX ? 8 : 4;
+        int open = -1;  // a 4-byte single still waiting for a partner
+        for (int c = 0; c < L::ncomp; ++c) {
+            if (L::comp_size(c) == 4 && open >= 0) {
+                b[open] = c; bytes[open] = 8; unit_of[c] = open; half_of[c] = 1; open = -1;
+            } else {
+                const int u = n++;
+                a[u] = c; b[u] = -1; bytes[u] = L::comp_size(c); unit_of[c] = u; half_of[c] = 0;
+                if (L::comp_size(c) == 4) open = u;
+            }
+        }
+    }
+};
+
+// ---- the order in which the units of a tile pass through the 3-stage ring, fixed at compile time ---------------------------
+// Units are LOADED in `load` order and MOVED (written to their destination) in `move` order; the two differ only under DRIFT,
+// where the position component c needs the unit that holds the velocity component c in shared memory at the same time: that
+// unit is loaded before pos_c and moved after the last position component that needs it.  Load k >= 3 goes into the stage
+// freed by move k - 3; the constructor checks that every unit a move needs has been requested by then.
 constexpr int kRingStages = 3;
 template <class L, bool HAS_IDX, bool DRIFT>
 struct RingPlan {
-    static constexpr int kFirstComp = HAS_IDX ? 2 : 1;
-    static constexpr int kArrays = kFirstComp + L::ncomp;
-    int load[kArrays] = {}, move[kArrays] = {}, stage[kArrays] = {}, parity[kArrays] = {}, partner[kArrays] = {};
+    using U = Units<L, HAS_IDX>;
+    static constexpr int kMaxUnits = U::kMax;
+    int nu = 0;
+    int load[kMaxUnits] = {}, move[kMaxUnits] = {}, stage[kMaxUnits] = {}, parity[kMaxUnits] = {};
+    int partner[kMaxUnits] = {}, partner_half[kMaxUnits] = {};  // by unit: the unit (and half) holding the velocity of a position unit
+    bool ok = true;
     constexpr RingPlan() {
+        constexpr U units{};
+        nu = units.n;
         int nl = 0, nm = 0;
-        for (int a = 0; a < kFirstComp; ++a) { load[nl++] = a; move[nm++] = a; }
-        bool used[L::ncomp > 0 ? L::ncomp : 1] = {};
-        for (int a = 0; a < kArrays; ++a) partner[a] = -1;
+        bool loaded[kMaxUnits] = {}, moved[kMaxUnits] = {};
+        for (int u = 0; u < kMaxUnits; ++u) partner[u] = -1;
+        load[nl++] = 0; move[nm++] = 0; loaded[0] = moved[0] = true;
         if constexpr (DRIFT) {
             constexpr int P0 = L::template begin_of<pos_tag>, V0 = L::template begin_of<vel_tag>;
             for (int c = 0; c < 3; ++c) {
-                load[nl++] = kFirstComp + V0 + c; load[nl++] = kFirstComp + P0 + c;
-                move[nm++] = kFirstComp + P0 + c; move[nm++] = kFirstComp + V0 + c;
-                partner[kFirstComp + P0 + c] = kFirstComp + V0 + c;
-                used[P0 + c] = used[V0 + c] = true;
+                const int up = units.unit_of[P0 + c], uv = units.unit_of[V0 + c];
+                partner[up] = uv; partner_half[up] = units.half_of[V0 + c];
+                if (!loaded[uv]) { load[nl++] = uv; loaded[uv] = true; }
+                load[nl++] = up; loaded[up] = true;
+                move[nm++] = up; moved[up] = true;
+                bool needed_later = false;
+                for (int c2 = c + 1; c2 < 3; ++c2) needed_later |= units.unit_of[V0 + c2] == uv;
+                if (!needed_later && !moved[uv]) { move[nm++] = uv; moved[uv] = true; }
             }
         }
-        for (int c = 0; c < L::ncomp; ++c)
-            if (!used[c]) { load[nl++] = kFirstComp + c; move[nm++] = kFirstComp + c; }
-        int uses[kRingStages] = {};
-        for (int k = 0; k < kArrays; ++k) {
+        for (int u = 1; u < nu; ++u) {
+            if (!loaded[u]) load[nl++] = u;
+            if (!moved[u]) move[nm++] = u;
+        }
+        int uses[kRingStages] = {}, load_index[kMaxUnits] = {};
+        for (int k = 0; k < nu; ++k) {
             const int s = k < kRingStages ? k : stage[move[k - kRingStages]];
             stage[load[k]] = s;
             parity[load[k]] = uses[s] & 1;
+            load_index[load[k]] = k;
             ++uses[s];
+        }
+        for (int m = 0; m < nu; ++m) {  // everything move m reads was requested no later than after move m - 1
+            const int u = move[m];
+            ok &= load_index[u] <= m + kRingStages - 1;
+            if (partner[u] >= 0) {
+                ok &= load_index[partner[u]] <= m + kRingStages - 1;
+                bool partner_still_there = true;  // the partner's stage is freed by the partner's own move, which must come later
+                for (int m2 = 0; m2 < m; ++m2) partner_still_there &= move[m2] != partner[u];
+                ok &= partner_still_there;
+            }
         }
     }
 };
@@ -252,13 +314,13 @@ __device__ __forceinline__ void cluster_sync_relaxed() {
     asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.aligned;" ::: "memory");
 }
 
-// Pacing of the scatter stores (measured, profiles/r2_bin_study.md): a thread has kItems stores per array; issued back to
+// Pacing of the scatter stores (measured, profiles/r2_bin_study.md): a thread has kItems stores per unit; issued back to
 // back they reach the L2 out of step with the stores of the neighbouring CTAs that complete the same sectors.  Between
 // two stores of a thread the CTA (pace_sync 1) or the whole cluster (2, the default with clusters) therefore meets at a
 // barrier, so that at any moment the cluster writes ONE window of ~64 neighbouring bins; a sleep of a few tens of
 // nanoseconds can be added for studies.
-__device__ __forceinline__ void pace(int k, int pace_sync, int pace_ns) {
-    if (k == 0) return;
+__device__ __forceinline__ void pace(int k, int pace_sync, int pace_ns, int pace_every = 1) {
+    if (k == 0 || (k % pace_every) != 0) return;
     if (pace_sync == 1) __syncthreads();
     if (pace_sync == 2) cluster_sync_relaxed();
     if (pace_ns) __nanosleep(pace_ns);
@@ -266,23 +328,32 @@ __device__ __forceinline__ void pace(int k, int pace_sync, int pace_ns) {
 
 // ---- stable scatter of one tile through the TMA ring ----------------------------------------------------------------
 // 64 registers/thread and ~106 KB of shared memory let two CTAs share an SM: one ranks while the other streams.
-constexpr int kStageBytes = kTileN * 8;  // one array of the tile at 8 bytes per element
+constexpr int kStageBytes = kTileN * 8;  // one unit of the tile at 8 bytes per element
 constexpr int kRingSmem = kRingStages * kStageBytes + kTileN * 2 /*inv*/ + kRadix * 4 /*delta*/ + 32 * 4 /*scan*/ + 64 /*mbarriers*/;
 static_assert(kWarps * kRadix * 4 <= kStageBytes, "the per-warp counters alias ring stage 1");
 
-struct ScatterArgs {
-    const uint32_t* key_in; uint32_t* key_out;   // key_out may be null (last pass when no counts are wanted)
-    const uint32_t* idx_in; uint32_t* idx_out;   // idx_out may be null (no permutation wanted)
-    const uint32_t* base;                        // [tile][nb] global slot of the first item of (digit, tile)
-    int64_t n; int shift; uint32_t mask; int nbits; int ntiles; int csync; double dt; int pace_sync, pace_ns;
+template <int N>
+struct UnitPtrs {
+    void* p[N];
 };
 
-template <class L, bool HAS_IDX, bool DRIFT>
-__global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_ring_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst, ScatterArgs g) {
-    static_assert(!(HAS_IDX && DRIFT), "the drift is applied in the first pass, which generates the indices");
+struct ScatterArgs {
+    const uint32_t* key_in;   // IN = SoA (first pass): the cell keys made by cell_hist_kernel
+    uint32_t* idx_out;        // OUT = SoA (last pass): the permutation (HAS_IDX)
+    const uint32_t* base;     // [tile][nb] global slot of the first item of (digit, tile)
+    int64_t n; int shift; uint32_t mask; int nbits; int ntiles; int csync; double dt; int pace_sync, pace_ns, pace_every;
+};
+
+// IN_PAIRED / OUT_PAIRED: the format on either side (false = plain SoA: src in the first pass, dst in the last).
+template <class L, bool HAS_IDX, bool IN_PAIRED, bool OUT_PAIRED, bool DRIFT>
+__global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads)
+scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + L::ncomp> pin, UnitPtrs<1 + L::ncomp> pout, ScatterArgs g) {
+    static_assert(!(DRIFT && IN_PAIRED), "the drift is applied in the first pass, which reads the caller's SoA");
     using Plan = RingPlan<L, HAS_IDX, DRIFT>;
     constexpr Plan plan{};
-    constexpr int kFirstComp = Plan::kFirstComp, kArrays = Plan::kArrays;
+    constexpr Units<L, HAS_IDX> units{};
+    static_assert(plan.ok, "the ring plan does not keep a velocity unit resident while its position component moves");
+    constexpr int kUnits = units.n;
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* ring = smem;
     uint16_t* inv = reinterpret_cast<uint16_t*>(smem + kRingStages * kStageBytes);
@@ -303,39 +374,68 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
         for (int s = 0; s < kRingStages; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
-    // fill(stage, array): start bringing `cnt` elements of an array into a ring stage.  Called by ALL threads at
-    // CTA-uniform points, after a __syncthreads() that retired every reader of the stage.
-    auto fill = [&](int stage, const auto* gp) {
-        using T = std::remove_cv_t<std::remove_pointer_t<decltype(gp)>>;
-        unsigned char* sb = ring + stage * kStageBytes;
+    // copy(stage, byte offset in the stage, global array, element bytes): bring `cnt` elements of one array into a ring stage.
+    // Called by ALL threads at CTA-uniform points, after a __syncthreads() that retired every reader of the stage.
+    auto copy = [&](int stage, int at, const void* gp, int esize) {
+        unsigned char* sb = ring + stage * kStageBytes + at;
+        const unsigned char* gb = static_cast<const unsigned char*>(gp) + tile0 * esize;
         if (bulk) {
-            if (tid == 0) {
-                mbar_expect_tx(&full[stage], kTileN * (uint32_t)sizeof(T));
-                bulk_g2s(sb, gp + tile0, kTileN * (uint32_t)sizeof(T), &full[stage]);
-            }
+            if (tid == 0) bulk_g2s(sb, gb, (uint32_t)(kTileN * esize), &full[stage]);
+        } else if (esize == 8) {
+            for (int i = tid; i < cnt; i += kSortThreads) reinterpret_cast<uint64_t*>(sb)[i] = reinterpret_cast<const uint64_t*>(gb)[i];
+        } else if (esize == 4) {
+            for (int i = tid; i < cnt; i += kSortThreads) reinterpret_cast<uint32_t*>(sb)[i] = reinterpret_cast<const uint32_t*>(gb)[i];
         } else {
-            T* s = reinterpret_cast<T*>(sb);
-            for (int i = tid; i < cnt; i += kSortThreads) s[i] = gp[tile0 + i];
+            for (int i = tid; i < cnt * esize; i += kSortThreads) sb[i] = gb[i];
         }
     };
-    // ready(stage, parity): the array requested by the matching fill() is in shared memory
+    // ready(stage, parity): the unit requested by the matching fill is in shared memory
     auto ready = [&](int stage, uint32_t parity) {
         if (bulk) mbar_wait(&full[stage], parity);
         else __syncthreads();
     };
-    // fill_load<k>(): issue the k-th load of the plan (nothing if the plan has fewer arrays)
+    // fill_load<k>(): issue the k-th load of the plan (nothing if the plan has fewer units)
     auto fill_load = [&](auto ki) {
         constexpr int k = decltype(ki)::value;
-        if constexpr (k < kArrays) {
-            constexpr int a = plan.load[k];
-            if constexpr (a == 0) fill(plan.stage[a], g.key_in);
-            else if constexpr (HAS_IDX && a == 1) fill(plan.stage[a], g.idx_in);
-            else fill(plan.stage[a], comp_ptr<L, a - kFirstComp>(src));
+        if constexpr (k < kUnits) {
+            constexpr int u = plan.load[k];
+            constexpr int st = plan.stage[u];
+            constexpr int ua = units.a[u], ub = units.b[u], ubytes = units.bytes[u];  // (constant-evaluated: `units` is not captured)
+            if constexpr (IN_PAIRED) {
+                if (bulk && tid == 0) mbar_expect_tx(&full[st], (uint32_t)(kTileN * ubytes));
+                copy(st, 0, pin.p[u], ubytes);
+            } else if constexpr (u == 0) {
+                if (bulk && tid == 0) mbar_expect_tx(&full[st], (uint32_t)(kTileN * 4));
+                copy(st, 0, g.key_in, 4);
+            } else if constexpr (ub < 0) {
+                if (bulk && tid == 0) mbar_expect_tx(&full[st], (uint32_t)(kTileN * ubytes));
+                copy(st, 0, soa_in.p[ua], ubytes);
+            } else {  // a pair read from plain SoA: two copies into the two halves of the stage
+                if (bulk && tid == 0) mbar_expect_tx(&full[st], (uint32_t)(kTileN * 8));
+                copy(st, 0, soa_in.p[ua], 4);
+                copy(st, kTileN * 4, soa_in.p[ub], 4);
+            }
         }
+    };
+    // halves of a pair unit in its stage: interleaved (lo, hi) when it arrived paired, two half-stages when it came from SoA
+    auto pair_at = [&](const unsigned char* sb, uint32_t s) -> uint2 {
+        if constexpr (IN_PAIRED) return reinterpret_cast<const uint2*>(sb)[s];
+        else return make_uint2(reinterpret_cast<const uint32_t*>(sb)[s], reinterpret_cast<const uint32_t*>(sb)[kTileN + s]);
+    };
+    constexpr bool kKeyIsPair = IN_PAIRED && HAS_IDX;  // unit 0 in shared memory: (key, idx) pairs, else plain keys
+    auto key_at = [&](uint32_t e) -> uint32_t {
+        if constexpr (kKeyIsPair) return reinterpret_cast<const uint2*>(ring)[e].x;
+        else return reinterpret_cast<const uint32_t*>(ring)[e];
     };
     static_assert(plan.load[0] == 0 && plan.move[0] == 0 && plan.stage[0] == 0, "the keys lead");
     for (int i = tid; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
-    const uint32_t my_base = (tid <= (int)mask && (int)blockIdx.x < g.ntiles ? g.base[(int64_t)blockIdx.x * (mask + 1) + tid] : 0u);  // consumed after the ranking
+    constexpr int kBinsPerThread = kRadix / kSortThreads > 0 ? kRadix / kSortThreads : 1;  // thread t owns bins [t B, t B + B)
+    uint32_t my_base[kBinsPerThread];  // consumed after the ranking
+#pragma unroll
+    for (int i = 0; i < kBinsPerThread; ++i) {
+        const int b = tid * kBinsPerThread + i;
+        my_base[i] = (b <= (int)mask && (int)blockIdx.x < g.ntiles ? g.base[(int64_t)blockIdx.x * (mask + 1) + b] : 0u);
+    }
     __syncthreads();  // barriers initialised, counters zeroed
 
     // Stage 1 is the counters for now, so start with loads 0 and 2.
@@ -344,7 +444,6 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
 
     // ---- ranking: warp w owns elements [256 w, 256 w + 256) of the tile, 8 rounds of 32 in element order -------
     ready(0, 0);
-    const uint32_t* keybuf = reinterpret_cast<const uint32_t*>(ring);
     const int e0 = warp * (32 * kItems) + lane;
     uint32_t lpos[kItems];
     uint32_t* mycnt = wcnt + warp * kRadix;
@@ -354,7 +453,7 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
     for (int k = 0; k < kItems; ++k) {  // lanes holding the same digit, from one ballot per digit bit (no MATCH: its cost grows with the number of distinct values)
         const int e = e0 + k * 32;
         const bool valid = e < cnt;
-        const uint32_t d = valid ? (keybuf[e] >> shift) & mask : 0u;
+        const uint32_t d = valid ? (key_at(e) >> shift) & mask : 0u;
         uint32_t m = __ballot_sync(0xffffffffu, valid);
 #pragma unroll
         for (int b = 0; b < kRadixBits; ++b) {
@@ -376,20 +475,30 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
         __syncwarp();
     }
     __syncthreads();
-    {   // digit d = tid: tile total -> first slot of the bin in tile-sorted order -> per-warp first slots
-        uint32_t total = 0;
-        if (tid < kRadix) {
+    {   // bins of this thread: tile totals -> first slot of each bin in tile-sorted order -> per-warp first slots
+        uint32_t tot[kBinsPerThread], sum = 0;
 #pragma unroll
-            for (int w = 0; w < kWarps; ++w) total += wcnt[w * kRadix + tid];
+        for (int i = 0; i < kBinsPerThread; ++i) {
+            const int b = tid * kBinsPerThread + i;
+            tot[i] = 0;
+            if (b < kRadix) {
+#pragma unroll
+                for (int w = 0; w < kWarps; ++w) tot[i] += wcnt[w * kRadix + b];
+            }
+            sum += tot[i];
         }
-        uint32_t run = block_excl_scan(total, scan_sm);
-        if (tid < kRadix) {
-            delta[tid] = my_base - run;
+        uint32_t run = block_excl_scan(sum, scan_sm);
 #pragma unroll
-            for (int w = 0; w < kWarps; ++w) {
-                const uint32_t c = wcnt[w * kRadix + tid];
-                wcnt[w * kRadix + tid] = run;
-                run += c;
+        for (int i = 0; i < kBinsPerThread; ++i) {
+            const int b = tid * kBinsPerThread + i;
+            if (b < kRadix) {
+                delta[b] = my_base[i] - run;
+#pragma unroll
+                for (int w = 0; w < kWarps; ++w) {
+                    const uint32_t c = wcnt[w * kRadix + b];
+                    wcnt[w * kRadix + b] = run;
+                    run += c;
+                }
             }
         }
     }
@@ -397,7 +506,7 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
 #pragma unroll
     for (int k = 0; k < kItems; ++k) {
         const int e = e0 + k * 32;
-        if (e < cnt) inv[lpos[k] + mycnt[(keybuf[e] >> shift) & mask]] = (uint16_t)e;
+        if (e < cnt) inv[lpos[k] + mycnt[(key_at(e) >> shift) & mask]] = (uint16_t)e;
     }
     fence_async_smem();  // the counters (generic-proxy writes) are about to be overwritten by a bulk copy
     __syncthreads();     // inv complete, counters dead: stage 1 joins the ring
@@ -408,100 +517,135 @@ __global__ void __launch_bounds__(kSortThreads, 1024 / kSortThreads) scatter_rin
     // neighbouring bins.  Few runs open at a time is what lets the L2 merge their pieces: giving every warp its own 256
     // consecutive slots instead (16 windows open per CTA) was measured 25 % slower (profiles/r2_bin_study.md).
 #define SLOT(k) (tid + (k) * kSortThreads)
+#define SRC(k) ((srcp[(k) >> 1] >> (((k) & 1) * 16)) & 0xffffu)
     uint32_t gdest[kItems], srcp[kItems / 2];  // source elements packed two per register
-    {
-        uint32_t kv[kItems];
+    {   // unit 0: the key [and the source index: generated in the first pass, carried afterwards]
+        uint32_t kv[kItems], iv[kItems];
 #pragma unroll
         for (int k = 0; k < kItems; ++k) {
             const int j = SLOT(k);
             uint32_t s = 0;
-            kv[k] = 0;
-            gdest[k] = 0;
+            kv[k] = iv[k] = gdest[k] = 0;
             if (j < cnt) {
                 s = inv[j];
-                kv[k] = keybuf[s];
+                if constexpr (kKeyIsPair) {
+                    const uint2 p = reinterpret_cast<const uint2*>(ring)[s];
+                    kv[k] = p.x; iv[k] = p.y;
+                } else {
+                    kv[k] = key_at(s);
+                    iv[k] = (uint32_t)(tile0 + s);
+                }
                 gdest[k] = delta[(kv[k] >> shift) & mask] + (uint32_t)j;
             }
             if (k & 1) srcp[k >> 1] |= s << 16; else srcp[k >> 1] = s;
         }
         if (g.csync) cluster_sync_relaxed();
-        if (g.key_out) {
+        // The stores come BEFORE the barrier on purpose: they consume the loaded values, so every shared-memory read of this
+        // stage has completed when its thread arrives.  A barrier alone does not order reads that are still in flight in the
+        // generic proxy against the bulk copy (async proxy) that refills the stage.
+        if constexpr (OUT_PAIRED) {
 #pragma unroll
             for (int k = 0; k < kItems; ++k) {
-                pace(k, g.pace_sync, g.pace_ns);
-                if (SLOT(k) < cnt) g.key_out[gdest[k]] = kv[k];
+                pace(k, g.pace_sync, g.pace_ns, g.pace_every);
+                if (SLOT(k) < cnt) {
+                    if constexpr (HAS_IDX) static_cast<uint2*>(pout.p[0])[gdest[k]] = make_uint2(kv[k], iv[k]);
+                    else static_cast<uint32_t*>(pout.p[0])[gdest[k]] = kv[k];
+                }
             }
-        }
-        if constexpr (!HAS_IDX) {
-            if (g.idx_out) {
-                if (g.csync && g.key_out) cluster_sync_relaxed();
+        } else {
+            if constexpr (HAS_IDX) {  // the last pass writes no keys: counts / offsets come from the sorted positions
 #pragma unroll
                 for (int k = 0; k < kItems; ++k) {
-                    pace(k, g.pace_sync, g.pace_ns);
-                    if (SLOT(k) < cnt) g.idx_out[gdest[k]] = (uint32_t)(tile0 + ((srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu));
+                    pace(k, g.pace_sync, g.pace_ns, g.pace_every);
+                    if (SLOT(k) < cnt) g.idx_out[gdest[k]] = iv[k];
                 }
             }
         }
     }
-    // gdest depends on every key read of this thread, and gdest is consumed by stores or kept live below: the reads of
-    // stage 0 have completed before the barrier (see the note in move()).
     __syncthreads();  // the keys have been read: stage 0 is free
     fill_load(std::integral_constant<int, kRingStages>{});
 
-    // move<m>(): write the m-th array of the move order to its destination, then refill its stage with load m + 3
+    // move<m>(): write the m-th unit of the move order to its destination, then refill its stage with load m + 3
     auto move = [&](auto mi) {
         constexpr int m = decltype(mi)::value;
-        constexpr int a = plan.move[m];
-        constexpr int p = plan.partner[a];
-        auto body = [&](const auto* tp, auto* gout) {
-            using T = std::remove_cv_t<std::remove_pointer_t<decltype(tp)>>;
-            ready(plan.stage[a], plan.parity[a]);
-            const T* sb = reinterpret_cast<const T*>(ring + plan.stage[a] * kStageBytes);
+        constexpr int u = plan.move[m];
+        constexpr int p = plan.partner[u];
+        constexpr int ca = units.a[u] >= 0 ? units.a[u] : 0, cb = units.b[u] >= 0 ? units.b[u] : 0;
+        constexpr bool is_pair = units.b[u] >= 0;
+        constexpr int st = plan.stage[u], par = plan.parity[u];
+        ready(st, par);
+        const unsigned char* sb = ring + st * kStageBytes;
+        if constexpr (is_pair) {  // a pair of 4-byte components
+            uint2 v[kItems];
+#pragma unroll
+            for (int k = 0; k < kItems; ++k)
+                if (SLOT(k) < cnt) v[k] = pair_at(sb, SRC(k));
+            if (g.csync) cluster_sync_relaxed();
+#pragma unroll
+            for (int k = 0; k < kItems; ++k) {
+                pace(k, g.pace_sync, g.pace_ns, g.pace_every);
+                if (SLOT(k) < cnt) {
+                    if constexpr (OUT_PAIRED) {
+                        static_cast<uint2*>(pout.p[u])[gdest[k]] = v[k];
+                    } else {
+                        static_cast<uint32_t*>(soa_out.p[ca])[gdest[k]] = v[k].x;
+                        static_cast<uint32_t*>(soa_out.p[cb])[gdest[k]] = v[k].y;
+                    }
+                    (void)cb;
+                }
+            }
+        } else {
+            using T = typename L::template comp_type<ca>;
+            const T* tb = reinterpret_cast<const T*>(sb);
             T v[kItems];
-            if constexpr (p >= 0) {  // DRIFT: this is a position component; its velocity component is in another stage
-                using V = typename L::template comp_type<(p >= 0 ? p - kFirstComp : 0)>;
-                ready(plan.stage[p >= 0 ? p : 0], plan.parity[p >= 0 ? p : 0]);
-                const V* vb = reinterpret_cast<const V*>(ring + plan.stage[p >= 0 ? p : 0] * kStageBytes);
+            if constexpr (p >= 0) {  // DRIFT: a position component; its velocity component sits in another unit's stage
+                constexpr int pu = p >= 0 ? p : 0;
+                constexpr int pst = plan.stage[pu], ppar = plan.parity[pu];
+                constexpr int voff = units.b[pu] >= 0 ? plan.partner_half[u] * kTileN : 0;  // second half of a pair's stage
+                using V = typename L::template type_of<vel_tag>;
+                ready(pst, ppar);
+                const V* vb = reinterpret_cast<const V*>(ring + pst * kStageBytes) + voff;
 #pragma unroll
                 for (int k = 0; k < kItems; ++k) {
-                    const uint32_t s = (srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
-                    if (SLOT(k) < cnt) v[k] = drift1<V>(g.dt, vb[s], sb[s]);
+                    const uint32_t s = SRC(k);
+                    if (SLOT(k) < cnt) v[k] = drift1<V>(g.dt, vb[s], tb[s]);
                 }
             } else {
 #pragma unroll
-                for (int k = 0; k < kItems; ++k) {
-                    const uint32_t s = (srcp[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
-                    if (SLOT(k) < cnt) v[k] = sb[s];
-                }
+                for (int k = 0; k < kItems; ++k)
+                    if (SLOT(k) < cnt) v[k] = tb[SRC(k)];
             }
             if (g.csync) cluster_sync_relaxed();
-            // The stores come BEFORE the barrier on purpose: they consume the loaded values, so every shared-memory read
-            // of this stage has completed when its thread arrives.  A barrier alone does not order reads that are still
-            // in flight in the generic proxy against the bulk copy (async proxy) that refills the stage.
+            T* gout = OUT_PAIRED ? static_cast<T*>(pout.p[u]) : static_cast<T*>(soa_out.p[ca]);
 #pragma unroll
             for (int k = 0; k < kItems; ++k) {
-                pace(k, g.pace_sync, g.pace_ns);
+                pace(k, g.pace_sync, g.pace_ns, g.pace_every);
                 if (SLOT(k) < cnt) gout[gdest[k]] = v[k];
             }
-            __syncthreads();  // the stage can take the next load
-            fill_load(std::integral_constant<int, m + kRingStages>{});
-        };
-        if constexpr (HAS_IDX && a == 1) body(g.idx_in, g.idx_out);
-        else body(comp_ptr<L, (a >= kFirstComp ? a - kFirstComp : 0)>(src), comp_ptr<L, (a >= kFirstComp ? a - kFirstComp : 0)>(dst));
+        }
+        __syncthreads();  // every read of the stage has been consumed by a store: it can take the next load
+        fill_load(std::integral_constant<int, m + kRingStages>{});
     };
-    for_each_int<kArrays - 1>([&](auto i) { move(std::integral_constant<int, decltype(i)::value + 1>{}); });
+    for_each_int<kUnits - 1>([&](auto i) { move(std::integral_constant<int, decltype(i)::value + 1>{}); });
 #undef SLOT
+#undef SRC
 }
 
-// ---- counts / offsets from the sorted keys: off[c] = first sorted slot whose key is >= c (binary search) -------------
-__global__ void __launch_bounds__(256) cell_bounds_kernel(const uint32_t* __restrict__ sorted, int64_t n, uint32_t ncell,
-                                                          uint32_t* __restrict__ counts, uint32_t* __restrict__ offsets) {
+// ---- counts / offsets from the SORTED POSITIONS: off[c] = first slot of dst whose cell is >= c (binary search) -------------
+// The last pass writes no key array at all: the cell of a sorted particle is recomputed from its (drifted) position, which
+// is exact (a10 is a pure function of the position).  262 144 cells x 27 probes x 3 loads: far cheaper than writing and
+// re-reading 4 bytes per particle.
+__global__ void __launch_bounds__(256) cell_bounds_kernel(const double* __restrict__ x0, const double* __restrict__ x1, const double* __restrict__ x2,
+                                                          int64_t n, int log2g, uint32_t* __restrict__ counts, uint32_t* __restrict__ offsets) {
     __shared__ uint32_t off[257];
+    const uint32_t ncell = 1u << (3 * log2g);
+    const double G = (double)(1 << log2g);
+    const int gmax = (1 << log2g) - 1;
     auto lower_bound = [&](uint32_t c) {
         int64_t lo = 0, hi = n;
         while (lo < hi) {
             const int64_t mid = (lo + hi) >> 1;
-            if (sorted[mid] < c) lo = mid + 1; else hi = mid;
+            if (cell_of(x0[mid], x1[mid], x2[mid], G, gmax, log2g) < c) lo = mid + 1; else hi = mid;
         }
         return (uint32_t)lo;
     };
@@ -530,23 +674,26 @@ struct PassPlan {
     }
 };
 
+// Scratch: the cell keys made by cell_hist_kernel, one buffer in the
+// PAIRED format per intermediate result that is alive at a time (one for two passes, two to ping-pong between for more),
+// and the small tables.  The unit arrays are sized for the units WITH a carried index (the larger of the two unit lists).
 template <class L>
 struct BinPlan {
-    size_t key0, key1, idx1, idx3, slab, hist, partial, dbase, ke, total;
+    static constexpr int kU = 1 + L::ncomp;
+    size_t key0, hist, partial, dbase, ke, total;
+    size_t unit_off[2][kU];
     int64_t ntiles, nchunks;
-    size_t comp_off[L::ncomp];
     BinPlan(int64_t n, int npass) {
+        constexpr Units<L, true> units{};
         ntiles = (n + kTileN - 1) / kTileN;
         if (ntiles < 1) ntiles = 1;
         nchunks = (ntiles + kScanRows - 1) / kScanRows;
         size_t o = 0;
         auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1, kAlign); return at; };
         key0 = take((size_t)n * 4);
-        key1 = take((size_t)n * 4);
-        idx1 = take(npass >= 2 ? (size_t)n * 4 : 0);
-        idx3 = take(npass >= 3 ? (size_t)n * 4 : 0);
-        slab = o;
-        for (int c = 0; c < L::ncomp; ++c) comp_off[c] = take(npass >= 2 ? (size_t)n * L::comp_size(c) : 0);
+        for (int b = 0; b < 2; ++b)
+            for (int u = 0; u < kU; ++u)
+                unit_off[b][u] = take(b < npass - 1 && u < units.n ? (size_t)n * units.bytes[u] : 0);
         hist = take((size_t)ntiles * kRadix * 4);
         partial = take((size_t)nchunks * kRadix * 4);
         dbase = take(kRadix * 4);
@@ -561,8 +708,13 @@ size_t bin_scratch_bytes(int64_t n, int log2g) {
     else return BinPlan<L>(n, PassPlan(log2g, g_tune.bin_bits).npass).total;
 }
 
-template <class K>
-int launch_scatter(K kernel, int cluster, unsigned ntiles, cudaStream_t st, const void* src, const void* dst, const ScatterArgs& g) {
+template <class L, bool HAS_IDX, bool IN_PAIRED, bool OUT_PAIRED, bool DRIFT>
+int launch_scatter(int cluster, unsigned ntiles, cudaStream_t st, const Ptrs<L::ncomp>& soa_in, const Ptrs<L::ncomp>& soa_out,
+                   const UnitPtrs<1 + L::ncomp>& pin, const UnitPtrs<1 + L::ncomp>& pout, const ScatterArgs& g) {
+    auto kernel = scatter_ring_kernel<L, HAS_IDX, IN_PAIRED, OUT_PAIRED, DRIFT>;
+    // The function attributes are per device: set them on every call (cheap) rather than once per process.
+    SOAX_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingSmem));
+    SOAX_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((ntiles + cluster - 1) / cluster * cluster);  // padding CTAs own no tile but join the cluster barriers
     cfg.blockDim = dim3(kSortThreads);
@@ -573,9 +725,25 @@ int launch_scatter(K kernel, int cluster, unsigned ntiles, cudaStream_t st, cons
     attr[0].val.clusterDim.x = cluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = cluster > 1 ? 1 : 0;
-    void* args[] = {const_cast<void*>(src), const_cast<void*>(dst), const_cast<ScatterArgs*>(&g)};
-    SOAX_CUDA(cudaLaunchKernelExC(&cfg, reinterpret_cast<const void*>(kernel), args));
+    SOAX_CUDA(cudaLaunchKernelEx(&cfg, kernel, soa_in, soa_out, pin, pout, g));
     return launched();
+}
+
+// one pass: the format on either side follows from its position; the drift belongs to the first pass
+template <class L, bool HAS_IDX>
+int scatter_pass(bool first, bool last, bool drift, int cluster, unsigned ntiles, cudaStream_t st, const Ptrs<L::ncomp>& src,
+                 const Ptrs<L::ncomp>& dst, const UnitPtrs<1 + L::ncomp>& pin, const UnitPtrs<1 + L::ncomp>& pout, const ScatterArgs& g) {
+    constexpr bool has_vel = L::template has_as<vel_tag, float, 3>() || L::template has_as<vel_tag, double, 3>();
+    if (first && last) {
+        if constexpr (has_vel) { if (drift) return launch_scatter<L, HAS_IDX, false, false, true>(cluster, ntiles, st, src, dst, pin, pout, g); }
+        return launch_scatter<L, HAS_IDX, false, false, false>(cluster, ntiles, st, src, dst, pin, pout, g);
+    }
+    if (first) {
+        if constexpr (has_vel) { if (drift) return launch_scatter<L, HAS_IDX, false, true, true>(cluster, ntiles, st, src, dst, pin, pout, g); }
+        return launch_scatter<L, HAS_IDX, false, true, false>(cluster, ntiles, st, src, dst, pin, pout, g);
+    }
+    if (last) return launch_scatter<L, HAS_IDX, true, false, false>(cluster, ntiles, st, src, dst, pin, pout, g);
+    return launch_scatter<L, HAS_IDX, true, true, false>(cluster, ntiles, st, src, dst, pin, pout, g);
 }
 
 template <class L>
@@ -600,46 +768,40 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
         const BinPlan<L> plan(n, npass);
         if (a.scratch_bytes < plan.total) return SOAX_ERR_ALLOC;
         char* sc = static_cast<char*>(a.scratch);
-        uint32_t* keys[2] = {reinterpret_cast<uint32_t*>(sc + plan.key0), reinterpret_cast<uint32_t*>(sc + plan.key1)};
-        uint32_t* idxs[2] = {reinterpret_cast<uint32_t*>(sc + plan.idx1), reinterpret_cast<uint32_t*>(sc + plan.idx3)};
+        uint32_t* key0 = reinterpret_cast<uint32_t*>(sc + plan.key0);
         uint32_t* hist = reinterpret_cast<uint32_t*>(sc + plan.hist);
         uint32_t* partial = reinterpret_cast<uint32_t*>(sc + plan.partial);
         uint32_t* dbase = reinterpret_cast<uint32_t*>(sc + plan.dbase);
         double* kep = reinterpret_cast<double*>(sc + plan.ke);
         const Ptrs<L::ncomp> src = make_ptrs<L>(a.src), dst = make_ptrs<L>(a.dst);
-        Ptrs<L::ncomp> tmp;
-        for (int c = 0; c < L::ncomp; ++c) tmp.p[c] = sc + plan.comp_off[c];
+        UnitPtrs<1 + L::ncomp> buf[2];
+        for (int b = 0; b < 2; ++b)
+            for (int u = 0; u < 1 + L::ncomp; ++u) buf[b].p[u] = sc + plan.unit_off[b][u];
         const unsigned ntiles = (unsigned)plan.ntiles, nchunks = (unsigned)plan.nchunks;
-        const bool want_sorted_keys = a.counts || a.offsets;
-
-        // The function attributes are per device: set them on every call (cheap) rather than once per process.
-        for (const void* f : {(const void*)scatter_ring_kernel<L, false, false>, (const void*)scatter_ring_kernel<L, true, false>,
-                              (const void*)scatter_ring_kernel<L, false, has_vel>}) {
-            SOAX_CUDA(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingSmem));
-            SOAX_CUDA(cudaFuncSetAttribute(f, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        }
+        const bool has_idx = a.perm != nullptr;
 
         // Least-significant-digit passes over the 3*log2g key bits.
         int shift = 0;
         for (int pass = 0; pass < npass; ++pass) {
-            const bool last = pass == npass - 1;
+            const bool first = pass == 0, last = pass == npass - 1;
             const int w = pp.width[pass];
             const uint32_t mask = (1u << w) - 1u;
             const int nb = (int)mask + 1, scan_threads = nb < 32 ? 32 : nb;  // the table is [tile][nb]
-            const uint32_t* kin = keys[pass & 1];
-            if (pass == 0) {  // [drift +] cell index [+ KE] + first-digit histogram; src is read only
+            const UnitPtrs<1 + L::ncomp>& pin = buf[(pass + 1) & 1];   // written by the pass before
+            const UnitPtrs<1 + L::ncomp>& pout = buf[pass & 1];
+            if (first) {  // [drift +] cell index [+ KE] + first-digit histogram; src is read only
                 if constexpr (has_vel) {
-                    if (drift && ke) cell_hist_kernel<L, true, true><<<ntiles, kCellThreads, 0, st>>>(src, n, keys[0], a.drift_dt, a.log2g, mask, hist, kep);
-                    else if (drift) cell_hist_kernel<L, true, false><<<ntiles, kCellThreads, 0, st>>>(src, n, keys[0], a.drift_dt, a.log2g, mask, hist, kep);
-                    else if (ke) cell_hist_kernel<L, false, true><<<ntiles, kCellThreads, 0, st>>>(src, n, keys[0], a.drift_dt, a.log2g, mask, hist, kep);
-                    else cell_hist_kernel<L, false, false><<<ntiles, kCellThreads, 0, st>>>(src, n, keys[0], a.drift_dt, a.log2g, mask, hist, kep);
+                    if (drift && ke) cell_hist_kernel<L, true, true><<<ntiles, kCellThreads, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, mask, hist, kep);
+                    else if (drift) cell_hist_kernel<L, true, false><<<ntiles, kCellThreads, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, mask, hist, kep);
+                    else if (ke) cell_hist_kernel<L, false, true><<<ntiles, kCellThreads, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, mask, hist, kep);
+                    else cell_hist_kernel<L, false, false><<<ntiles, kCellThreads, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, mask, hist, kep);
                 } else {
-                    cell_hist_kernel<L, false, false><<<ntiles, kCellThreads, 0, st>>>(src, n, keys[0], a.drift_dt, a.log2g, mask, hist, kep);
+                    cell_hist_kernel<L, false, false><<<ntiles, kCellThreads, 0, st>>>(src, n, key0, a.drift_dt, a.log2g, mask, hist, kep);
                 }
                 SOAX_TRY(launched());
                 if (ke) SOAX_TRY(sum_partials(kep, (int)ntiles, a.kinetic, st));
-            } else {
-                tile_hist_kernel<<<ntiles, kSortThreads, 0, st>>>(kin, n, shift, mask, hist);
+            } else {  // the keys of the pass before: unit 0 of the paired buffer, every second word if an index travels along
+                tile_hist_kernel<<<ntiles, kSortThreads, 0, st>>>(static_cast<const uint32_t*>(pin.p[0]), has_idx ? 2 : 1, n, shift, mask, hist);
                 SOAX_TRY(launched());
             }
             colscan_reduce_kernel<<<nchunks, scan_threads, 0, st>>>(hist, (int)ntiles, nb, partial);
@@ -649,39 +811,25 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
             colscan_apply_kernel<<<nchunks, scan_threads, 0, st>>>(hist, (int)ntiles, nb, partial, dbase);
             SOAX_TRY(launched());
 
-            // the last pass writes dst; before it the records alternate between the scratch slab and dst
-            const bool to_dst = ((npass - 1 - pass) & 1) == 0;
-            const Ptrs<L::ncomp>& from = pass == 0 ? src : (to_dst ? tmp : dst);
-            const Ptrs<L::ncomp>& to = to_dst ? dst : tmp;
             ScatterArgs g{};
-            g.key_in = kin;
-            g.key_out = (!last || want_sorted_keys) ? keys[(pass + 1) & 1] : nullptr;  // sorted keys end in keys[npass & 1]
-            g.idx_in = pass == 0 || !a.perm ? nullptr : idxs[(pass - 1) & 1];
-            g.idx_out = !a.perm ? nullptr : (last ? a.perm : idxs[pass & 1]);
-            g.base = hist; g.n = n; g.shift = shift; g.mask = mask; g.nbits = w; g.ntiles = (int)ntiles; g.dt = a.drift_dt; 
-            // Short runs (wide digits) need the neighbouring tiles' pieces to reach the L2 together: clusters + barrier.
+            g.key_in = key0;
+            g.idx_out = a.perm;
+            g.base = hist; g.n = n; g.shift = shift; g.mask = mask; g.nbits = w; g.ntiles = (int)ntiles; g.dt = a.drift_dt;
+            // Short runs (wide digits) need the neighbouring tiles' pieces to reach the L2 together: clusters + barriers.
             const int want_cluster = g_tune.bin_cluster > 0 ? g_tune.bin_cluster : 4;
             const int cluster = (g_tune.bin_cluster > 0 || w >= 8) ? want_cluster : 1;
             g.csync = cluster > 1 && g_tune.bin_csync != 0;
             g.pace_sync = g_tune.bin_pace >= 0 ? (g_tune.bin_pace >> 12) & 3 : (cluster > 1 ? 2 : 0);
             if (g.pace_sync == 2 && cluster == 1) g.pace_sync = 1;
             g.pace_ns = g_tune.bin_pace >= 0 ? g_tune.bin_pace & 0xfff : 0;
-            if (pass == 0) {
-                if constexpr (has_vel) {
-                    if (drift) SOAX_TRY(launch_scatter(scatter_ring_kernel<L, false, true>, cluster, ntiles, st, &from, &to, g));
-                    else SOAX_TRY(launch_scatter(scatter_ring_kernel<L, false, false>, cluster, ntiles, st, &from, &to, g));
-                } else {
-                    SOAX_TRY(launch_scatter(scatter_ring_kernel<L, false, false>, cluster, ntiles, st, &from, &to, g));
-                }
-            } else if (a.perm) {
-                SOAX_TRY(launch_scatter(scatter_ring_kernel<L, true, false>, cluster, ntiles, st, &from, &to, g));
-            } else {
-                SOAX_TRY(launch_scatter(scatter_ring_kernel<L, false, false>, cluster, ntiles, st, &from, &to, g));
-            }
+            g.pace_every = g_tune.bin_pace_every > 0 ? g_tune.bin_pace_every : (g.pace_sync == 2 ? 2 : 1);  // measured: a cluster barrier every second store
+            if (has_idx) SOAX_TRY((scatter_pass<L, true>(first, last, drift, cluster, ntiles, st, src, dst, pin, pout, g)));
+            else SOAX_TRY((scatter_pass<L, false>(first, last, drift, cluster, ntiles, st, src, dst, pin, pout, g)));
             shift += w;
         }
-        if (want_sorted_keys) {
-            cell_bounds_kernel<<<ncell / 256 + 1, 256, 0, st>>>(keys[npass & 1], n, ncell, a.counts, a.offsets);
+        if (a.counts || a.offsets) {
+            cell_bounds_kernel<<<ncell / 256 + 1, 256, 0, st>>>(field_ptr<L, pos_tag>(dst, 0), field_ptr<L, pos_tag>(dst, 1), field_ptr<L, pos_tag>(dst, 2), n,
+                                                                 a.log2g, a.counts, a.offsets);
             SOAX_TRY(launched());
         }
         return SOAX_OK;

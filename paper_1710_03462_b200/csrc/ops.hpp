@@ -23,6 +23,7 @@ struct Tuning {
     int xpose_r = 0, xpose_ns = 0, xpose_ctas = 0;  // ring shape override: 256*r records per stage, ns stages, CTAs per SM cap (0 = default)
     int bin_bits = 0;       // digit width of the counting-sort passes: 0 = default (9: two passes for G = 64), else 1..9
     int bin_cluster = 0;    // 0 = default (clusters of 4 CTAs for digits of 8 or 9 bits, none below); 1, 2, 4, 8, 16: forced
+    int bin_pace_every = 0; // a pacing barrier every this many stores of a thread (0 = default: 2 for the cluster barrier, else 1)
     int bin_pace = -1;      // pacing of the scatter stores: -1 = default (cluster barrier with clusters); else bits 12-13 = 1: CTA barrier, 2: cluster barrier between a thread's stores; low 12 bits = nanoseconds of sleep
     int bin_csync = 1;      // with clusters: 1 = cluster barrier before every array's stores (default), 0 = none
 };
