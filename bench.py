@@ -506,8 +506,9 @@ def _extra_config4(torch, B, Cn, peak, ex, gbs, iters):
 
 def _extra_config5(torch, B, Cn, peak, ex, gbs, iters):
     """config 5: N = 2^27: drift + cell + KE + first histogram (src read-only), two 9-bit stable scatter passes moving all
-    7 arrays + key + carried index (the drift applied on the way), counts / offsets.  Ideal = 60 (drift) + 4 + 84 (permute
-    once) = 148 B/particle; what this pipeline must move = 40 (cell_hist) + 4 (hist) + 92 + 96 (two passes) = 232."""
+    7 arrays + key + carried index in a paired scratch format (the drift applied on the way), counts / offsets from the
+    sorted positions.  Ideal = 60 (drift) + 4 + 84 (permute once) = 148 B/particle; what this pipeline must move = 40
+    (cell_hist) + 8 (second histogram) + 44 + 48 (pass 1) + 48 + 44 (pass 2) = 232."""
     n5 = 1 << 27
     s5, d5 = Cn.Soax(Cn.R1, n5), Cn.Soax(Cn.R1, n5)
     device_fill(torch, s5, 7)
@@ -604,10 +605,11 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
     ref = torch.sort((i[0] * 64 + i[1]) * 64 + i[2], stable=True)[1].to(torch.int32)
     del i
     S = 4096                                                      # bin_pace bit 12: a CTA barrier between a thread's stores
-    rows = [(6, 1, 1, 0), (6, 1, 1, S), (6, 4, 1, S), (9, 1, 1, 0), (9, 1, 1, S), (9, 2, 1, S), (9, 4, 0, 0), (9, 4, 1, 0), (9, 4, 0, S),
-            (9, 4, 1, S), (9, 4, 1, 2 * S), (9, 4, 1, 100), (9, 4, 1, S + 100), (9, 8, 1, S), (9, 16, 1, S), (7, 4, 1, S), (5, 1, 1, 0), (0, 0, 1, -1)]
-    for bits, cl, cs, pace in rows:
-        for key, v in (("bin_bits", bits), ("bin_cluster", cl), ("bin_csync", cs), ("bin_pace", pace)):
+    rows = [(6, 1, 1, 0, 1), (6, 1, 1, S, 1), (6, 4, 1, S, 1), (9, 1, 1, 0, 1), (9, 1, 1, S, 1), (9, 2, 1, S, 1), (9, 4, 0, 0, 1), (9, 4, 1, 0, 1),
+            (9, 4, 0, S, 1), (9, 4, 1, S, 1), (9, 4, 1, 2 * S, 1), (9, 4, 1, 2 * S, 2), (9, 4, 1, 2 * S, 4), (9, 4, 1, 100, 1), (9, 4, 1, S + 100, 1),
+            (9, 8, 1, 2 * S, 2), (9, 16, 1, 2 * S, 2), (7, 4, 1, 2 * S, 2), (5, 1, 1, 0, 1), (0, 0, 1, -1, 0)]
+    for bits, cl, cs, pace, every in rows:
+        for key, v in (("bin_bits", bits), ("bin_cluster", cl), ("bin_csync", cs), ("bin_pace", pace), ("bin_pace_every", every)):
             B.soax_tune(key, v)
         scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
         r = s5.bin_permute(d5, 64, scratch=scratch)
@@ -616,10 +618,10 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
         ms1 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), 5, 2)
         print(json.dumps({"study": "config 5 pipeline at 2^27", "digit_bits": bits or 9, "passes": (18 + (bits or 9) - 1) // (bits or 9),
                           "cluster": cl or "default(4)", "cluster_barrier": cs, "pace_barrier": "default(cluster)" if pace < 0 else ("none", "cta", "cluster")[pace >> 12],
-                          "pace_sleep_ns": 0 if pace < 0 else pace & 0xfff, "ms_no_drift": round(ms0, 3), "ms_drift_ke": round(ms1, 3),
+                          "pace_sleep_ns": 0 if pace < 0 else pace & 0xfff, "pace_every_n_stores": every or "default(2)", "ms_no_drift": round(ms0, 3), "ms_drift_ke": round(ms1, 3),
                           "permutation_equals_stable_argsort": ok, "scratch_GB": round(scratch.numel() / 1e9, 3)}), flush=True)
         del scratch, r
-    for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1), ("bin_pace", -1)):
+    for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1), ("bin_pace", -1), ("bin_pace_every", 0)):
         B.soax_tune(key, v)
 
 
