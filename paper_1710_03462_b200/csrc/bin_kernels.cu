@@ -690,7 +690,7 @@ struct BinPlan {
         nchunks = (ntiles + kScanRows - 1) / kScanRows;
         size_t o = 0;
         auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1, kAlign); return at; };
-        key0 = take((size_t)n * 4);
+        key0 = take(npass >= 2 ? 0 : (size_t)n * 4);  // with two or more passes the keys live in dst (see bin_permute_entry)
         for (int b = 0; b < 2; ++b)
             for (int u = 0; u < kU; ++u)
                 unit_off[b][u] = take(b < npass - 1 && u < units.n ? (size_t)n * units.bytes[u] : 0);
@@ -768,7 +768,13 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
         const BinPlan<L> plan(n, npass);
         if (a.scratch_bytes < plan.total) return SOAX_ERR_ALLOC;
         char* sc = static_cast<char*>(a.scratch);
+        // The cell keys are dead once the first pass has read them, and dst is not written before the last pass: with two
+        // or more passes the keys live in dst's own memory (its first component array of >= 4 bytes per element).
         uint32_t* key0 = reinterpret_cast<uint32_t*>(sc + plan.key0);
+        if (npass >= 2) {
+            for (int c = 0; c < L::ncomp; ++c)
+                if (L::comp_size(c) >= 4) { key0 = static_cast<uint32_t*>(a.dst[c]); break; }
+        }
         uint32_t* hist = reinterpret_cast<uint32_t*>(sc + plan.hist);
         uint32_t* partial = reinterpret_cast<uint32_t*>(sc + plan.partial);
         uint32_t* dbase = reinterpret_cast<uint32_t*>(sc + plan.dbase);
