@@ -10,10 +10,9 @@
 //   * gather of arbitrary rows into packed AoS records -- the bulk form of getElement(i);
 //     push_back of AoS records is soax_aos_to_soa at an offset (api.cu).
 // Mask bytes are counted per SEGMENT of 256 (one warp's worth: 8 rounds of 32 lanes) and per tile of 16 segments; a
-// one-CTA scan turns the tile counts into prefixes.  The data kernels have no shared memory and no CTA barrier: each
-// warp owns one segment, rebuilds its prefix from the tile prefix + the counts of the segments before it, ranks its
-// 256 elements with ballots, and moves them -- warps in different phases overlap freely, which a barrier-phased CTA
-// (mask, rank, load, store) does not allow at one CTA per SM.
+// one-CTA scan turns the tile counts into prefixes.  The stable compaction takes a tile per CTA through a TMA ring and writes
+// 16-byte vectors (compact_ring_kernel); the in-place removal ranks holes and movers per warp-owned segment without shared
+// memory or CTA barriers and then moves one row per thread.
 #include "common.cuh"
 #include "ops.hpp"
 #include "tma.cuh"
@@ -189,50 +188,129 @@ __global__ void __launch_bounds__(256) move_rows_kernel(Ptrs<L::ncomp> a, const 
 }
 
 // ---- STABLE: dst[i - #flagged before i] = src[i] for every surviving i, every component array ---------------------------
+// One CTA per tile of 4096 source rows (the tile of the count pass, so tile_prefix[tile] = flagged rows before it).  Thread t
+// owns rows [8 t, 8 t + 8): a block scan of the survivor counts gives every survivor its slot in the tile's compacted run, and
+// `inv` (slot -> source row) is built once.  Then every component array of the tile arrives by ONE bulk asynchronous copy (TMA)
+// into a 3-stage ring, and the compacted run leaves as 16-BYTE VECTOR STORES: the run is contiguous in dst, so after at most 3
+// (4-byte types) head elements every thread writes 4 consecutive elements (2 of 8 bytes, 16 of 1 byte) at a 16-byte aligned
+// address -- 16 sectors per store request instead of the ~5 of a warp that writes 29 survivors one element per lane.
+constexpr int kCompThreads = 512;
+constexpr int kCompItems = kCTile / kCompThreads;  // 8 rows per thread
+constexpr int kCompStages = 3;
+constexpr int kCompStageBytes = kCTile * 8;
+constexpr int kCompSmem = kCompStages * kCompStageBytes + kCTile * 2 /*inv*/ + 32 * 4 /*scan*/ + 64 /*mbarriers*/;
+
 template <class L>
-__global__ void __launch_bounds__(256, 2) compact_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst, const uint8_t* __restrict__ kill, int64_t n,
-                                                      const uint32_t* __restrict__ tile_prefix, const uint32_t* __restrict__ seg_count,
-                                                      int64_t dst_capacity) {
-    const int64_t seg = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (seg * kSeg >= n) return;
-    const int lane = threadIdx.x & 31;
-    const uint32_t lt = (1u << lane) - 1u;
-    const SegRank r = seg_rank(kill, n, seg, tile_prefix, seg_count);
-    const int64_t s0 = seg * kSeg;                // first source element of the segment
-    const int64_t d0 = s0 - (int64_t)r.before;    // first destination slot of the segment's survivors
-    const uint32_t room = dst_capacity > d0 ? (uint32_t)min((int64_t)kSeg, dst_capacity - d0) : 0u;
-    uint32_t slot[kSegRounds], live = 0, run = 0;  // slot within the segment's run of survivors; bit k of live: moves
+__global__ void __launch_bounds__(kCompThreads, 2) compact_ring_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst, const uint8_t* __restrict__ kill, int64_t n,
+                                                                      const uint32_t* __restrict__ tile_prefix, int64_t dst_capacity) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* ring = smem;
+    uint16_t* inv = reinterpret_cast<uint16_t*>(smem + kCompStages * kCompStageBytes);
+    uint32_t* scan_sm = reinterpret_cast<uint32_t*>(smem + kCompStages * kCompStageBytes + kCTile * 2);
+    uint64_t* full = reinterpret_cast<uint64_t*>(scan_sm + 32);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t tile0 = (int64_t)blockIdx.x * kCTile;
+    const int cnt = (int)(n - tile0 < kCTile ? n - tile0 : kCTile);
+    const bool bulk = cnt == kCTile;
+    if (tid == 0) {
 #pragma unroll
-    for (int k = 0; k < kSegRounds; ++k) {
-        const uint32_t surv = ~r.bal[k];
-        slot[k] = run + __popc(surv & lt);
-        run += 32u - __popc(r.bal[k]);
-        // too small a destination is reported by the host (ALLOC); never write past it
-        if (s0 + k * 32 + lane < n && (surv >> lane & 1u) && slot[k] < room) live |= 1u << k;
+        for (int s = 0; s < kCompStages; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
     }
-    // Component arrays move in groups of up to kGroup: every load of a group is issued before its first store.  The values
-    // sit in TYPED per-component registers (CompRegs): funnelling them through a common 64-bit image made the compiler
-    // reuse one temporary per load and serialise the loads.
-    constexpr int kGroup = 4;
-    constexpr int kGroups = (L::ncomp + kGroup - 1) / kGroup;
-    for_each_int<kGroups>([&](auto gi) {
-        constexpr int G0 = decltype(gi)::value * kGroup;
-        constexpr int GN = L::ncomp - G0 < kGroup ? L::ncomp - G0 : kGroup;
-        CompRegs<L, G0, kSegRounds, std::make_integer_sequence<int, GN>> v;
-        for_each_int<GN>([&](auto ci) {
-            constexpr int C = G0 + decltype(ci)::value;
-            const auto* s = comp_ptr<L, C>(src) + s0 + lane;
+    __syncthreads();
+    auto fill = [&](auto ci) {  // start bringing component C of the tile into stage C % 3 (nothing past the last component)
+        constexpr int C = decltype(ci)::value;
+        if constexpr (C < L::ncomp) {
+            using T = typename L::template comp_type<C>;
+            unsigned char* sb = ring + (C % kCompStages) * kCompStageBytes;
+            const T* g = comp_ptr<L, C>(src) + tile0;
+            if (bulk) {
+                if (tid == 0) {
+                    mbar_expect_tx(&full[C % kCompStages], kCTile * (uint32_t)sizeof(T));
+                    bulk_g2s(sb, g, kCTile * (uint32_t)sizeof(T), &full[C % kCompStages]);
+                }
+            } else {
+                for (int i = tid; i < cnt; i += kCompThreads) reinterpret_cast<T*>(sb)[i] = g[i];
+            }
+        }
+    };
+    fill(std::integral_constant<int, 0>{});
+    fill(std::integral_constant<int, 1>{});
+    fill(std::integral_constant<int, 2>{});
+
+    // ---- survivors of this thread's 8 rows, block scan, inv ------------------------------------------------------------------
+    uint32_t alive = 0;  // bit i: row 8 t + i survives
+    {
+        const int64_t r0 = tile0 + (int64_t)tid * kCompItems;
+        if (r0 + kCompItems <= n && (reinterpret_cast<uintptr_t>(kill + r0) & 7) == 0) {
+            const uint2 m = *reinterpret_cast<const uint2*>(kill + r0);
 #pragma unroll
-            for (int k = 0; k < kSegRounds; ++k)
-                if (live >> k & 1u) v.template get<C>()[k] = s[k * 32];
-        });
-        for_each_int<GN>([&](auto ci) {
-            constexpr int C = G0 + decltype(ci)::value;
-            auto* d = comp_ptr<L, C>(dst) + d0;
+            for (int i = 0; i < 4; ++i) {
+                alive |= (((m.x >> (8 * i)) & 0xffu) == 0 ? 1u : 0u) << i;
+                alive |= (((m.y >> (8 * i)) & 0xffu) == 0 ? 1u : 0u) << (4 + i);
+            }
+        } else {
 #pragma unroll
-            for (int k = 0; k < kSegRounds; ++k)
-                if (live >> k & 1u) d[slot[k]] = v.template get<C>()[k];
-        });
+            for (int i = 0; i < kCompItems; ++i)
+                if (r0 + i < n && kill[r0 + i] == 0) alive |= 1u << i;
+        }
+    }
+    const uint32_t mine = __popc(alive);
+    uint32_t inc = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += y;
+    }
+    if (lane == 31) scan_sm[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t w = lane < kCompThreads / 32 ? scan_sm[lane] : 0u;
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += y;
+        }
+        scan_sm[lane] = winc - w;
+        if (lane == 31) scan_sm[31] = winc;  // (lanes >= 16 hold the total as well: kCompThreads / 32 = 16 warps)
+    }
+    __syncthreads();
+    uint32_t slot = scan_sm[warp] + inc - mine;
+    const uint32_t total = scan_sm[31];
+#pragma unroll
+    for (int i = 0; i < kCompItems; ++i)
+        if (alive >> i & 1u) inv[slot++] = (uint16_t)(tid * kCompItems + i);
+    __syncthreads();
+
+    // ---- the compacted run of the tile: dst slots [d0, d0 + S) -----------------------------------------------------------------
+    const int64_t d0 = tile0 - (int64_t)tile_prefix[blockIdx.x];
+    // too small a destination is reported through the count (Q25); never write past it
+    const int S = (int)(dst_capacity > d0 ? (dst_capacity - d0 < (int64_t)total ? dst_capacity - d0 : (int64_t)total) : 0);
+    for_each_comp<L>([&](auto ci) {
+        constexpr int C = decltype(ci)::value;
+        using T = typename L::template comp_type<C>;
+        constexpr int V = 16 / (int)sizeof(T);  // elements per 16-byte store
+        if (bulk) mbar_wait(&full[C % kCompStages], (C / kCompStages) & 1);
+        else __syncthreads();
+        const T* sb = reinterpret_cast<const T*>(ring + (C % kCompStages) * kCompStageBytes);
+        T* out = comp_ptr<L, C>(dst) + d0;
+        const int head = (int)((V - (d0 & (V - 1))) & (V - 1)) < S ? (int)((V - (d0 & (V - 1))) & (V - 1)) : S;
+        const int ngroups = (S - head) / V;
+        for (int g = tid; g < ngroups; g += kCompThreads) {
+            const int j0 = head + g * V;
+            struct alignas(16) Pack { T v[V]; } p;
+#pragma unroll
+            for (int i = 0; i < V; ++i) p.v[i] = sb[inv[j0 + i]];
+            *reinterpret_cast<Pack*>(out + j0) = p;  // 16-byte aligned: (d0 + head) is a multiple of V and the array base of 256
+        }
+        const int tail0 = head + ngroups * V;
+        if (tid < head) out[tid] = sb[inv[tid]];
+        if (tid < S - tail0) out[tail0 + tid] = sb[inv[tail0 + tid]];
+        // The stores come BEFORE the barrier: they consume the loaded values, so every read of the stage has completed when
+        // its thread arrives and the bulk copy that refills the stage cannot overtake them (see bin_kernels.cu).
+        __syncthreads();
+        fill(std::integral_constant<int, C + kCompStages>{});
     });
 }
 
@@ -335,7 +413,8 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
         move_rows_kernel<L><<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(make_ptrs<L>(src), holes, movers, info);
         SOAX_TRY(launched());
     } else {
-        compact_kernel<L><<<seg_blocks, 256, 0, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, tile_count, seg_count, dst_capacity);
+        SOAX_CUDA(cudaFuncSetAttribute(compact_ring_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCompSmem));
+        compact_ring_kernel<L><<<(unsigned)plan.ntiles, kCompThreads, kCompSmem, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, tile_count, dst_capacity);
         SOAX_TRY(launched());
     }
     return SOAX_OK;
