@@ -1028,6 +1028,7 @@ def main() -> None:
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
     ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (digit width, cluster size, pacing)")
     ap.add_argument("--sweeps", action="store_true", help="launch-shape sweeps of the step and transpose kernels + the stream-count control")
+    ap.add_argument("--mem-probes", action="store_true", help="memory-system probes behind the scatter design (half-written sectors in the L2, DRAM rate vs burst size)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     ap.add_argument("--spawn-check", action="store_true", help="test aid: exercise the --gpus N launch path alone over gloo (no GPU)")
     args = ap.parse_args()
@@ -1035,6 +1036,10 @@ def main() -> None:
         raise SystemExit(spawn_ranks(args, sys.argv[1:]))
     if args.spawn_check:
         run_spawn_check(args)
+    elif args.mem_probes:                                           # a stand-alone executable built from csrc/probes/mem_probes.cu
+        import subprocess
+        from paper_1710_03462_b200.build import build_probe
+        raise SystemExit(subprocess.call([build_probe("mem_probes")]))
     elif args.impl == "reference":
         run_reference(args)
     else:

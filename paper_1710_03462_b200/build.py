@@ -29,7 +29,7 @@ def _nvcc() -> str:
 
 def _deps_mtime() -> float:
     files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INC, "soax.h"), os.path.abspath(__file__)]
-    return max(os.path.getmtime(f) for f in files)
+    return max(os.path.getmtime(f) for f in files if os.path.isfile(f))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -73,6 +73,17 @@ def _build_locked(verbose: bool) -> str:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     os.replace(tmp, LIB)
     return LIB
+
+
+def build_probe(name: str = "mem_probes") -> str:
+    """Compile csrc/probes/<name>.cu into a stand-alone executable under build/ (measurement aids, not part of libsoax.so)."""
+    os.makedirs(OBJ, exist_ok=True)
+    src, exe = os.path.join(CSRC, "probes", name + ".cu"), os.path.join(OBJ, name)
+    if not os.path.exists(exe) or os.path.getmtime(exe) < os.path.getmtime(src):
+        r = subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-o", exe, src], capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")
+    return exe
 
 
 if __name__ == "__main__":
