@@ -625,6 +625,51 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
         B.soax_tune(key, v)
 
 
+def run_scatter_trace(torch, B, Cn, prefix: str, log2n: int = 27) -> None:
+    """Per-phase timeline of the binning scatter (--scatter-trace PREFIX).  Needs a STUDY BUILD of the library:
+        SOAX_NVCC_FLAGS=-DSOAX_SCATTER_TRACE python -m paper_1710_03462_b200.build --force
+    in which thread 0 of every CTA stamps the phases of its tile with %globaltimer.  Runs config 5 once at N = 2^27 (drift + KE),
+    reads the two files the library wrote (one per pass) and prints one JSON line per phase: mean / median / 90th percentile over
+    the 32768 tiles, in nanoseconds.  Rebuild without the flag afterwards."""
+    import numpy as np
+    os.environ["SOAX_TRACE"] = prefix
+    n = 1 << log2n
+    s5, d5 = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
+    device_fill(torch, s5, 7)
+    s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True)
+    torch.cuda.synchronize()
+    del os.environ["SOAX_TRACE"]
+    names = {0: "kernel start", 1: "set-up done (barriers, counters zeroed, CTA barrier)", 2: "keys in shared memory", 40: "digit ballots done",
+             41: "per-warp counters updated", 42: "CTA barrier", 43: "bin totals + scan done", 44: "CTA barrier", 45: "inverse permutation written",
+             3: "fence + CTA barrier: stage 1 joins the ring", 4: "unit 0 (keys): sources and destinations computed", 5: "cluster barrier",
+             6: "unit 0 stored", 7: "CTA barrier"}
+    order = [0, 1, 2, 40, 41, 42, 43, 44, 45, 3, 4, 5, 6, 7]
+    for m in range(1, 6):
+        b = 8 + 6 * (m - 1)
+        names.update({b: f"move {m}: begin", b + 1: f"move {m}: unit in shared memory", b + 2: f"move {m}: gathered into registers",
+                      b + 3: f"move {m}: cluster barrier", b + 4: f"move {m}: stored (3 more cluster barriers inside)", b + 5: f"move {m}: CTA barrier"})
+        order += list(range(b, b + 6))
+    for tag, what in (("01", "pass 1 (SoA -> paired, drift applied)"), ("10", "pass 2 (paired -> SoA)")):
+        path = f"{prefix}_{tag}_0.bin"
+        if not os.path.exists(path):
+            print(json.dumps({"scatter_trace": what, "error": f"{path} missing: is the library a -DSOAX_SCATTER_TRACE build?"}))
+            continue
+        t = np.fromfile(path, dtype=np.uint64).reshape(-1, 64).astype(np.int64)
+        t = t[t[:, 0] > 0]
+        total = t[:, order[-1]] - t[:, 0]
+        span = float(t[:, order[-1]].max() - t[:, 0].min())
+        print(json.dumps({"scatter_trace": what, "tiles": int(len(t)), "tile_us_mean": round(float(total.mean()) / 1e3, 2),
+                          "kernel_span_us": round(span / 1e3, 1), "mean_concurrent_ctas": round(float(total.sum()) / span, 1)}))
+        for a, b in zip(order[:-1], order[1:]):
+            d = t[:, b] - t[:, a]
+            print(json.dumps({"pass": tag, "from": names[a], "to": names[b], "ns_mean": round(float(d.mean())), "ns_p50": round(float(np.percentile(d, 50))),
+                              "ns_p90": round(float(np.percentile(d, 90)))}))
+        os.remove(path)
+    for f in (f"{prefix}_01_1.bin", f"{prefix}_10_1.bin"):
+        if os.path.exists(f):
+            os.remove(f)
+
+
 def run_sweeps(torch, B, Cn) -> None:
     """The launch-shape sweeps DESIGN.md section 6 cites (--sweeps), each one JSON line per point, N = 2^24 R1:
       step      symplectic-Euler step: particles per thread x threads per CTA x persistent grid
@@ -791,6 +836,9 @@ def _run_soax(args) -> None:
         return
     if args.bin_study:
         run_bin_study(torch, B, Cn)
+        return
+    if args.scatter_trace:
+        run_scatter_trace(torch, B, Cn, args.scatter_trace)
         return
     if args.sweeps:
         run_sweeps(torch, B, Cn)
@@ -1028,6 +1076,7 @@ def main() -> None:
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
     ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (digit width, cluster size, pacing)")
     ap.add_argument("--sweeps", action="store_true", help="launch-shape sweeps of the step and transpose kernels + the stream-count control")
+    ap.add_argument("--scatter-trace", default="", metavar="PREFIX", help="per-phase timeline of the binning scatter (needs a -DSOAX_SCATTER_TRACE study build)")
     ap.add_argument("--mem-probes", action="store_true", help="memory-system probes behind the scatter design (half-written sectors in the L2, DRAM rate vs burst size)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     ap.add_argument("--spawn-check", action="store_true", help="test aid: exercise the --gpus N launch path alone over gloo (no GPU)")
@@ -1036,10 +1085,10 @@ def main() -> None:
         raise SystemExit(spawn_ranks(args, sys.argv[1:]))
     if args.spawn_check:
         run_spawn_check(args)
-    elif args.mem_probes:                                           # a stand-alone executable built from csrc/probes/mem_probes.cu
+    elif args.mem_probes:                                           # stand-alone executables built from csrc/probes/*.cu
         import subprocess
         from paper_1710_03462_b200.build import build_probe
-        raise SystemExit(subprocess.call([build_probe("mem_probes")]))
+        raise SystemExit(subprocess.call([build_probe("mem_probes")]) or subprocess.call([build_probe("rank_probe")]))
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -18,6 +18,7 @@ LIB = os.path.join(HERE, "libsoax.so")
 SOURCES = ["api.cu", "step_kernels.cu", "reduce_kernels.cu", "aos_kernels.cu", "bin_kernels.cu", "expr.cu", "container_kernels.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-I", INC]
+NVCC_FLAGS += os.environ.get("SOAX_NVCC_FLAGS", "").split()     # study builds only, e.g. -DSOAX_SCATTER_TRACE (bin_kernels.cu)
 
 
 def _nvcc() -> str:

@@ -23,7 +23,10 @@
 // a bin's run reach the L2 together and merge into full sectors.
 // Every step is a pure function of the data (no arrival-order atomics decide a position), so the result is the
 // unique stable permutation for ANY particle distribution, and bit-identical from run to run.
+#include <cstdio>
+#include <cstdlib>
 #include <type_traits>
+#include <vector>
 
 #include "common.cuh"
 #include "ops.hpp"
@@ -255,6 +258,16 @@ struct Units {
 // unit is loaded before pos_c and moved after the last position component that needs it.  Load k >= 3 goes into the stage
 // freed by move k - 3; the constructor checks that every unit a move needs has been requested by then.
 constexpr int kRingStages = 3;
+
+// Study builds (-DSOAX_SCATTER_TRACE, see build.py): thread 0 of every CTA stamps the phases of its tile with %globaltimer; with
+// SOAX_TRACE=<prefix> in the environment the first launches of the scatter write <prefix>_<n>.bin ([CTA][64] uint64 nanoseconds).
+// Compiled out of the shipped library.
+#ifdef SOAX_SCATTER_TRACE
+__device__ unsigned long long* g_trace = nullptr;
+#define TR(i) do { if (g_trace && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_trace[(size_t)blockIdx.x * 64 + (i)] = t_; } } while (0)
+#else
+#define TR(i) do { } while (0)
+#endif
 template <class L, bool HAS_IDX, bool DRIFT>
 struct RingPlan {
     using U = Units<L, HAS_IDX>;
@@ -369,6 +382,7 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
     const int cnt = n - tile0 < kTileN ? (n > tile0 ? (int)(n - tile0) : 0) : kTileN;  // 0: padding CTA of a cluster launch
     const bool bulk = cnt == kTileN;  // CTA-uniform: the ragged last tile is filled by ordinary loads instead
 
+    TR(0);
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < kRingStages; ++s) mbar_init(&full[s], 1);
@@ -428,6 +442,10 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
         else return reinterpret_cast<const uint32_t*>(ring)[e];
     };
     static_assert(plan.load[0] == 0 && plan.move[0] == 0 && plan.stage[0] == 0, "the keys lead");
+    // Stage 1 is the counters for now, so start with loads 0 and 2 -- at once: thread 0 has initialised the barriers it arms
+    // (program order + the init fence), and the latency of the keys' copy hides behind the set-up below.
+    fill_load(std::integral_constant<int, 0>{});
+    fill_load(std::integral_constant<int, 2>{});
     for (int i = tid; i < kWarps * kRadix; i += kSortThreads) wcnt[i] = 0;
     constexpr int kBinsPerThread = kRadix / kSortThreads > 0 ? kRadix / kSortThreads : 1;  // thread t owns bins [t B, t B + B)
     uint32_t my_base[kBinsPerThread];  // consumed after the ranking
@@ -438,19 +456,17 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
     }
     __syncthreads();  // barriers initialised, counters zeroed
 
-    // Stage 1 is the counters for now, so start with loads 0 and 2.
-    fill_load(std::integral_constant<int, 0>{});
-    fill_load(std::integral_constant<int, 2>{});
-
     // ---- ranking: warp w owns elements [256 w, 256 w + 256) of the tile, 8 rounds of 32 in element order -------
+    TR(1);
     ready(0, 0);
+    TR(2);
     const int e0 = warp * (32 * kItems) + lane;
     uint32_t lpos[kItems];
     uint32_t* mycnt = wcnt + warp * kRadix;
     const uint32_t lt = (1u << lane) - 1u;
     uint32_t peers[kItems];
 #pragma unroll
-    for (int k = 0; k < kItems; ++k) {  // lanes holding the same digit, from one ballot per digit bit (no MATCH: its cost grows with the number of distinct values)
+    for (int k = 0; k < kItems; ++k) {  // lanes holding the same digit, from one ballot per digit bit (MATCH costs twice as much; an atomicOr into a per-warp mask table the same: profiles/r2_scatter_trace.md)
         const int e = e0 + k * 32;
         const bool valid = e < cnt;
         const uint32_t d = valid ? (key_at(e) >> shift) & mask : 0u;
@@ -465,6 +481,7 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
         peers[k] = valid ? m : 0u;
         lpos[k] = d;
     }
+    TR(40);
 #pragma unroll
     for (int k = 0; k < kItems; ++k) {
         const uint32_t d = lpos[k];
@@ -474,7 +491,9 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
         if (peers[k] != 0u && lane == 31 - __clz(peers[k])) mycnt[d] = old + __popc(peers[k]);
         __syncwarp();
     }
+    TR(41);
     __syncthreads();
+    TR(42);
     {   // bins of this thread: tile totals -> first slot of each bin in tile-sorted order -> per-warp first slots
         uint32_t tot[kBinsPerThread], sum = 0;
 #pragma unroll
@@ -502,15 +521,19 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
             }
         }
     }
+    TR(43);
     __syncthreads();
+    TR(44);
 #pragma unroll
     for (int k = 0; k < kItems; ++k) {
         const int e = e0 + k * 32;
         if (e < cnt) inv[lpos[k] + mycnt[(key_at(e) >> shift) & mask]] = (uint16_t)e;
     }
+    TR(45);
     fence_async_smem();  // the counters (generic-proxy writes) are about to be overwritten by a bulk copy
     __syncthreads();     // inv complete, counters dead: stage 1 joins the ring
     fill_load(std::integral_constant<int, 1>{});
+    TR(3);
 
     // ---- output slots: thread t owns slots t, t + 512, ... of the tile-sorted order, so that in its k-th store the whole CTA
     // (and, in step with it, the other CTAs of the cluster) writes ONE window of 512 consecutive slots = the runs of ~64
@@ -539,7 +562,9 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
             }
             if (k & 1) srcp[k >> 1] |= s << 16; else srcp[k >> 1] = s;
         }
+        TR(4);
         if (g.csync) cluster_sync_relaxed();
+        TR(5);
         // The stores come BEFORE the barrier on purpose: they consume the loaded values, so every shared-memory read of this
         // stage has completed when its thread arrives.  A barrier alone does not order reads that are still in flight in the
         // generic proxy against the bulk copy (async proxy) that refills the stage.
@@ -562,7 +587,9 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
             }
         }
     }
+    TR(6);
     __syncthreads();  // the keys have been read: stage 0 is free
+    TR(7);
     fill_load(std::integral_constant<int, kRingStages>{});
 
     // move<m>(): write the m-th unit of the move order to its destination, then refill its stage with load m + 3
@@ -573,14 +600,18 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
         constexpr int ca = units.a[u] >= 0 ? units.a[u] : 0, cb = units.b[u] >= 0 ? units.b[u] : 0;
         constexpr bool is_pair = units.b[u] >= 0;
         constexpr int st = plan.stage[u], par = plan.parity[u];
+        TR(8 + 6 * (m - 1) + 0);
         ready(st, par);
+        TR(8 + 6 * (m - 1) + 1);
         const unsigned char* sb = ring + st * kStageBytes;
         if constexpr (is_pair) {  // a pair of 4-byte components
             uint2 v[kItems];
 #pragma unroll
             for (int k = 0; k < kItems; ++k)
                 if (SLOT(k) < cnt) v[k] = pair_at(sb, SRC(k));
+            TR(8 + 6 * (m - 1) + 2);
             if (g.csync) cluster_sync_relaxed();
+            TR(8 + 6 * (m - 1) + 3);
 #pragma unroll
             for (int k = 0; k < kItems; ++k) {
                 pace(k, g.pace_sync, g.pace_ns, g.pace_every);
@@ -615,7 +646,9 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
                 for (int k = 0; k < kItems; ++k)
                     if (SLOT(k) < cnt) v[k] = tb[SRC(k)];
             }
+            TR(8 + 6 * (m - 1) + 2);
             if (g.csync) cluster_sync_relaxed();
+            TR(8 + 6 * (m - 1) + 3);
             T* gout = OUT_PAIRED ? static_cast<T*>(pout.p[u]) : static_cast<T*>(soa_out.p[ca]);
 #pragma unroll
             for (int k = 0; k < kItems; ++k) {
@@ -623,7 +656,9 @@ scatter_ring_kernel(Ptrs<L::ncomp> soa_in, Ptrs<L::ncomp> soa_out, UnitPtrs<1 + 
                 if (SLOT(k) < cnt) gout[gdest[k]] = v[k];
             }
         }
+        TR(8 + 6 * (m - 1) + 4);
         __syncthreads();  // every read of the stage has been consumed by a store: it can take the next load
+        TR(8 + 6 * (m - 1) + 5);
         fill_load(std::integral_constant<int, m + kRingStages>{});
     };
     for_each_int<kUnits - 1>([&](auto i) { move(std::integral_constant<int, decltype(i)::value + 1>{}); });
@@ -725,7 +760,34 @@ int launch_scatter(int cluster, unsigned ntiles, cudaStream_t st, const Ptrs<L::
     attr[0].val.clusterDim.x = cluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = cluster > 1 ? 1 : 0;
+#ifdef SOAX_SCATTER_TRACE
+    static int trace_no = 0;  // per instantiation: <prefix>_<in paired><out paired>_<n>.bin
+    const char* tp = getenv("SOAX_TRACE");
+    if (tp && (trace_no >= 2 || 1 + L::ncomp > 9)) tp = nullptr;  // trace slots exist for up to 8 moves
+    unsigned long long* tbuf = nullptr;
+    if (tp) {
+        SOAX_CUDA(cudaMalloc(&tbuf, (size_t)cfg.gridDim.x * 64 * 8));
+        SOAX_CUDA(cudaMemset(tbuf, 0, (size_t)cfg.gridDim.x * 64 * 8));
+        SOAX_CUDA(cudaMemcpyToSymbol(g_trace, &tbuf, sizeof(tbuf)));
+    }
+#endif
     SOAX_CUDA(cudaLaunchKernelEx(&cfg, kernel, soa_in, soa_out, pin, pout, g));
+#ifdef SOAX_SCATTER_TRACE
+    if (tp) {
+        SOAX_CUDA(cudaDeviceSynchronize());
+        std::vector<unsigned long long> h((size_t)cfg.gridDim.x * 64);
+        SOAX_CUDA(cudaMemcpy(h.data(), tbuf, h.size() * 8, cudaMemcpyDeviceToHost));
+        char name[512];
+        std::snprintf(name, sizeof name, "%s_%d%d_%d.bin", tp, (int)IN_PAIRED, (int)OUT_PAIRED, trace_no++);
+        if (FILE* f = std::fopen(name, "wb")) {
+            std::fwrite(h.data(), 8, h.size(), f);
+            std::fclose(f);
+        }
+        SOAX_CUDA(cudaFree(tbuf));
+        tbuf = nullptr;
+        SOAX_CUDA(cudaMemcpyToSymbol(g_trace, &tbuf, sizeof(tbuf)));
+    }
+#endif
     return launched();
 }
 
