@@ -623,6 +623,27 @@ def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
         del scratch, r
     for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1), ("bin_pace", -1), ("bin_pace_every", 0)):
         B.soax_tune(key, v)
+    # Control: the SAME default kernel on sets whose tiles fall into fewer bins in the first pass (longer pieces per bin; the
+    # second pass sees all 512 bins as before).  If the first pass speeds up, the scatter is bound by how the memory system takes
+    # short pieces, not by the work of the SMs, which is the same.
+    del ref
+    g = torch.Generator(device="cuda")
+    g.manual_seed(1)
+    tile = torch.arange(n, device="cuda") // 4096
+    scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
+    for distinct in (512, 128, 64, 16):
+        w = max(distinct // 8, 1)                                 # low digit = (i1 & 7) 64 + i2: 8 values of i1 x w values of i2
+        for c in range(3):
+            s5.comp_view("pos", c).copy_(torch.rand(n, generator=g, device="cuda", dtype=torch.float64))
+        if distinct < 512:
+            for c, mult in ((2, 2654435761), (0, 40503)):
+                base = (tile * mult % 64) // w * w
+                i = base + torch.randint(0, w, (n,), generator=g, device="cuda")
+                s5.comp_view("pos", c).copy_((i.double() + torch.rand(n, generator=g, device="cuda", dtype=torch.float64)) / 64)
+                del base, i
+        ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, scratch=scratch), 5, 2)
+        print(json.dumps({"study": "piece-length control, default kernel, 2^27", "distinct_first_pass_digits_per_tile": distinct,
+                          "elements_per_tile_and_bin_first_pass": 4096 // distinct, "ms_no_drift": round(ms, 3)}), flush=True)
 
 
 def run_scatter_trace(torch, B, Cn, prefix: str, log2n: int = 27) -> None:
