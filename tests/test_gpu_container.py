@@ -184,9 +184,11 @@ def test_get_elements_out_of_range_rows_are_zero_records(gpu):
         assert np.array_equal(got[j], base[i] if i < n else np.zeros(40, np.uint8)), (j, i)
 
 
-@pytest.mark.parametrize("world,n_each", [(3, 4001), (8, 700), (1, 5000), (2, 0)])
+@pytest.mark.parametrize("world,n_each", [(3, 4001), (8, 700), (1, 5000), (2, 0), (8, 100), (5, 1)])
 def test_gather_segments_merges_sorted_runs(gpu, world, n_each):
-    """soax_gather_segments_aos against oracle.gather_segments, on the tables of a `world`-run merge by cell (G = 8)."""
+    """soax_gather_segments_aos against oracle.gather_segments, on the tables of a `world`-run merge by cell (G = 8).
+    (8, 100) and (5, 1): more segments per 1024-row tile than the kernel stages in shared memory (mostly empty ones), so the
+    whole-table search runs; the others take the staged path, with ragged last tiles."""
     torch, B, Cn = gpu
     G = 8
     rng = np.random.default_rng(world)
