@@ -208,6 +208,18 @@ size_t soax_scratch_bytes(const soax_layout* layout, int64_t n, int32_t grid_dim
 int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
                      uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
                      size_t scratch_bytes, void* stream);
+/* The same operation IN PLACE: on return `s` holds its particles [drifted and] sorted by cell; `work` (same layout, capacity
+ * >= n, must not alias s) is a work area whose contents are destroyed and whose live count does not change.  With src
+ * read-only, two out-of-place passes need an intermediate copy of every record plus key and carried index in scratch
+ * (48 B/particle for the 40-byte record); here the intermediate's 8-byte arrays live in `work`, the sorted set returns to
+ * `s` in the second pass, and scratch holds only (key, index) and the paired 4-byte components: 24 B/particle for that record
+ * (soax_scratch_bytes_inplace; 0 if unsupported).  Needs the default two-pass plan (16 <= G <= 64): UNSUPPORTED otherwise.
+ * dev_perm[j] = the index particle j of the result had before the call.  Everything else as soax_bin_permute. */
+size_t soax_scratch_bytes_inplace(const soax_layout* layout, int64_t n, int32_t grid_dim);
+int soax_bin_permute_inplace(soax_t* s, soax_t* work, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
+                             uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
+                             size_t scratch_bytes, void* stream);
+
 
 /* ---- NEXT-3: container operations on the device ---------------------------------
  * soax_remove deletes the particles whose byte in dev_kill (n bytes, one per live particle) is non-zero, from EVERY

@@ -66,6 +66,8 @@ SIGNATURES = {
     "soax_reduce_energy": (C.c_int, [_vp, _i32, _f64, _f64, _vp, _sz, _vp, _vp]),
     "soax_scratch_bytes": (_sz, [_vp, _i64, _i32]),
     "soax_bin_permute": (C.c_int, [_vp, _vp, _i32, _f64, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "soax_scratch_bytes_inplace": (_sz, [_vp, _i64, _i32]),
+    "soax_bin_permute_inplace": (C.c_int, [_vp, _vp, _i32, _f64, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "soax_gather_segments_aos": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _i64, _vp]),
     "soax_remove_scratch_bytes": (_sz, [_i64]),
     "soax_remove": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _sz, C.POINTER(_i64), _vp]),
@@ -239,6 +241,17 @@ def soax_bin_permute(src: int, dst: int, grid_dim: int, drift_dt: float, dev_cou
                      stream: int = 0) -> None:
     _check(lib().soax_bin_permute(src, dst, grid_dim, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
                                   dev_scratch, scratch_bytes, stream), "soax_bin_permute")
+
+
+def soax_scratch_bytes_inplace(layout: int, n: int, grid_dim: int) -> int:
+    return lib().soax_scratch_bytes_inplace(layout, n, grid_dim)
+
+
+def soax_bin_permute_inplace(s: int, work: int, grid_dim: int, drift_dt: float, dev_counts: int | None, dev_offsets: int | None,
+                             dev_perm: int | None, dev_kinetic: int | None, dev_scratch: int, scratch_bytes: int,
+                             stream: int = 0) -> None:
+    _check(lib().soax_bin_permute_inplace(s, work, grid_dim, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
+                                          dev_scratch, scratch_bytes, stream), "soax_bin_permute_inplace")
 
 
 # ---- container operations (NEXT-3) ------------------------------------------------------------------------------------

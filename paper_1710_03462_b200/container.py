@@ -131,20 +131,21 @@ class Soax:
         return aos
 
     def bin_permute(self, dst: "Soax", grid_dim: int, drift_dt: float = 0.0, want_kinetic: bool = False,
-                    scratch: torch.Tensor | None = None) -> dict:
-        """Returns device tensors: counts, offsets (uint32 as int32 views), perm, and kinetic (or None)."""
+                    scratch: torch.Tensor | None = None, inplace: bool = False) -> dict:
+        """Returns device tensors: counts, offsets (uint32 as int32 views), perm, and kinetic (or None).
+        inplace: the sorted set returns to self and `dst` is only a work container (soax_bin_permute_inplace)."""
         dev, n = self.slab.device, self.n
         ncell = grid_dim ** 3
-        need = B.soax_scratch_bytes(self.layout, n, grid_dim)
+        need = (B.soax_scratch_bytes_inplace if inplace else B.soax_scratch_bytes)(self.layout, n, grid_dim)
         if scratch is None:
             scratch = torch.empty(need, dtype=torch.uint8, device=dev)
         counts = torch.empty(ncell, dtype=torch.int32, device=dev)
         offsets = torch.empty(ncell, dtype=torch.int32, device=dev)
         perm = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
         kin = torch.empty(1, dtype=torch.float64, device=dev) if want_kinetic else None
-        B.soax_bin_permute(self.handle, dst.handle, grid_dim, drift_dt, counts.data_ptr(), offsets.data_ptr(),
-                           perm.data_ptr(), None if kin is None else kin.data_ptr(), scratch.data_ptr(), scratch.numel(),
-                           _stream())
+        (B.soax_bin_permute_inplace if inplace else B.soax_bin_permute)(
+            self.handle, dst.handle, grid_dim, drift_dt, counts.data_ptr(), offsets.data_ptr(), perm.data_ptr(),
+            None if kin is None else kin.data_ptr(), scratch.data_ptr(), scratch.numel(), _stream())
         return {"counts": counts, "offsets": offsets, "perm": perm[:n], "kinetic": kin, "scratch": scratch}
 
 

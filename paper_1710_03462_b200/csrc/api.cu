@@ -33,7 +33,7 @@ struct soax_layout {
     int (*gather_segments)(void* const*, const void*, const uint32_t*, const uint32_t*, int64_t, int64_t, cudaStream_t);
     int (*energy)(void* const*, int64_t, int, double, double, void*, double*, cudaStream_t);
     int (*bin_permute)(const BinArgs&, cudaStream_t);
-    size_t (*bin_scratch)(int64_t, int);
+    size_t (*bin_scratch)(int64_t, int, bool);
     int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t);
     int (*gather_rows)(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
 };
@@ -422,12 +422,16 @@ int soax_reduce_energy(const soax_t* s, int32_t kind, double k, double center, v
 
 size_t soax_scratch_bytes(const soax_layout* l, int64_t n, int32_t grid_dim) {
     if (!l || n < 0 || ilog2_exact(grid_dim) < 0 || !l->bin_scratch) return 0;
-    return l->bin_scratch(n, ilog2_exact(grid_dim));
+    return l->bin_scratch(n, ilog2_exact(grid_dim), false);
+}
+size_t soax_scratch_bytes_inplace(const soax_layout* l, int64_t n, int32_t grid_dim) {
+    if (!l || n < 0 || ilog2_exact(grid_dim) < 0 || !l->bin_scratch) return 0;
+    return l->bin_scratch(n, ilog2_exact(grid_dim), true);
 }
 
-int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
-                     uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
-                     size_t scratch_bytes, void* stream) {
+static int bin_permute_common(soax_t* src, soax_t* dst, bool inplace, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
+                              uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch, size_t scratch_bytes,
+                              void* stream) {
     if (!src || !dst || src == dst || src->layout != dst->layout || !dev_scratch || !aligned(dev_scratch, kAlign))
         return SOAX_ERR_INVALID_ARG;
     const int log2g = ilog2_exact(grid_dim);
@@ -436,13 +440,26 @@ int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt
     for (int c = 0; c < src->layout->ncomp; ++c)
         if (src->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
     if (live(src) >= ((int64_t)1 << 32)) return SOAX_ERR_UNSUPPORTED;
-    const size_t need = src->layout->bin_scratch(live(src), log2g);
+    const size_t need = src->layout->bin_scratch(live(src), log2g, inplace);
     if (need == 0) return SOAX_ERR_UNSUPPORTED;
     if (scratch_bytes < need) return SOAX_ERR_ALLOC;
     BinArgs a{src->comp, dst->comp, live(src), log2g, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic,
-              dev_scratch, scratch_bytes};
-    set_live(dst, live(src));
+              dev_scratch, scratch_bytes, inplace};
+    if (!inplace) set_live(dst, live(src));
     return src->layout->bin_permute(a, (cudaStream_t)stream);
+}
+
+int soax_bin_permute(soax_t* src, soax_t* dst, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
+                     uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
+                     size_t scratch_bytes, void* stream) {
+    return bin_permute_common(src, dst, false, grid_dim, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic, dev_scratch,
+                              scratch_bytes, stream);
+}
+int soax_bin_permute_inplace(soax_t* s, soax_t* work, int32_t grid_dim, double drift_dt, uint32_t* dev_counts,
+                             uint32_t* dev_offsets, uint32_t* dev_perm, double* dev_kinetic, void* dev_scratch,
+                             size_t scratch_bytes, void* stream) {
+    return bin_permute_common(s, work, true, grid_dim, drift_dt, dev_counts, dev_offsets, dev_perm, dev_kinetic, dev_scratch,
+                              scratch_bytes, stream);
 }
 
 // ---- NEXT-3: container operations (container_kernels.cu) ------------------------------------------------------------

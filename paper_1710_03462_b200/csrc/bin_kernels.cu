@@ -712,23 +712,41 @@ struct PassPlan {
 // Scratch: the cell keys made by cell_hist_kernel, one buffer in the
 // PAIRED format per intermediate result that is alive at a time (one for two passes, two to ping-pong between for more),
 // and the small tables.  The unit arrays are sized for the units WITH a carried index (the larger of the two unit lists).
+// IN PLACE (soax_bin_permute_inplace, two passes): the sorted set returns to src and the second container is only a work
+// area, so the intermediate's 8-byte single units live in the work container's own component arrays and its first 4-byte
+// array holds the cell keys; only unit 0 (key, carried index) and the PAIRS of 4-byte components need scratch.
+template <class L>
+constexpr bool unit_in_work(int u) {  // in-place: does unit u of the intermediate live in the work container?
+    constexpr Units<L, true> units{};
+    return u >= 1 && u < units.n && units.b[u] < 0 && units.bytes[u] == 8;
+}
+template <class L>
+constexpr int key_comp_in_work() {  // in-place: the work container's array that holds the cell keys (-1: scratch)
+    for (int c = 0; c < L::ncomp; ++c)
+        if (L::comp_size(c) == 4) return c;
+    return -1;
+}
 template <class L>
 struct BinPlan {
     static constexpr int kU = 1 + L::ncomp;
     size_t key0, hist, partial, dbase, ke, total;
     size_t unit_off[2][kU];
     int64_t ntiles, nchunks;
-    BinPlan(int64_t n, int npass) {
+    BinPlan(int64_t n, int npass, bool inplace) {
         constexpr Units<L, true> units{};
         ntiles = (n + kTileN - 1) / kTileN;
         if (ntiles < 1) ntiles = 1;
         nchunks = (ntiles + kScanRows - 1) / kScanRows;
         size_t o = 0;
         auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes ? bytes : 1, kAlign); return at; };
-        key0 = take(npass >= 2 ? 0 : (size_t)n * 4);  // with two or more passes the keys live in dst (see bin_permute_entry)
+        // with two or more passes the keys live in dst (see bin_permute_entry); in place: in the work container's first 4-byte array
+        key0 = take((inplace ? key_comp_in_work<L>() >= 0 : npass >= 2) ? 0 : (size_t)n * 4);
         for (int b = 0; b < 2; ++b)
-            for (int u = 0; u < kU; ++u)
-                unit_off[b][u] = take(b < npass - 1 && u < units.n ? (size_t)n * units.bytes[u] : 0);
+            for (int u = 0; u < kU; ++u) {
+                bool here = b < npass - 1 && u < units.n;
+                if (inplace) here = here && !unit_in_work<L>(u);
+                unit_off[b][u] = take(here ? (size_t)n * units.bytes[u] : 0);
+            }
         hist = take((size_t)ntiles * kRadix * 4);
         partial = take((size_t)nchunks * kRadix * 4);
         dbase = take(kRadix * 4);
@@ -738,9 +756,13 @@ struct BinPlan {
 };
 
 template <class L>
-size_t bin_scratch_bytes(int64_t n, int log2g) {
+size_t bin_scratch_bytes(int64_t n, int log2g, bool inplace) {
     if constexpr (!L::template has_as<pos_tag, double, 3>()) return 0;
-    else return BinPlan<L>(n, PassPlan(log2g, g_tune.bin_bits).npass).total;
+    else {
+        const int npass = PassPlan(log2g, g_tune.bin_bits).npass;
+        if (inplace && npass != 2) return 0;
+        return BinPlan<L>(n, npass, inplace).total;
+    }
 }
 
 template <class L, bool HAS_IDX, bool IN_PAIRED, bool OUT_PAIRED, bool DRIFT>
@@ -827,13 +849,17 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
         }
         const PassPlan pp(a.log2g, g_tune.bin_bits);
         const int npass = pp.npass;
-        const BinPlan<L> plan(n, npass);
+        if (a.inplace && npass != 2) return SOAX_ERR_UNSUPPORTED;  // the set returns to src after an even number of passes
+        const BinPlan<L> plan(n, npass, a.inplace);
         if (a.scratch_bytes < plan.total) return SOAX_ERR_ALLOC;
         char* sc = static_cast<char*>(a.scratch);
         // The cell keys are dead once the first pass has read them, and dst is not written before the last pass: with two
-        // or more passes the keys live in dst's own memory (its first component array of >= 4 bytes per element).
+        // or more passes the keys live in dst's own memory (its first component array of >= 4 bytes per element).  In place
+        // dst is the work container, whose 8-byte arrays hold intermediate units: the keys take its first 4-byte array.
         uint32_t* key0 = reinterpret_cast<uint32_t*>(sc + plan.key0);
-        if (npass >= 2) {
+        if (a.inplace) {
+            if constexpr (key_comp_in_work<L>() >= 0) key0 = static_cast<uint32_t*>(a.dst[key_comp_in_work<L>()]);
+        } else if (npass >= 2) {
             for (int c = 0; c < L::ncomp; ++c)
                 if (L::comp_size(c) >= 4) { key0 = static_cast<uint32_t*>(a.dst[c]); break; }
         }
@@ -841,10 +867,18 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
         uint32_t* partial = reinterpret_cast<uint32_t*>(sc + plan.partial);
         uint32_t* dbase = reinterpret_cast<uint32_t*>(sc + plan.dbase);
         double* kep = reinterpret_cast<double*>(sc + plan.ke);
-        const Ptrs<L::ncomp> src = make_ptrs<L>(a.src), dst = make_ptrs<L>(a.dst);
+        // in place the last pass writes the caller's src again (nothing reads src after the first pass)
+        const Ptrs<L::ncomp> src = make_ptrs<L>(a.src), dst = make_ptrs<L>(a.inplace ? a.src : a.dst);
         UnitPtrs<1 + L::ncomp> buf[2];
         for (int b = 0; b < 2; ++b)
             for (int u = 0; u < 1 + L::ncomp; ++u) buf[b].p[u] = sc + plan.unit_off[b][u];
+        if (a.inplace) {
+            constexpr Units<L, true> units{};
+            for_each_int<1 + L::ncomp>([&](auto ui) {
+                constexpr int u = decltype(ui)::value;
+                if constexpr (unit_in_work<L>(u)) buf[0].p[u] = a.dst[units.a[u]];
+            });
+        }
         const unsigned ntiles = (unsigned)plan.ntiles, nchunks = (unsigned)plan.nchunks;
         const bool has_idx = a.perm != nullptr;
 
@@ -906,7 +940,7 @@ int bin_permute_entry(const BinArgs& a, cudaStream_t st) {
 
 #define X(L)                                                               \
     template int bin_permute_entry<L>(const BinArgs&, cudaStream_t);      \
-    template size_t bin_scratch_bytes<L>(int64_t, int);
+    template size_t bin_scratch_bytes<L>(int64_t, int, bool);
 SOAX_FOR_EACH_LAYOUT(X)
 #undef X
 

@@ -41,9 +41,10 @@ struct BinArgs {
     void* const* src; void* const* dst; int64_t n; int log2g; double drift_dt;
     uint32_t* counts; uint32_t* offsets; uint32_t* perm; double* kinetic;
     void* scratch; size_t scratch_bytes;
+    bool inplace;  // soax_bin_permute_inplace: `dst` is a WORK container; the sorted set returns to src
 };
 template <class L> int bin_permute_entry(const BinArgs& a, cudaStream_t st);
-template <class L> size_t bin_scratch_bytes(int64_t n, int log2g);
+template <class L> size_t bin_scratch_bytes(int64_t n, int log2g, bool inplace);
 
 // NEXT-3 (container_kernels.cu)
 // Enqueues everything and returns: the survivor count is copied (asynchronously) into pin_n (pinned host memory) and, if

@@ -161,3 +161,14 @@ def test_config5_full_size_vs_oracle(gpu):
     ke = float(r["kinetic"].item())
     oke = oracle.energy(host, oracle.KINETIC)                        # the drift does not change vel
     assert abs(ke - oke) <= 1e-10 * oke and abs(ke / n - 1.5) < 1e-3
+    # the same call IN PLACE (soax_bin_permute_inplace: the set returns to src, dst is the work area) must reproduce what was
+    # just checked against the oracle, bit for bit, with half the scratch
+    del drifted, perm, ids
+    checked = dst.slab.clone()
+    assert B.soax_scratch_bytes_inplace(src.layout, n, G) < 0.51 * B.soax_scratch_bytes(src.layout, n, G)
+    r2 = src.bin_permute(dst, G, drift_dt=DT, want_kinetic=True, inplace=True)
+    torch.cuda.synchronize()
+    for k in ("counts", "offsets", "perm"):
+        assert torch.equal(r2[k], r[k]), k
+    assert float(r2["kinetic"].item()) == ke
+    assert src.n == n and torch.equal(src.slab, checked)             # same layout, same capacity: the slabs are images of each other

@@ -400,6 +400,55 @@ def test_bin_permute_optional_outputs(gpu, want):
         assert abs(float(kin.item()) - oke) <= 1e-10 * oke
 
 
+@pytest.mark.parametrize("n,G,drift", [(100003, 64, 0.0), (4097, 16, DT), (8191, 32, 0.0), (1, 64, DT), (0, 64, 0.0)])
+def test_bin_permute_inplace_r1(gpu, n, G, drift):
+    """soax_bin_permute_inplace: the sorted [drifted] set returns to the SAME container, the second one is a work area;
+    counts / offsets / perm / every array equal the oracle's, as for the out-of-place call; the scratch is smaller."""
+    torch, B, Cn = gpu
+    host = inputs.make_r1(n, seed=11)
+    s, work = to_device(Cn, Cn.R1, host), Cn.Soax(Cn.R1, max(n, 1))
+    need_in, need_out = B.soax_scratch_bytes_inplace(s.layout, max(n, 1), G), B.soax_scratch_bytes(s.layout, max(n, 1), G)
+    assert 0 < need_in <= need_out and (n < 4096 or need_out - need_in >= 23 * n)   # R1: 48 -> 24 bytes per particle (give or take the 256-byte alignment)
+    r = s.bin_permute(work, G, drift_dt=drift, want_kinetic=True, inplace=True)
+    torch.cuda.synchronize()
+    assert s.n == n
+    if n == 0:
+        assert int(r["counts"].sum()) == 0
+        return
+    after = oracle.drift(host, drift, 1) if drift else host
+    out = {k: r[k].cpu().numpy().view(np.uint32) for k in ("counts", "offsets", "perm")}
+    check_bin(after, s.download(), out, G)
+    oke = oracle.energy(host, oracle.KINETIC)
+    assert abs(float(r["kinetic"].item()) - oke) <= 1e-10 * max(oke, 1e-300)
+
+
+def test_bin_permute_inplace_r2_and_limits(gpu):
+    """the 13-array record in place (its 8-byte arrays travel through the work container, mass/charge as a pair and the
+    flags through scratch), without a carried index; grids that need one or three passes answer UNSUPPORTED."""
+    torch, B, Cn = gpu
+    n, G = 30011, 16
+    host = inputs.make_r2(n, seed=5)
+    host["acc"][:] = np.random.default_rng(3).normal(size=host["acc"].shape)
+    s, work = to_device(Cn, Cn.R2, host), Cn.Soax(Cn.R2, n)
+    scratch = torch.empty(B.soax_scratch_bytes_inplace(s.layout, n, G), dtype=torch.uint8, device="cuda")
+    counts = torch.empty(G ** 3, dtype=torch.int32, device="cuda")
+    B.soax_bin_permute_inplace(s.handle, work.handle, G, DT, counts.data_ptr(), None, None, None, scratch.data_ptr(), scratch.numel(),
+                               torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    drifted = oracle.drift(host, DT, 1)
+    as_r1 = {"id": np.zeros((1, n), np.int32), "pos": drifted["pos"], "vel": np.zeros((3, n), np.float32)}
+    exp = oracle.bin_r1(as_r1, G)
+    assert np.array_equal(counts.cpu().numpy().view(np.uint32), exp["counts"])
+    got = s.download()
+    for name in host:
+        assert np.array_equal(bits(got[name]), bits(drifted[name][:, exp["perm"]])), name
+    assert B.soax_scratch_bytes_inplace(s.layout, n, 8) == 0            # 9 key bits: one pass, the set would end in `work`
+    with pytest.raises(Exception):
+        B.soax_bin_permute_inplace(s.handle, work.handle, 8, 0.0, None, None, None, None, scratch.data_ptr(), scratch.numel(), 0)
+    with pytest.raises(Exception):                                       # a container cannot be its own work area
+        B.soax_bin_permute_inplace(s.handle, s.handle, G, 0.0, None, None, None, None, scratch.data_ptr(), scratch.numel(), 0)
+
+
 def test_bin_empty(gpu):
     torch, B, Cn = gpu
     host = inputs.make_r1(0, seed=1)
