@@ -296,9 +296,12 @@ def _extra_exchange(torch, B, Cn, s, peak, ex, gbs):
     """NEXT-4 on ONE GPU: the device-side pieces of the cross-GPU exchange, timed alone (no multi-GPU number exists).
     (1) The merge of 8 received runs (2^24 R1 records in all, each run sorted by cell on a 64^3 grid): one segmented gather
     (soax_gather_segments_aos, 80 B/particle) against what round 1 did (soax_aos_to_soa + a second soax_bin_permute).
-    (2) One migration step's local work at ~1 % leavers: two mask programs, the stable copy-out of the leavers, the
-    overwrite-with-last removal, and the sort of the leavers."""
+    (2) One migration step's local work at 2 % leavers: two mask programs, the stable copy-out of the leavers, the
+    overwrite-with-last removal, and the sort of the leavers.  Runs on its own uniformly filled set (2 % leavers)."""
     n, G, world = s.n, 64, 8
+    fresh = Cn.Soax(Cn.R1, n)                                        # uniform positions, whatever the headline run left in `s`
+    device_fill(torch, fresh, 3)
+    s = fresh
     sizes = [n // world] * world
     runs, cnts = [], []
     for q in range(world):
