@@ -296,7 +296,7 @@ def _extra_exchange(torch, B, Cn, s, peak, ex, gbs):
     """NEXT-4 on ONE GPU: the device-side pieces of the cross-GPU exchange, timed alone (no multi-GPU number exists).
     (1) The merge of 8 received runs (2^24 R1 records in all, each run sorted by cell on a 64^3 grid): one segmented gather
     (soax_gather_segments_aos, 80 B/particle) against what round 1 did (soax_aos_to_soa + a second soax_bin_permute).
-    (2) One migration step's local work at 2 % leavers: two mask programs, the stable copy-out of the leavers, the
+    (2) One migration step's local work at 2 % leavers: one mask program, the stable copy-out of the leavers, the
     overwrite-with-last removal, and the sort of the leavers.  Runs on its own uniformly filled set (2 % leavers)."""
     n, G, world = s.n, 64, 8
     fresh = Cn.Soax(Cn.R1, n)                                        # uniform positions, whatever the headline run left in `s`
@@ -338,16 +338,15 @@ def _extra_exchange(torch, B, Cn, s, peak, ex, gbs):
     # (2) migration, local part: this GPU owns cells [lo, hi) = the middle 98 % of the cell range after a drift
     lo, hi = int(0.01 * G ** 3), int(0.99 * G ** 3)
     cond_leave = f"(double(cell({G})) < lo) | (double(cell({G})) >= hi)"
-    cond_stay = f"(double(cell({G})) >= lo) & (double(cell({G})) < hi)"
-    leave, stay = Cn.MaskProgram(Cn.R1, cond_leave, ["lo", "hi"]), Cn.MaskProgram(Cn.R1, cond_stay, ["lo", "hi"])
+    leave = Cn.MaskProgram(Cn.R1, cond_leave, ["lo", "hi"])      # ONE mask: STABLE | KEEP_FLAGGED copies the leavers out, SWAP_LAST deletes them
     work, gone = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, 0, capacity=n)
-    m1, m2 = torch.empty(n, dtype=torch.uint8, device="cuda"), torch.empty(n, dtype=torch.uint8, device="cuda")
+    m1 = torch.empty(n, dtype=torch.uint8, device="cuda")
     rs = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
     rs2 = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
 
     work.copy_from(s)
-    ms_masks = ev_time_ms(torch, lambda: (leave.mask(work, out=m1, lo=lo, hi=hi), stay.mask(work, out=m2, lo=lo, hi=hi)), 10)
-    ms_out = ev_time_ms(torch, lambda: work.remove_async(m2, stable=True, dst=gone, scratch=rs), 10)
+    ms_masks = ev_time_ms(torch, lambda: leave.mask(work, out=m1, lo=lo, hi=hi), 10)
+    ms_out = ev_time_ms(torch, lambda: work.remove_async(m1, stable=True, dst=gone, scratch=rs, keep_flagged=True), 10)
     n_gone = gone.n
     ms_copy = ev_time_ms(torch, lambda: work.copy_from(s), 10)
 
@@ -359,7 +358,7 @@ def _extra_exchange(torch, B, Cn, s, peak, ex, gbs):
     ex["next4_exchange_local_work"] = {
         "n": n, "runs": world, "merge_segmented_gather_ms": ms_new, "merge_segmented_gather_GBps_80B": gbs(80, n, ms_new),
         "merge_round1_transpose_plus_sort_ms": ms_old, "merge_speedup": ms_old / ms_new, "merge_results_identical": bool(same),
-        "migration_local_ms": ms_mig, "migration_masks_ms": ms_masks, "migration_copy_out_leavers_ms": ms_out,
+        "migration_local_ms": ms_mig, "migration_mask_ms": ms_masks, "migration_copy_out_leavers_ms": ms_out,
         "migration_overwrite_with_last_ms": ms_swap, "migration_leavers": n_gone, "migration_particles_per_s": n / (ms_mig * 1e-3),
         "note": "device-side pieces of the multi-GPU exchange on one GPU; the collectives themselves are unmeasured on hardware"}
 

@@ -233,6 +233,10 @@ int soax_bin_permute_inplace(soax_t* s, soax_t* work, int32_t grid_dim, double d
  *                          row moves.
  *   SOAX_REMOVE_STABLE     order-preserving compaction into dst (same layout, no aliasing, capacity >= survivors;
  *                          s is left untouched).
+ *   | SOAX_REMOVE_KEEP_FLAGGED  (ORed to either mode) the mask marks the particles that STAY: a particle is removed iff its
+ *                          byte is ZERO.  One mask then serves both halves of a migration step (copy the leavers out:
+ *                          STABLE | KEEP_FLAGGED; delete them in place: SWAP_LAST) without a second pass that writes its
+ *                          complement.
  * The result is unique and deterministic for any mask.  The call is ASYNCHRONOUS like every other: the kernels read the
  * survivor count on the device, and the host learns it without a synchronisation in this call -- the stream copies it
  * into a pinned word owned by the target handle (s for SWAP_LAST, dst for STABLE) and records an event; the first later
@@ -244,7 +248,7 @@ int soax_bin_permute_inplace(soax_t* s, soax_t* work, int32_t grid_dim, double d
  * STABLE into a destination whose capacity is below the survivor count: dst receives the survivors that fit and its live
  * count becomes its capacity; *host_new_n still reports the true count (a capacity >= n can never overflow).
  * Errors: INVALID_ARG, ALLOC (scratch too small), UNSUPPORTED (n >= 2^32), CUDA. */
-typedef enum { SOAX_REMOVE_SWAP_LAST = 0, SOAX_REMOVE_STABLE = 1 } soax_remove_mode;
+typedef enum { SOAX_REMOVE_SWAP_LAST = 0, SOAX_REMOVE_STABLE = 1, SOAX_REMOVE_KEEP_FLAGGED = 4 } soax_remove_mode;
 size_t soax_remove_scratch_bytes(int64_t n);
 int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, void* dev_scratch, size_t scratch_bytes,
                 int64_t* host_new_n, void* stream);

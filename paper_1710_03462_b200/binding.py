@@ -17,7 +17,7 @@ SOAX_OK, SOAX_ERR_INVALID_ARG, SOAX_ERR_UNKNOWN_LAYOUT, SOAX_ERR_UNSUPPORTED, SO
 SOAX_I32, SOAX_I64, SOAX_U8, SOAX_F32, SOAX_F64 = 0, 1, 2, 3, 4
 SOAX_STEP_DRIFT, SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, SOAX_STEP_EULER_NOWRAP = 0, 1, 2, 3
 SOAX_ENERGY_KINETIC, SOAX_ENERGY_KINETIC_PLUS_HARMONIC = 0, 1
-SOAX_REMOVE_SWAP_LAST, SOAX_REMOVE_STABLE = 0, 1
+SOAX_REMOVE_SWAP_LAST, SOAX_REMOVE_STABLE, SOAX_REMOVE_KEEP_FLAGGED = 0, 1, 4
 DTYPE_SIZE = {SOAX_I32: 4, SOAX_I64: 8, SOAX_U8: 1, SOAX_F32: 4, SOAX_F64: 8}
 
 

@@ -160,14 +160,17 @@ class Soax:
         self.remove_async(kill, stable=stable, dst=dst, scratch=scratch)
         return (dst if stable else self).n                      # soax_size waits for the count, not for the rows
 
-    def remove_async(self, kill: torch.Tensor, stable: bool = False, dst: "Soax | None" = None, scratch: torch.Tensor | None = None) -> None:
-        """soax_remove without touching the count: nothing waits, the handle learns its new size when it is next needed."""
+    def remove_async(self, kill: torch.Tensor, stable: bool = False, dst: "Soax | None" = None, scratch: torch.Tensor | None = None,
+                     keep_flagged: bool = False) -> None:
+        """soax_remove without touching the count: nothing waits, the handle learns its new size when it is next needed.
+        keep_flagged: the mask marks the particles that STAY (SOAX_REMOVE_KEEP_FLAGGED)."""
         need = B.soax_remove_scratch_bytes(self.n)
         if scratch is None:
             scratch = torch.empty(max(need, 256), dtype=torch.uint8, device=self.slab.device)
         self._remove_scratch = scratch                          # keep it alive until the enqueued kernels have run
         B.soax_remove(self.handle, dst.handle if stable else None, kill.data_ptr(),
-                      B.SOAX_REMOVE_STABLE if stable else B.SOAX_REMOVE_SWAP_LAST, scratch.data_ptr(), scratch.numel(), _stream())
+                      (B.SOAX_REMOVE_STABLE if stable else B.SOAX_REMOVE_SWAP_LAST) | (B.SOAX_REMOVE_KEEP_FLAGGED if keep_flagged else 0),
+                      scratch.data_ptr(), scratch.numel(), _stream())
 
     def push_back_aos(self, aos: torch.Tensor, m: int) -> None:
         B.soax_push_back_aos(self.handle, aos.data_ptr(), m, _stream())

@@ -470,9 +470,10 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
     if (!s) return SOAX_ERR_INVALID_ARG;
     const int64_t n = live(s);
     if ((n > 0 && (!dev_kill || !dev_scratch)) || !aligned(dev_scratch, kAlign)) return SOAX_ERR_INVALID_ARG;
-    if (mode != SOAX_REMOVE_SWAP_LAST && mode != SOAX_REMOVE_STABLE) return SOAX_ERR_INVALID_ARG;
+    const int32_t base_mode = mode & ~SOAX_REMOVE_KEEP_FLAGGED;  // KEEP_FLAGGED: the mask marks the particles that stay
+    if (base_mode != SOAX_REMOVE_SWAP_LAST && base_mode != SOAX_REMOVE_STABLE) return SOAX_ERR_INVALID_ARG;
     if (n >= ((int64_t)1 << 32) || !s->layout->remove) return SOAX_ERR_UNSUPPORTED;
-    if (mode == SOAX_REMOVE_SWAP_LAST) {
+    if (base_mode == SOAX_REMOVE_SWAP_LAST) {
         if (dst) return SOAX_ERR_INVALID_ARG;  // in place
     } else {
         if (!dst || dst == s || dst->layout != s->layout) return SOAX_ERR_INVALID_ARG;
@@ -480,7 +481,7 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
             if (s->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
     }
     if (n > 0 && scratch_bytes < remove_scratch_bytes(n)) return SOAX_ERR_ALLOC;
-    soax_container* target = mode == SOAX_REMOVE_SWAP_LAST ? s : dst;
+    soax_container* target = base_mode == SOAX_REMOVE_SWAP_LAST ? s : dst;
     if (n == 0) {
         if (host_new_n) *host_new_n = 0;
         set_live(target, 0);

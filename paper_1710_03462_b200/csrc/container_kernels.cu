@@ -26,7 +26,8 @@ constexpr int kSegsPerTile = kCTile / kSeg;  // 16
 
 // ---- pass 1: flagged bytes per segment and per tile ----------------------------------------------------------------
 // thread t owns mask bytes [16 t, 16 t + 16) of the tile; 16 consecutive threads cover one segment
-__global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restrict__ kill, int64_t n, uint32_t* __restrict__ tile_count,
+// `flip` = 1 (SOAX_REMOVE_KEEP_FLAGGED): the mask marks the particles to KEEP; a row is removed iff (byte != 0) != flip.
+__global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restrict__ kill, int64_t n, uint32_t flip, uint32_t* __restrict__ tile_count,
                                                          uint32_t* __restrict__ seg_count) {
     __shared__ uint32_t sm[8];
     const int64_t b0 = (int64_t)blockIdx.x * kCTile + 16 * threadIdx.x;
@@ -37,10 +38,10 @@ __global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restri
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int b = 0; b < 4; ++b) c += ((w[i] >> (8 * b)) & 0xffu) != 0;
+            for (int b = 0; b < 4; ++b) c += (uint32_t)(((w[i] >> (8 * b)) & 0xffu) != 0) ^ flip;
     } else {
         for (int i = 0; i < 16; ++i)
-            if (b0 + i < n) c += kill[b0 + i] != 0;
+            if (b0 + i < n) c += (uint32_t)(kill[b0 + i] != 0) ^ flip;
     }
 #pragma unroll
     for (int o = 8; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);  // sum over the 16 threads of a segment
@@ -58,7 +59,7 @@ __global__ void __launch_bounds__(256) kill_count_kernel(const uint8_t* __restri
 // ---- pass 2 (one CTA): exclusive scan of the tile counts in place; info[0] = K = #flagged, info[1] = h = #flagged
 // below m = n - K (the holes of SWAP_LAST) ------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024) kill_scan_kernel(uint32_t* __restrict__ tile_count, int64_t ntiles, const uint8_t* __restrict__ kill,
-                                                         int64_t n, uint64_t* __restrict__ info, int64_t* __restrict__ host_count) {
+                                                         int64_t n, uint32_t flip, uint64_t* __restrict__ info, int64_t* __restrict__ host_count) {
     __shared__ uint32_t warp_sum[32];
     __shared__ uint32_t carry_sm;
     __shared__ uint32_t cnt_sm;
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(1024) kill_scan_kernel(uint32_t* __restrict__ 
     // flagged below m: the exclusive prefix of m's tile plus the flagged bytes of that tile before m
     const int64_t tm = m / kCTile;
     uint32_t c = 0;
-    for (int64_t e = tm * kCTile + threadIdx.x; e < m; e += 1024) c += kill[e] != 0;
+    for (int64_t e = tm * kCTile + threadIdx.x; e < m; e += 1024) c += (uint32_t)(kill[e] != 0) ^ flip;
     if (c) atomicAdd(&cnt_sm, c);  // integer: order does not matter
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -117,14 +118,14 @@ struct SegRank {
     uint32_t bal[kSegRounds];
     uint32_t before;
 };
-__device__ __forceinline__ SegRank seg_rank(const uint8_t* __restrict__ kill, int64_t n, int64_t seg, const uint32_t* __restrict__ tile_prefix,
-                                            const uint32_t* __restrict__ seg_count) {
+__device__ __forceinline__ SegRank seg_rank(const uint8_t* __restrict__ kill, int64_t n, uint32_t flip, int64_t seg,
+                                            const uint32_t* __restrict__ tile_prefix, const uint32_t* __restrict__ seg_count) {
     const int lane = threadIdx.x & 31;
     SegRank r;
     const int64_t e0 = seg * kSeg + lane;
     uint8_t f[kSegRounds];
 #pragma unroll
-    for (int k = 0; k < kSegRounds; ++k) f[k] = e0 + k * 32 < n ? kill[e0 + k * 32] : (uint8_t)0;
+    for (int k = 0; k < kSegRounds; ++k) f[k] = e0 + k * 32 < n ? (uint8_t)((uint32_t)(kill[e0 + k * 32] != 0) ^ flip) : (uint8_t)0;
     const int64_t tile = seg / kSegsPerTile;
     const int s_in = (int)(seg % kSegsPerTile);
     uint32_t c = lane < s_in ? seg_count[tile * kSegsPerTile + lane] : 0u;  // counts of the segments before this one
@@ -137,7 +138,7 @@ __device__ __forceinline__ SegRank seg_rank(const uint8_t* __restrict__ kill, in
 }
 
 // ---- SWAP_LAST: the slots to fill (flagged, below m) and the rows that fill them (surviving, at or above m) -----------
-__global__ void __launch_bounds__(256) holes_movers_kernel(const uint8_t* __restrict__ kill, int64_t n, const uint64_t* __restrict__ info,
+__global__ void __launch_bounds__(256) holes_movers_kernel(const uint8_t* __restrict__ kill, int64_t n, uint32_t flip, const uint64_t* __restrict__ info,
                                                            const uint32_t* __restrict__ tile_prefix, const uint32_t* __restrict__ seg_count,
                                                            uint32_t* __restrict__ holes, uint32_t* __restrict__ movers) {
     const int64_t m = n - (int64_t)info[0];  // survivors; read from the device so that the host need not wait for it
@@ -147,7 +148,7 @@ __global__ void __launch_bounds__(256) holes_movers_kernel(const uint8_t* __rest
     if (seg * kSeg >= n) return;
     const int lane = threadIdx.x & 31;
     const uint32_t lt = (1u << lane) - 1u;
-    const SegRank r = seg_rank(kill, n, seg, tile_prefix, seg_count);
+    const SegRank r = seg_rank(kill, n, flip, seg, tile_prefix, seg_count);
     uint32_t run = r.before;
 #pragma unroll
     for (int k = 0; k < kSegRounds; ++k) {
@@ -202,7 +203,7 @@ constexpr int kCompSmem = kCompStages * kCompStageBytes + kCTile * 2 /*inv*/ + 3
 
 template <class L>
 __global__ void __launch_bounds__(kCompThreads, 2) compact_ring_kernel(Ptrs<L::ncomp> src, Ptrs<L::ncomp> dst, const uint8_t* __restrict__ kill, int64_t n,
-                                                                      const uint32_t* __restrict__ tile_prefix, int64_t dst_capacity) {
+                                                                      uint32_t flip, const uint32_t* __restrict__ tile_prefix, int64_t dst_capacity) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* ring = smem;
     uint16_t* inv = reinterpret_cast<uint16_t*>(smem + kCompStages * kCompStageBytes);
@@ -246,13 +247,13 @@ __global__ void __launch_bounds__(kCompThreads, 2) compact_ring_kernel(Ptrs<L::n
             const uint2 m = *reinterpret_cast<const uint2*>(kill + r0);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                alive |= (((m.x >> (8 * i)) & 0xffu) == 0 ? 1u : 0u) << i;
-                alive |= (((m.y >> (8 * i)) & 0xffu) == 0 ? 1u : 0u) << (4 + i);
+                alive |= ((uint32_t)(((m.x >> (8 * i)) & 0xffu) == 0) ^ flip) << i;
+                alive |= ((uint32_t)(((m.y >> (8 * i)) & 0xffu) == 0) ^ flip) << (4 + i);
             }
         } else {
 #pragma unroll
             for (int i = 0; i < kCompItems; ++i)
-                if (r0 + i < n && kill[r0 + i] == 0) alive |= 1u << i;
+                if (r0 + i < n) alive |= ((uint32_t)(kill[r0 + i] == 0) ^ flip) << i;
         }
     }
     const uint32_t mine = __popc(alive);
@@ -395,10 +396,12 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
     uint64_t* info = reinterpret_cast<uint64_t*>(sc + plan.info);
     uint32_t* holes = reinterpret_cast<uint32_t*>(sc + plan.holes);
     uint32_t* movers = reinterpret_cast<uint32_t*>(sc + plan.movers);
-    kill_count_kernel<<<(unsigned)plan.ntiles, 256, 0, st>>>(kill, n, tile_count, seg_count);
+    const uint32_t flip = (mode & SOAX_REMOVE_KEEP_FLAGGED) ? 1u : 0u;
+    mode &= ~SOAX_REMOVE_KEEP_FLAGGED;
+    kill_count_kernel<<<(unsigned)plan.ntiles, 256, 0, st>>>(kill, n, flip, tile_count, seg_count);
     const unsigned seg_blocks = (unsigned)(((n + kSeg - 1) / kSeg + 7) / 8);  // 8 warps = 8 segments per CTA
     SOAX_TRY(launched());
-    kill_scan_kernel<<<1, 1024, 0, st>>>(tile_count, plan.ntiles, kill, n, info, pin_n);
+    kill_scan_kernel<<<1, 1024, 0, st>>>(tile_count, plan.ntiles, kill, n, flip, info, pin_n);
     SOAX_TRY(launched());
     // Nothing waits for the count, neither here nor on the device: the data kernels read it from `info`, and the scan
     // kernel itself stores it into the handle's mapped pinned word (no copy node in the stream); `count_ready` lets the
@@ -407,14 +410,14 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
     if (host_new_n) SOAX_CUDA(cudaMemcpyAsync(host_new_n, info + 2, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     SOAX_CUDA(cudaEventRecord(count_ready, st));
     if (mode == SOAX_REMOVE_SWAP_LAST) {
-        holes_movers_kernel<<<seg_blocks, 256, 0, st>>>(kill, n, info, tile_count, seg_count, holes, movers);
+        holes_movers_kernel<<<seg_blocks, 256, 0, st>>>(kill, n, flip, info, tile_count, seg_count, holes, movers);
         SOAX_TRY(launched());
         const unsigned blocks = (unsigned)((n / 2 + 255) / 256);  // #holes <= n / 2
         move_rows_kernel<L><<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(make_ptrs<L>(src), holes, movers, info);
         SOAX_TRY(launched());
     } else {
         SOAX_CUDA(cudaFuncSetAttribute(compact_ring_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCompSmem));
-        compact_ring_kernel<L><<<(unsigned)plan.ntiles, kCompThreads, kCompSmem, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, tile_count, dst_capacity);
+        compact_ring_kernel<L><<<(unsigned)plan.ntiles, kCompThreads, kCompSmem, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, flip, tile_count, dst_capacity);
         SOAX_TRY(launched());
     }
     return SOAX_OK;

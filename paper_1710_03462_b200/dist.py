@@ -196,9 +196,8 @@ class SoaxEngine:
         (per-cell counts of the leavers [ncell], the leavers sorted by cell as packed records, their number)."""
         G = self.grid_dim
         leave = self._mask(f"(double(cell({G})) < lo) | (double(cell({G})) >= hi)").mask(s, lo=lo, hi=hi)
-        stay = self._mask(f"(double(cell({G})) >= lo) & (double(cell({G})) < hi)").mask(s, lo=lo, hi=hi)
         out = self._Cn.Soax(s.fields, 0, capacity=max(s.n, 1))
-        s.remove_async(stay, stable=True, dst=out)                   # the leavers, in order
+        s.remove_async(leave, stable=True, dst=out, keep_flagged=True)   # the leavers, in order (the flagged ones are KEPT)
         s.remove_async(leave)                                        # PAPER.md:175: the holes are filled from the end
         m = out.n
         srt = self._Cn.Soax(s.fields, 0, capacity=max(m, 1))

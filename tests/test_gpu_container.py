@@ -61,6 +61,29 @@ def test_remove_matches_oracle(gpu, n):
         assert np.array_equal(image(s), base)                        # the source of a stable removal is untouched
 
 
+@pytest.mark.parametrize("n", [70001, 4097, 31])
+def test_remove_keep_flagged(gpu, n):
+    """SOAX_REMOVE_KEEP_FLAGGED: the mask marks the particles that STAY -- both modes equal the oracle run on the complemented
+    mask (any non-zero byte is a flag), and together with the plain call one mask splits a set into stayers and leavers."""
+    torch, B, Cn = gpu
+    host = inputs.make_r1(n, seed=n + 1)
+    base = oracle.r1_soa_to_aos(host)
+    for keep in masks(n, n + 7):
+        comp = (keep == 0).astype(np.uint8)                           # what the oracle is told to remove
+        kd = torch.from_numpy(keep).cuda()
+        s = device(Cn, Cn.R1, host)
+        s.remove_async(kd, keep_flagged=True)
+        assert s.n == int((keep != 0).sum())
+        assert np.array_equal(image(s), oracle.remove_swap_last(base, 40, comp))
+        s = device(Cn, Cn.R1, host)
+        kept, dropped = Cn.Soax(Cn.R1, 0, capacity=n), Cn.Soax(Cn.R1, 0, capacity=n)
+        s.remove_async(kd, stable=True, dst=kept, keep_flagged=True)
+        s.remove_async(kd, stable=True, dst=dropped)
+        assert kept.n + dropped.n == n
+        assert np.array_equal(image(kept), oracle.remove_stable(base, 40, comp))
+        assert np.array_equal(image(dropped), oracle.remove_stable(base, 40, keep))
+
+
 def test_remove_wide_record_and_errors(gpu):
     torch, B, Cn = gpu
     n = 20011
