@@ -16,11 +16,12 @@
 //               through the ring (src is never written), the last pass writes the caller's SoA.
 //   tile_hist   per-tile histogram of the next digit (later passes)                                  4 B read
 //   cell_bounds counts / offsets from the sorted positions by binary search per cell                 (small)
-// A 512-bin pass leaves runs of only ~8 elements per tile and bin, whose ragged ends are partial 32-byte sectors; the
-// L2 turns a partial-sector write into a DRAM read-modify-write unless the rest of the sector arrives within about a
-// microsecond (measured, profiles/r2_bin_study.md).  Wide-digit passes are therefore launched in THREAD-BLOCK CLUSTERS
-// of 4 CTAs that own neighbouring tiles and meet at a cluster barrier before every array's stores: the four pieces of
-// a bin's run reach the L2 together and merge into full sectors.
+// A 512-bin pass leaves runs of only ~8 elements per tile and bin, whose ragged ends are partial 32-byte sectors.  The L2
+// keeps a partly written sector until its other half arrives only while FEW are open (a few MB; an unsynchronised pass holds
+// ~1.8 M of them open and pays a DRAM read-modify-write for most), and DRAM reaches its copy rate only for contiguous pieces
+// of 256 bytes and more (both measured: profiles/r2_mem_probes.md).  Wide-digit passes are therefore launched in THREAD-BLOCK
+// CLUSTERS of 4 CTAs that own neighbouring tiles and meet at a cluster barrier before every array's stores: the four pieces
+// of a bin's run reach the L2 together, merge into full sectors, and leave for DRAM as one 256-byte piece.
 // Every step is a pure function of the data (no arrival-order atomics decide a position), so the result is the
 // unique stable permutation for ANY particle distribution, and bit-identical from run to run.
 #include <cstdio>
@@ -322,7 +323,8 @@ struct RingPlan {
 };
 
 // Time-synchronisation of the CTAs of a thread-block cluster (no memory ordering needed: it only makes the CTAs that
-// own neighbouring tiles write the pieces of a bin's run at the same moment, so that the L2 merges them into full sectors).
+// own neighbouring tiles write the pieces of a bin's run at the same moment, so that the L2 merges them into full sectors
+// while few partly written sectors are open: profiles/r2_mem_probes.md).
 __device__ __forceinline__ void cluster_sync_relaxed() {
     asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.aligned;" ::: "memory");
 }
