@@ -525,8 +525,12 @@ def _extra_config5(torch, B, Cn, peak, ex, gbs, iters):
                                  "round1_ms": 8.47}
     # the same pipeline IN PLACE (soax_bin_permute_inplace): the set returns to s5, d5 is the work area, scratch shrinks from 48
     # to 24 B/particle.  Every timed call gets the unsorted set again (restored outside the timed region).
-    del scratch
     backup = s5.slab.clone()
+    # the PIC steady state: re-binning a set that is already in cell order (d5 -> s5; no drift).  Same kernels, but a tile's
+    # particles now fall into a handful of bins, so the pieces it writes are long (profiles/r2_bin_study.md, last table).
+    ms_re = ev_time_ms(torch, lambda: d5.bin_permute(s5, 64, scratch=scratch), iters, 1)
+    ex["config5_bin_permute"]["rebin_of_sorted_set_ms"] = ms_re
+    del scratch
     scratch_in = torch.empty(B.soax_scratch_bytes_inplace(s5.layout, n5, 64), dtype=torch.uint8, device="cuda")
     times = []
     for it in range(iters + 1):
