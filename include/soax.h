@@ -39,7 +39,9 @@ typedef enum {
     SOAX_ERR_UNSUPPORTED = -3,    /* the operation needs a field (or a field type / dimension) the layout lacks:
                                      the run-time face of the paper's compile-time SFINAE check, PAPER.md:320   */
     SOAX_ERR_ALLOC = -4,          /* slab or scratch too small, or host allocation of a handle failed          */
-    SOAX_ERR_CUDA = -5            /* a CUDA runtime call failed; see soax_last_cuda_error()                     */
+    SOAX_ERR_CUDA = -5,           /* a CUDA runtime call failed; see soax_last_cuda_error()                     */
+    SOAX_ERR_TOO_LARGE = -6       /* more particles than the fixed work area of soax_remove_stable_noalloc holds
+                                     (SOAX_NOALLOC_MAX_N): use soax_remove with a scratch buffer of your own      */
 } soax_status;
 
 /* Element type of one field (id<int,1>, pos<double,3>, vel<double,3>, mass<float,1>). */
@@ -252,6 +254,39 @@ typedef enum { SOAX_REMOVE_SWAP_LAST = 0, SOAX_REMOVE_STABLE = 1, SOAX_REMOVE_KE
 size_t soax_remove_scratch_bytes(int64_t n);
 int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, void* dev_scratch, size_t scratch_bytes,
                 int64_t* host_new_n, void* stream);
+/* Stable removal for callers that have NO device memory to offer as scratch and no means of getting any.
+ * soax_remove leaves the scratch to the caller, which suits a host program that manages its own memory.  It does not suit
+ * code that is merely handed the particle arrays: a diagnostics or load-balancing hook called from inside somebody else's
+ * time step, where a cudaMalloc would stall every stream of the device and the memory budget belongs to the host code; a
+ * simulation that has already given the whole of HBM to its particle slabs, so that an allocation would simply fail; a
+ * plugin interface that passes device pointers through but exposes no allocator.  For those there is this ONE entry point,
+ * which allocates nothing -- no device memory, no pinned memory, no event, on any call: its work area (per-tile and
+ * per-segment counts of the mask, 68 bytes per 4096 rows) is an array compiled into the library, about 0.27 MB that every
+ * GPU using the library keeps until the process ends.  That fixes the largest set it can serve:
+ *     live(s) <= SOAX_NOALLOC_MAX_N = 2^24 particles; anything larger answers SOAX_ERR_TOO_LARGE and enqueues nothing.
+ * What it computes is soax_remove(s, dst, dev_kill, SOAX_REMOVE_STABLE [| SOAX_REMOVE_KEEP_FLAGGED], ...) with the same
+ * kernels: dst (same layout as s, no array shared with s) receives the surviving rows of s in their original order, s is
+ * left as it was.  keep_flagged = 0: a non-zero mask byte removes the row; != 0: a non-zero byte keeps it.
+ * Differences from soax_remove, all of them consequences of not allocating:
+ *   - the survivor count is written to *dev_new_n, one int64 in DEVICE memory of the caller (required, 8-byte aligned);
+ *     the handle-owned pinned word and event through which soax_remove reports it lazily would have to be created;
+ *   - therefore dst's live count is NOT changed by this call.  Once the stream has passed the call (after the caller's own
+ *     synchronisation or a copy of the word), set it with soax_resize(dst, min(count, capacity of dst)).  As with
+ *     soax_remove, a destination smaller than the survivor count receives the survivors that fit, and the word still holds
+ *     the true count;
+ *   - the very first call on each device looks up the device address of the work area (one cudaGetSymbolAddress, with the
+ *     caller's current device; nothing is allocated by it).  Make that first call outside any stream capture, and with the
+ *     device that owns the containers current; later calls on that device only launch kernels;
+ *   - ALL calls on one device share the one work area, which still holds whatever the previous call left in it.  Nothing
+ *     in it needs clearing (each call overwrites every entry it reads later), but two calls whose kernels can run at the
+ *     same time -- different streams without an ordering between them, or two host threads -- overwrite each other's
+ *     counts and produce garbage.  Keep the calls of one device on one stream, or order them with events.
+ * Errors: INVALID_ARG (null or aliasing handles, different layouts, null mask with n > 0, null or misaligned dev_new_n),
+ * TOO_LARGE, UNSUPPORTED (layout without compiled kernels; device ordinal >= 64), CUDA.  n = 0 enqueues one 8-byte memset of
+ * *dev_new_n and nothing else. */
+#define SOAX_NOALLOC_MAX_N 16777216 /* 2^24 */
+int soax_remove_stable_noalloc(const soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t keep_flagged, int64_t* dev_new_n,
+                               void* stream);
 /* push_back of m particle objects (PAPER.md:304-307 `soax.push_back(particle)`): m packed AoS records (see
  * soax_layout_aos, 16-byte aligned) are appended behind the live particles; the live count grows by m.
  * ALLOC if n + m exceeds the capacity (the caller owns the memory: to regrow, soax_alloc a larger slab and

@@ -14,6 +14,8 @@ from typing import Sequence
 from . import build as _build
 
 SOAX_OK, SOAX_ERR_INVALID_ARG, SOAX_ERR_UNKNOWN_LAYOUT, SOAX_ERR_UNSUPPORTED, SOAX_ERR_ALLOC, SOAX_ERR_CUDA = 0, -1, -2, -3, -4, -5
+SOAX_ERR_TOO_LARGE = -6
+SOAX_NOALLOC_MAX_N = 1 << 24
 SOAX_I32, SOAX_I64, SOAX_U8, SOAX_F32, SOAX_F64 = 0, 1, 2, 3, 4
 SOAX_STEP_DRIFT, SOAX_STEP_SYMPLECTIC_EULER_HARMONIC, SOAX_STEP_RK2_MIDPOINT_HARMONIC_MASKED, SOAX_STEP_EULER_NOWRAP = 0, 1, 2, 3
 SOAX_ENERGY_KINETIC, SOAX_ENERGY_KINETIC_PLUS_HARMONIC = 0, 1
@@ -71,6 +73,7 @@ SIGNATURES = {
     "soax_gather_segments_aos": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _i64, _vp]),
     "soax_remove_scratch_bytes": (_sz, [_i64]),
     "soax_remove": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _sz, C.POINTER(_i64), _vp]),
+    "soax_remove_stable_noalloc": (C.c_int, [_vp, _vp, _vp, _i32, _vp, _vp]),
     "soax_push_back_aos": (C.c_int, [_vp, _vp, _i64, _vp]),
     "soax_get_elements": (C.c_int, [_vp, _vp, _i64, _vp, _vp]),
     "soax_copy": (C.c_int, [_vp, _vp, _vp]),
@@ -266,6 +269,13 @@ def soax_remove(s: int, dst: int | None, dev_kill: int, mode: int, dev_scratch: 
     the count ready).  host_new_n: optional address of a PINNED int64 that also receives the survivor count."""
     ptr = C.cast(host_new_n, C.POINTER(_i64)) if host_new_n else None
     _check(lib().soax_remove(s, dst, dev_kill, mode, dev_scratch, scratch_bytes, ptr, stream), "soax_remove")
+
+
+def soax_remove_stable_noalloc(s: int, dst: int, dev_kill: int, keep_flagged: bool, dev_new_n: int, stream: int = 0) -> None:
+    """The stable removal for callers that cannot allocate (see include/soax.h): no scratch argument, nothing allocated by
+    the library either; at most SOAX_NOALLOC_MAX_N particles (SoaxError with status SOAX_ERR_TOO_LARGE beyond).  The
+    survivor count lands in the int64 DEVICE word dev_new_n; dst's live count is left for the caller to set (soax_resize)."""
+    _check(lib().soax_remove_stable_noalloc(s, dst, dev_kill, 1 if keep_flagged else 0, dev_new_n, stream), "soax_remove_stable_noalloc")
 
 
 def soax_push_back_aos(s: int, dev_aos: int, m: int, stream: int = 0) -> None:

@@ -172,6 +172,15 @@ class Soax:
                       (B.SOAX_REMOVE_STABLE if stable else B.SOAX_REMOVE_SWAP_LAST) | (B.SOAX_REMOVE_KEEP_FLAGGED if keep_flagged else 0),
                       scratch.data_ptr(), scratch.numel(), _stream())
 
+    def remove_stable_noalloc(self, kill: torch.Tensor, dst: "Soax", count: torch.Tensor, keep_flagged: bool = False) -> None:
+        """soax_remove_stable_noalloc: the stable removal for callers that may not allocate -- no scratch is passed and the
+        library allocates none (its work area is built into libsoax.so; at most B.SOAX_NOALLOC_MAX_N particles).  `count`:
+        a one-element int64 device tensor of the caller that receives the survivor count; dst's live count is NOT updated
+        (that needs the count on the host): after synchronising, call B.soax_resize(dst.handle, int(count))."""
+        assert kill.dtype == torch.uint8 and kill.is_contiguous() and kill.numel() >= self.n
+        assert count.dtype == torch.int64 and count.is_cuda and count.numel() >= 1
+        B.soax_remove_stable_noalloc(self.handle, dst.handle, kill.data_ptr(), keep_flagged, count.data_ptr(), _stream())
+
     def push_back_aos(self, aos: torch.Tensor, m: int) -> None:
         B.soax_push_back_aos(self.handle, aos.data_ptr(), m, _stream())
 

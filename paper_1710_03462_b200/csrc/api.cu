@@ -36,6 +36,7 @@ struct soax_layout {
     size_t (*bin_scratch)(int64_t, int, bool);
     int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t);
     int (*gather_rows)(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
+    int (*remove_stable_noalloc)(void* const*, void* const*, const uint8_t*, int64_t, uint32_t, int64_t, int64_t*, cudaStream_t);
 };
 
 // A captured loop of `nlaunch` kernel launches, replayed while the call that made it is repeated unchanged: small
@@ -153,6 +154,7 @@ soax_layout describe(const char* name) {
     d.bin_scratch = &bin_scratch_bytes<L>;
     d.remove = &remove_entry<L>;
     d.gather_rows = &gather_rows_entry<L>;
+    d.remove_stable_noalloc = &remove_stable_noalloc_entry<L>;
     return d;
 }
 
@@ -500,6 +502,25 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
     return SOAX_OK;
 }
 
+// The one entry point that allocates nothing (see soax.h): no pinned word, no event, scratch inside the library image.  It reads
+// the live count of s the usual way but leaves dst's count to the caller, who learns the survivor count from *dev_new_n.
+int soax_remove_stable_noalloc(const soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t keep_flagged, int64_t* dev_new_n,
+                               void* stream) {
+    if (!s || !dst || dst == s || dst->layout != s->layout || !dev_new_n || !aligned(dev_new_n, 8)) return SOAX_ERR_INVALID_ARG;
+    const int64_t n = live(s);
+    if (n > 0 && !dev_kill) return SOAX_ERR_INVALID_ARG;
+    if (!s->layout->remove_stable_noalloc) return SOAX_ERR_UNSUPPORTED;
+    for (int c = 0; c < s->layout->ncomp; ++c)
+        if (s->comp[c] == dst->comp[c]) return SOAX_ERR_INVALID_ARG;
+    if (n > SOAX_NOALLOC_MAX_N) return SOAX_ERR_TOO_LARGE;  // the work area compiled into the library holds counts for 2^24 rows
+    if (n == 0) {
+        SOAX_CUDA(cudaMemsetAsync(dev_new_n, 0, sizeof(int64_t), (cudaStream_t)stream));
+        return SOAX_OK;
+    }
+    return s->layout->remove_stable_noalloc(s->comp, dst->comp, dev_kill, n, keep_flagged ? 1u : 0u, dst->capacity, dev_new_n,
+                                            (cudaStream_t)stream);
+}
+
 int soax_push_back_aos(soax_t* s, const void* dev_aos, int64_t m, void* stream) {
     if (!s || m < 0 || (m > 0 && !dev_aos) || !aligned(dev_aos, 16)) return SOAX_ERR_INVALID_ARG;
     if (!s->layout->aos_to_soa) return SOAX_ERR_UNSUPPORTED;
@@ -633,6 +654,7 @@ const char* soax_strerror(int status) {
         case SOAX_ERR_UNSUPPORTED: return "operation not supported by this layout (missing field, wrong type or dimension)";
         case SOAX_ERR_ALLOC: return "buffer too small or host allocation failed";
         case SOAX_ERR_CUDA: return "CUDA runtime error (see soax_last_cuda_error)";
+        case SOAX_ERR_TOO_LARGE: return "more particles than the built-in work area of soax_remove_stable_noalloc holds (SOAX_NOALLOC_MAX_N = 2^24): use soax_remove with your own scratch";
         default: return "unknown status";
     }
 }

@@ -13,6 +13,8 @@
 // one-CTA scan turns the tile counts into prefixes.  The stable compaction takes a tile per CTA through a TMA ring and writes
 // 16-byte vectors (compact_ring_kernel); the in-place removal ranks holes and movers per warp-owned segment without shared
 // memory or CTA barriers and then moves one row per thread.
+#include <mutex>
+
 #include "common.cuh"
 #include "ops.hpp"
 #include "tma.cuh"
@@ -433,7 +435,69 @@ int gather_rows_entry(void* const* comps, int64_t n, const uint32_t* idx, int64_
     return launched();
 }
 
+// ---- stable removal without a scratch buffer from the caller (soax_remove_stable_noalloc) -------------------------------------
+// The per-tile and per-segment counts of the mask and the three result words of the scan are the only scratch the stable
+// compaction needs (68 bytes per tile of 4096 rows; holes and movers belong to SWAP_LAST only).  For callers that have no
+// way of providing device memory for them, that scratch lives HERE, in an array that is part of the library image: every
+// GPU that loads libsoax.so holds these kStaticScratchBytes (about 0.27 MB) until the process exits.  Layout of the array
+// (every piece 256-byte aligned): tile counts for kNoAllocMaxN rows | segment counts | info[3].
+constexpr int64_t kNoAllocMaxN = (int64_t)1 << 24;                    // SOAX_NOALLOC_MAX_N of soax.h
+constexpr size_t kStaticTiles = (size_t)(kNoAllocMaxN / kCTile);      // 4096
+constexpr size_t kStaticTileOff = 0;
+constexpr size_t kStaticSegOff = kStaticTileOff + kStaticTiles * 4;                  // 16 KB of tile counts before it
+constexpr size_t kStaticInfoOff = kStaticSegOff + kStaticTiles * kSegsPerTile * 4;   // 256 KB of segment counts before it
+constexpr size_t kStaticScratchBytes = kStaticInfoOff + kAlign;
+static_assert(kStaticSegOff % kAlign == 0 && kStaticInfoOff % kAlign == 0, "pieces of the static scratch start on 256-byte boundaries");
+static_assert(SOAX_NOALLOC_MAX_N == kNoAllocMaxN, "soax.h states the limit this array was sized for");
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+// In HOST code the name g_static_scratch is only a handle for the runtime, not an address a kernel could use: the device
+// address has to be asked for, per device, with that device current.  Done once per device, at the first call there.
+constexpr int kMaxDevices = 64;
+static std::mutex g_static_mu;
+static unsigned char* g_static_ptr[kMaxDevices] = {};
+
+static int static_scratch(unsigned char** out) {
+    int dev = -1;
+    SOAX_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return SOAX_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        SOAX_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));  // the copy of the array that lives on the current device
+        if (!p) return SOAX_ERR_CUDA;
+        g_static_ptr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_static_ptr[dev];
+    return SOAX_OK;
+}
+
+// The same three kernels, in the same order and launch shapes, as the STABLE branch of remove_entry; only where the counts
+// live differs, and the survivor count goes to the caller's device word instead of a pinned word of the handle (creating
+// that word and its event would allocate).  Nothing in the array has to start at zero: kill_count_kernel writes the count
+// of every tile and of every segment of [0, n) before anything reads them, the scan writes info, and entries past this
+// call's tiles -- left over from an earlier, larger call -- are never read.
+template <class L>
+int remove_stable_noalloc_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, uint32_t flip, int64_t dst_capacity,
+                                int64_t* dev_new_n, cudaStream_t st) {
+    if (n > kNoAllocMaxN) return SOAX_ERR_TOO_LARGE;
+    unsigned char* sc = nullptr;
+    SOAX_TRY(static_scratch(&sc));
+    uint32_t* tile_count = reinterpret_cast<uint32_t*>(sc + kStaticTileOff);
+    uint32_t* seg_count = reinterpret_cast<uint32_t*>(sc + kStaticSegOff);
+    uint64_t* info = reinterpret_cast<uint64_t*>(sc + kStaticInfoOff);
+    const int64_t ntiles = (n + kCTile - 1) / kCTile;
+    kill_count_kernel<<<(unsigned)ntiles, 256, 0, st>>>(kill, n, flip, tile_count, seg_count);
+    SOAX_TRY(launched());
+    kill_scan_kernel<<<1, 1024, 0, st>>>(tile_count, ntiles, kill, n, flip, info, dev_new_n);
+    SOAX_TRY(launched());
+    SOAX_CUDA(cudaFuncSetAttribute(compact_ring_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCompSmem));
+    compact_ring_kernel<L><<<(unsigned)ntiles, kCompThreads, kCompSmem, st>>>(make_ptrs<L>(src), make_ptrs<L>(dst), kill, n, flip, tile_count, dst_capacity);
+    return launched();
+}
+
 #define X(L)                                                                                                                  \
+    template int remove_stable_noalloc_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, uint32_t, int64_t, int64_t*, cudaStream_t); \
     template int remove_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t); \
     template int gather_rows_entry<L>(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
 SOAX_FOR_EACH_LAYOUT(X)

@@ -52,6 +52,10 @@ template <class L> size_t bin_scratch_bytes(int64_t n, int log2g, bool inplace);
 template <class L> int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch,
                                     const int64_t** dev_count, int64_t dst_capacity, int64_t* pin_n, int64_t* host_new_n,
                                     cudaEvent_t count_ready, cudaStream_t st);
+// The STABLE removal with its scratch in a file-scope device array of container_kernels.cu (soax_remove_stable_noalloc): no
+// device, pinned or event allocation anywhere on the path; the survivor count goes to dev_new_n (device memory).
+template <class L> int remove_stable_noalloc_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, uint32_t flip,
+                                                   int64_t dst_capacity, int64_t* dev_new_n, cudaStream_t st);
 template <class L> int gather_rows_entry(void* const* comps, int64_t n, const uint32_t* idx, int64_t m, void* aos, cudaStream_t st);
 size_t remove_scratch_bytes(int64_t n);
 
