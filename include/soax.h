@@ -102,7 +102,9 @@ size_t soax_slab_bytes(const soax_layout* layout, int64_t capacity);
 int soax_alloc(const soax_layout* layout, int64_t n, int64_t capacity, void* dev_slab, size_t slab_bytes,
                soax_t** out);
 int soax_free(soax_t* s);
-/* Live particle count; resize within capacity (PAPER.md:296 resize; no regrow, no data movement). */
+/* Live particle count; resize within capacity (PAPER.md:296 resize; no data movement).  Regrow is a CALLER-SIDE operation,
+ * because the caller owns device memory: soax_alloc over a larger slab, soax_copy, soax_free of the old handle -- the Python
+ * container does exactly that in Soax.reserve() / resize() / push_back_aos() with a growth factor of 1.5. */
 int64_t soax_size(const soax_t* s);
 int soax_resize(soax_t* s, int64_t n);
 /* Device pointer of one component array: field f, component c -- the paper's posArr(c).
@@ -175,7 +177,10 @@ int soax_soa_to_aos(const soax_t* src, void* dev_aos, int64_t n, void* stream);
  * non-decreasing (an empty segment repeats the next start); both tables are uint32 device arrays built by the caller from
  * counts (paper_1710_03462_b200/dist.py builds them from the all-gathered per-cell counts, so that `world` runs that are
  * each sorted by cell merge into one set sorted by (cell, run, position): one pass of 40 B read + 40 B written per particle
- * instead of a transpose plus a full sort).  Source records are not range-checked.  dst's live count becomes n. */
+ * instead of a transpose plus a full sort).  The tables are trusted, on purpose (the call does not know how many records
+ * dev_aos holds): a dev_seg_src entry that points past the source is the caller's error and reads out of bounds.  Only the
+ * index arithmetic is made safe -- rows in front of dev_seg_dst[0] (a table that does not start at 0) are served from
+ * segment 0 with offset 0, never from a negative index.  dst's live count becomes n. */
 int soax_gather_segments_aos(soax_t* dst, const void* dev_aos, const uint32_t* dev_seg_dst, const uint32_t* dev_seg_src,
                              int64_t nseg, int64_t n, void* stream);
 
@@ -240,12 +245,16 @@ int soax_bin_permute_inplace(soax_t* s, soax_t* work, int32_t grid_dim, double d
  *                          STABLE | KEEP_FLAGGED; delete them in place: SWAP_LAST) without a second pass that writes its
  *                          complement.
  * The result is unique and deterministic for any mask.  The call is ASYNCHRONOUS like every other: the kernels read the
- * survivor count on the device, and the host learns it without a synchronisation in this call -- the stream copies it
- * into a pinned word owned by the target handle (s for SWAP_LAST, dst for STABLE) and records an event; the first later
- * call that needs that handle's live count on the host (soax_size, or any call that launches over its particles) waits for
- * that one event, which completes after the two small counting kernels, not after the rows have moved.  host_new_n:
- * optional HOST pointer (NULL allowed) that also receives the survivor count by an asynchronous copy on `stream`; it must be
- * pinned memory for the copy to be asynchronous, and may be read after the caller has synchronised the stream.
+ * survivor count on the device, and the host learns it without a synchronisation in this call -- the counting kernel stores
+ * it into a mapped pinned word owned by the target handle (s for SWAP_LAST, dst for STABLE) and the stream records an event;
+ * the first later call that needs that handle's live count on the host (soax_size, or any call that launches over its
+ * particles) waits for that one event, which completes after the two small counting kernels, not after the rows have moved.
+ * While such a count is pending, use the target handle from ONE host thread only (the calls documented as read-only resolve
+ * the count, i.e. write the handle); a call that gives the handle a new count (soax_resize, soax_upload, ...) first waits for
+ * the pending one.  host_new_n: optional HOST pointer (NULL allowed) that also receives the survivor count by a
+ * cudaMemcpyAsync on `stream`; give it PINNED memory -- with a pageable pointer that copy BLOCKS the host until both counting
+ * kernels have run, which makes the call synchronous without any other sign; read it after synchronising the stream.
+ * UNSUPPORTED while `stream` is being captured into a CUDA graph (the count event would never fire).
  * dev_scratch: >= soax_remove_scratch_bytes(n) bytes, 256-byte aligned; it must stay valid until the enqueued work is done.
  * STABLE into a destination whose capacity is below the survivor count: dst receives the survivors that fit and its live
  * count becomes its capacity; *host_new_n still reports the true count (a capacity >= n can never overflow).

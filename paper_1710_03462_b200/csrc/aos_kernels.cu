@@ -482,7 +482,7 @@ __global__ void __launch_bounds__(kGatherThreads) gather_segments_kernel(Ptrs<L:
             const int64_t mid = (lo + hi) >> 1;
             if ((int64_t)seg_dst[mid] <= j) lo = mid + 1; else hi = mid;
         }
-        return lo - 1;
+        return lo > 0 ? lo - 1 : 0;  // a table that does not start at row 0 is served from segment 0, not from index -1
     };
     if (threadIdx.x < 2) {
         const int64_t i = last_le(threadIdx.x == 0 ? j0 : j1 - 1);
@@ -509,10 +509,13 @@ __global__ void __launch_bounds__(kGatherThreads) gather_segments_kernel(Ptrs<L:
                 const int mid = (lo + hi) >> 1;
                 if ((int64_t)s_dst[mid] <= j) lo = mid + 1; else hi = mid;
             }
-            src_row = (int64_t)s_src[lo - 1] + (j - (int64_t)s_dst[lo - 1]);
+            const int i = lo > 0 ? lo - 1 : 0;
+            const int64_t off = j - (int64_t)s_dst[i];
+            src_row = (int64_t)s_src[i] + (off > 0 ? off : 0);
         } else {
             const int64_t i = last_le(j);
-            src_row = (int64_t)seg_src[i] + (j - (int64_t)seg_dst[i]);
+            const int64_t off = j - (int64_t)seg_dst[i];
+            src_row = (int64_t)seg_src[i] + (off > 0 ? off : 0);
         }
         const unsigned char* rec = aos + src_row * L::aos_stride;
         constexpr int kGroup = 16;

@@ -34,7 +34,7 @@ struct soax_layout {
     int (*energy)(void* const*, int64_t, int, double, double, void*, double*, cudaStream_t);
     int (*bin_permute)(const BinArgs&, cudaStream_t);
     size_t (*bin_scratch)(int64_t, int, bool);
-    int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t);
+    int (*remove)(void* const*, void* const*, const uint8_t*, int64_t, int, void*, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t);
     int (*gather_rows)(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
     int (*remove_stable_noalloc)(void* const*, void* const*, const uint8_t*, int64_t, uint32_t, int64_t, int64_t*, cudaStream_t);
 };
@@ -96,9 +96,10 @@ struct soax_container {
     void* comp[kMaxComp];
     uint64_t serial;  // unique per soax_alloc: part of every graph key
     GraphCache graph;
-    // A live count that a kernel is still computing (soax_remove): the stream copies it into `pin_n` (pinned host
-    // memory owned by the handle) and records `n_event`; the first later call that needs the count on the host waits for
-    // that one event -- the count is ready after two small kernels, long before the rows have moved.
+    // A live count that a kernel is still computing (soax_remove): the scan kernel stores it straight into `pin_n` (mapped
+    // pinned host memory owned by the handle, -1 while nothing has landed) and the stream records `n_event`; the first later
+    // call that needs the count on the host waits for that one event -- the count is ready after two small kernels, long
+    // before the rows have moved.  One pending count per handle, resolved by one host thread: see soax.h.
     mutable bool n_pending = false;
     int64_t* pin_n = nullptr;
     cudaEvent_t n_event = nullptr;
@@ -107,15 +108,24 @@ struct soax_container {
 // live particle count of a handle, resolving a pending one
 static int64_t live(const soax_container* s) {
     if (s->n_pending) {
-        cudaEventSynchronize(s->n_event);
-        int64_t m = *s->pin_n;
-        if (m > s->capacity) m = s->capacity;  // STABLE into too small a destination: it holds the survivors that fit
-        const_cast<soax_container*>(s)->n = m;
+        const cudaError_t e = cudaEventSynchronize(s->n_event);
+        const int64_t m = *s->pin_n;
+        // The word holds -1 until the scan kernel has stored the count: a kernel that faulted, or an event that never really
+        // fired, must not turn a stale word into the live count.  On failure the handle keeps the count it had and the CUDA
+        // error is left for soax_last_cuda_error().
+        if (e == cudaSuccess && m >= 0) const_cast<soax_container*>(s)->n = m > s->capacity ? s->capacity : m;  // STABLE into too small a destination holds the survivors that fit
+        else if (e != cudaSuccess) cuda_fail(e);
         s->n_pending = false;
     }
     return s->n;
 }
-static void set_live(soax_container* s, int64_t n) { s->n = n; s->n_pending = false; }
+// A count that is still on its way targets pin_n: let it land (and be discarded) before the handle is given a new one, so that
+// a later soax_remove on another stream never has two kernels writing that word unordered.
+static void set_live(soax_container* s, int64_t n) {
+    if (s->n_pending) cudaEventSynchronize(s->n_event);
+    s->n = n;
+    s->n_pending = false;
+}
 
 static std::string container_key(const soax_container* s) {
     std::string k;
@@ -489,14 +499,24 @@ int soax_remove(soax_t* s, soax_t* dst, const uint8_t* dev_kill, int32_t mode, v
         set_live(target, 0);
         return SOAX_OK;
     }
-    if (!target->pin_n) {
-        SOAX_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&target->pin_n), sizeof(int64_t), cudaHostAllocMapped | cudaHostAllocPortable));
-        SOAX_CUDA(cudaEventCreateWithFlags(&target->n_event, cudaEventDisableTiming));
+    // The count travels through an event this call records and a later call waits for on the host: inside a stream capture
+    // the event would never fire and the handle would read a stale word.
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing((cudaStream_t)stream, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+    if (cs != cudaStreamCaptureStatusNone) return SOAX_ERR_UNSUPPORTED;
+    if (!target->pin_n) {  // the event first: a handle never has the word without the event that guards it
+        cudaEvent_t ev = nullptr;
+        SOAX_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        int64_t* word = nullptr;
+        const cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&word), sizeof(int64_t), cudaHostAllocMapped | cudaHostAllocPortable);
+        if (e != cudaSuccess) { cudaEventDestroy(ev); return cuda_fail(e); }
+        target->n_event = ev;
+        target->pin_n = word;
     } else if (target->n_pending) {
         live(target);  // an earlier pending count still targets pin_n: let it land before the word is reused
     }
-    const int64_t* dev_m = nullptr;
-    SOAX_TRY(s->layout->remove(s->comp, dst ? dst->comp : nullptr, dev_kill, n, mode, dev_scratch, &dev_m, dst ? dst->capacity : 0,
+    *target->pin_n = -1;  // "nothing has landed yet" (the kernels of this call are enqueued after this store)
+    SOAX_TRY(s->layout->remove(s->comp, dst ? dst->comp : nullptr, dev_kill, n, mode, dev_scratch, dst ? dst->capacity : 0,
                                target->pin_n, host_new_n, target->n_event, (cudaStream_t)stream));
     target->n_pending = true;
     return SOAX_OK;

@@ -389,7 +389,7 @@ struct RemovePlan {
 size_t remove_scratch_bytes(int64_t n) { return RemovePlan(n).total; }
 
 template <class L>
-int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch, const int64_t** dev_count,
+int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch,
                  int64_t dst_capacity, int64_t* pin_n, int64_t* host_new_n, cudaEvent_t count_ready, cudaStream_t st) {
     const RemovePlan plan(n);
     char* sc = static_cast<char*>(scratch);
@@ -408,7 +408,8 @@ int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_
     // Nothing waits for the count, neither here nor on the device: the data kernels read it from `info`, and the scan
     // kernel itself stores it into the handle's mapped pinned word (no copy node in the stream); `count_ready` lets the
     // handle pick it up later.
-    *dev_count = reinterpret_cast<const int64_t*>(info + 2);
+    // The caller's own word is the one thing that goes through a copy node; from pageable memory that copy blocks the host
+    // until both count kernels have run (soax.h says so).
     if (host_new_n) SOAX_CUDA(cudaMemcpyAsync(host_new_n, info + 2, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     SOAX_CUDA(cudaEventRecord(count_ready, st));
     if (mode == SOAX_REMOVE_SWAP_LAST) {
@@ -498,7 +499,7 @@ int remove_stable_noalloc_entry(void* const* src, void* const* dst, const uint8_
 
 #define X(L)                                                                                                                  \
     template int remove_stable_noalloc_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, uint32_t, int64_t, int64_t*, cudaStream_t); \
-    template int remove_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, int, void*, const int64_t**, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t); \
+    template int remove_entry<L>(void* const*, void* const*, const uint8_t*, int64_t, int, void*, int64_t, int64_t*, int64_t*, cudaEvent_t, cudaStream_t); \
     template int gather_rows_entry<L>(void* const*, int64_t, const uint32_t*, int64_t, void*, cudaStream_t);
 SOAX_FOR_EACH_LAYOUT(X)
 #undef X

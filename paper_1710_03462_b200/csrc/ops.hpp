@@ -47,10 +47,10 @@ template <class L> int bin_permute_entry(const BinArgs& a, cudaStream_t st);
 template <class L> size_t bin_scratch_bytes(int64_t n, int log2g, bool inplace);
 
 // NEXT-3 (container_kernels.cu)
-// Enqueues everything and returns: the survivor count is copied (asynchronously) into pin_n (pinned host memory) and, if
-// not null, into host_new_n; count_ready is recorded right after those copies.  *dev_count = its device location.
+// Enqueues everything and returns: the scan kernel stores the survivor count straight into pin_n (MAPPED pinned host memory: no
+// copy node), a cudaMemcpyAsync brings it to host_new_n if that is not null, and count_ready is recorded after both.
 template <class L> int remove_entry(void* const* src, void* const* dst, const uint8_t* kill, int64_t n, int mode, void* scratch,
-                                    const int64_t** dev_count, int64_t dst_capacity, int64_t* pin_n, int64_t* host_new_n,
+                                    int64_t dst_capacity, int64_t* pin_n, int64_t* host_new_n,
                                     cudaEvent_t count_ready, cudaStream_t st);
 // The STABLE removal with its scratch in a file-scope device array of container_kernels.cu (soax_remove_stable_noalloc): no
 // device, pinned or event allocation anywhere on the path; the survivor count goes to dev_new_n (device memory).

@@ -163,6 +163,9 @@ class SoaxEngine:
         self._masks = {}
 
     def local_sort(self):
+        """With drift_dt != 0 the drift happens on the way into the sorted copy: soax_bin_permute leaves `src` READ ONLY
+        (Q22), so after this call self.src still holds the PRE-drift positions while the records handed to the
+        exchange are the drifted ones.  self.src is stale from here on; the state of the step is what `merge` returns."""
         tmp = self._Cn.Soax(self.src.fields, 0, capacity=max(self.src.n, 1))
         r = self.src.bin_permute(tmp, self.grid_dim, drift_dt=self.drift_dt, want_kinetic=self.drift_dt != 0.0)
         self.kinetic = r["kinetic"]
