@@ -307,6 +307,19 @@ void soax_oracle_get_elements(const void* aos, int64_t stride, const uint32_t* i
     unsigned char* o = (unsigned char*)out;
     for (int64_t k = 0; k < m; ++k) std::memcpy(o + k * stride, a + (int64_t)idx[k] * stride, (size_t)stride);
 }
+// NEXT-4 (include/soax.h soax_gather_segments_aos): output row j is input row seg_src[i] + (j - seg_dst[i]), i the
+// LAST segment with seg_dst[i] <= j.  The same row-by-row loop as oracle.gather_segments in Python (which stays, and pins
+// this one in tests/test_container_oracle.py); written in C only so that 2^24 rows finish in seconds.
+void soax_oracle_gather_segments(const void* aos, int64_t stride, const int64_t* seg_dst, const int64_t* seg_src, int64_t nseg,
+                                 int64_t n, void* out) {
+    const unsigned char* a = (const unsigned char*)aos;
+    unsigned char* o = (unsigned char*)out;
+    int64_t i = 0;
+    for (int64_t j = 0; j < n; ++j) {
+        while (i + 1 < nseg && seg_dst[i + 1] <= j) ++i;
+        std::memcpy(o + j * stride, a + (seg_src[i] + (j - seg_dst[i])) * stride, (size_t)stride);
+    }
+}
 
 // ---- NEXT-2: the one elementary operation numpy lacks, for oracle/expr.py: a correctly rounded fused multiply-add
 //      over arrays (std::fma / std::fmaf are correctly rounded with or without hardware FMA).

@@ -181,7 +181,39 @@ class Soax:
         assert count.dtype == torch.int64 and count.is_cuda and count.numel() >= 1
         B.soax_remove_stable_noalloc(self.handle, dst.handle, kill.data_ptr(), keep_flagged, count.data_ptr(), _stream())
 
+    def reserve(self, capacity: int) -> None:
+        """Regrow (the paper's resize / push_back grow every array).  The C ABI never allocates -- the
+        caller owns device memory -- so growing is done here, on the caller's side: a new torch slab of at least
+        max(capacity, 1.5 x the old capacity) particles, soax_alloc over it, ONE soax_copy of the live particles (a device
+        copy of every component array, enqueued on the current stream), then the handle and the slab are swapped and the old
+        handle is freed.  The old slab goes back to torch's allocator, which orders its reuse after the copy on this stream.
+        Views from comp_view() and graphs captured for the old arrays do not follow (graph keys hold the array addresses and
+        the allocation serial, so they invalidate themselves).  No-op if the capacity already suffices."""
+        if capacity <= self.capacity:
+            return
+        new_cap = max(int(capacity), self.capacity + self.capacity // 2, 1)
+        slab_bytes = B.soax_slab_bytes(self.layout, new_cap)
+        slab = torch.empty(slab_bytes, dtype=torch.uint8, device=self.slab.device)
+        h = B.soax_alloc(self.layout, 0, new_cap, slab.data_ptr(), slab_bytes)
+        try:
+            B.soax_copy(h, self.handle, _stream())                  # sets the new handle's live count to the old one's
+        except Exception:
+            B.soax_free(h)
+            raise
+        old, self.handle = self.handle, h
+        self.slab, self.slab_bytes, self.capacity = slab, slab_bytes, new_cap
+        B.soax_free(old)
+
+    def resize(self, n: int) -> None:
+        """`soax.resize(n)`: the live count becomes n, growing the arrays first if n exceeds the capacity.
+        New rows are uninitialised, as with the paper's arrays."""
+        self.reserve(n)
+        B.soax_resize(self.handle, n)
+
     def push_back_aos(self, aos: torch.Tensor, m: int) -> None:
+        """`soax.push_back(particle)`, bulk: m packed records are appended; the arrays grow geometrically
+        through reserve() when they are full (soax_push_back_aos itself answers ALLOC past the capacity)."""
+        self.reserve(self.n + m)
         B.soax_push_back_aos(self.handle, aos.data_ptr(), m, _stream())
 
     def get_elements(self, idx: torch.Tensor, aos: torch.Tensor | None = None) -> torch.Tensor:

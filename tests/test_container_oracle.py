@@ -86,3 +86,20 @@ def test_gather_segments_is_the_merge_of_sorted_runs():
     got = oracle.gather_segments(recs.reshape(-1), 2, seg_dst, src_start.T.reshape(-1), cells.size).reshape(-1, 2)
     order = np.argsort(cells, kind="stable")
     assert np.array_equal(got, recs[order])
+
+
+def test_gather_segments_c_is_the_python_row_loop():
+    """The C row loop (used at 2^24 rows by the full-size GPU test) returns what the plain Python definition returns: random
+    tables with empty segments, repeated sources, single-row segments and a ragged end."""
+    rng = np.random.default_rng(11)
+    for trial in range(20):
+        stride = int(rng.choice([1, 3, 40, 89]))
+        nsrc, nseg = int(rng.integers(1, 300)), int(rng.integers(1, 40))
+        lens = rng.integers(0, 12, nseg)
+        seg_dst = np.cumsum(lens) - lens                              # starts at 0, non-decreasing, empty segments repeat
+        n = int(lens.sum())
+        seg_src = np.array([rng.integers(0, max(nsrc - l, 0) + 1) for l in lens])
+        a = rng.integers(0, 256, (nsrc + 12) * stride, dtype=np.uint8)
+        assert np.array_equal(oracle.gather_segments_c(a, stride, seg_dst, seg_src, n), oracle.gather_segments(a, stride, seg_dst, seg_src, n))
+    rows = np.arange(10 * 3, dtype=np.uint8)
+    assert oracle.gather_segments_c(rows, 3, [0, 2, 2, 5], [7, 0, 4, 1], 6).reshape(-1, 3)[:, 0].tolist() == [21, 24, 12, 15, 18, 3]

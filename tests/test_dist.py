@@ -125,8 +125,7 @@ else:
     (out, c32, _), bounds, n_local = D.bin_exchange(engine)
     mine = out.download()
     counts = c32.cpu().numpy().view(np.uint32)
-    big = Cn.Soax(Cn.R1, 0, capacity=sum(sizes))                   # room for arrivals: the caller owns the memory
-    big.copy_from(out)
+    big = out                                                      # sized to the LOCAL count: arrivals beyond it regrow it (Soax.reserve)
     big.step(B.SOAX_STEP_DRIFT, DT, nsteps=1)
     n_after = D.migrate(engine, big, bounds)
     after = big.to_aos().cpu().numpy()

@@ -126,8 +126,8 @@ def test_push_back_get_elements_copy(gpu):
     whole = np.concatenate([oracle.r1_soa_to_aos(a), oracle.r1_soa_to_aos(b)])
     assert np.array_equal(image(s), whole)
     with pytest.raises(B.SoaxError) as ei:
-        s.push_back_aos(extra, 1)
-    assert ei.value.status == B.SOAX_ERR_ALLOC                       # no regrow: the caller owns the memory
+        B.soax_push_back_aos(s.handle, extra.data_ptr(), 1)
+    assert ei.value.status == B.SOAX_ERR_ALLOC                       # the C call never allocates: the caller owns the memory
     idx = np.random.default_rng(4).integers(0, n + m, 1234).astype(np.uint32)
     idx[:3] = [0, n + m - 1, 0]
     got = s.get_elements(torch.from_numpy(idx.view(np.int32)).cuda()).cpu().numpy()
@@ -236,3 +236,69 @@ def test_gather_segments_merges_sorted_runs(gpu, world, n_each):
     if n:                                                             # and it IS the stable sort by cell of the concatenation
         whole = oracle.r1_aos_to_soa(recs)
         assert np.array_equal(want, oracle.r1_soa_to_aos(oracle.permute_r1(whole, oracle.bin_r1(whole, G)["perm"])))
+
+
+def test_push_back_regrows_like_the_papers_container(gpu):
+    """push_back past the capacity and resize(n) grow every array.  Repeated push_back into a
+    container that starts with room for 3 particles equals the oracle-side concatenation byte for byte after every step, and
+    the capacity grows geometrically (few regrows, not one per call); R2 as well, and resize() beyond the capacity keeps the
+    live rows."""
+    torch, B, Cn = gpu
+    for fields, make, to_aos in ((Cn.R1, inputs.make_r1, oracle.r1_soa_to_aos),):
+        s = Cn.Soax(fields, 0, capacity=3)
+        whole, caps = np.zeros(0, np.uint8), []
+        for step, m in enumerate([1, 2, 1, 700, 4097, 0, 33, 20000]):
+            rec = to_aos(make(m, seed=100 + step)) if m else np.zeros(0, np.uint8)
+            s.push_back_aos(torch.from_numpy(np.concatenate([rec, np.zeros(16, np.uint8)])).cuda(), m)
+            whole = np.concatenate([whole, rec])
+            caps.append(s.capacity)
+            assert s.n == whole.size // 40 <= s.capacity
+            assert np.array_equal(image(s), whole), step
+        assert caps[0] == 3 and caps[2] >= 4 and len(set(caps)) <= 6 and caps[-1] >= 24834
+        live = s.n
+        s.resize(2 * s.capacity + 5)                                  # the paper's resize: the live rows survive a regrow
+        assert s.n == 2 * caps[-1] + 5 and s.capacity >= s.n
+        B.soax_resize(s.handle, live)
+        assert np.array_equal(image(s), whole)
+        s.step(B.SOAX_STEP_DRIFT, 1e-3, nsteps=3)                     # the regrown container is a full citizen (graph replay included)
+        exp = oracle.drift(oracle.r1_aos_to_soa(whole), 1e-3, 3)
+        assert np.array_equal(image(s), oracle.r1_soa_to_aos(exp))
+    h = inputs.make_r2(501, seed=4)
+    s2 = device(Cn, Cn.R2, h)
+    before = image(s2)
+    s2.reserve(502)
+    assert s2.capacity == 751 and s2.n == 501 and np.array_equal(image(s2), before)
+
+
+def test_advice_hardening_of_remove_and_gather(gpu):
+    """(a) soax_remove answers UNSUPPORTED while its stream is being captured (the count event would never fire and the handle
+    would read a stale word); (b) soax_gather_segments_aos with a table that does not start at row 0 is served from segment 0
+    with offset 0 instead of reading index -1; (c) a call that sets a handle's count while a removal count is pending waits
+    for it, and the handle reports the new count."""
+    torch, B, Cn = gpu
+    n = 5000
+    host = inputs.make_r1(n, seed=77)
+    base = oracle.r1_soa_to_aos(host)
+    s = device(Cn, Cn.R1, host)
+    kd = torch.from_numpy((np.arange(n) % 3 == 0).astype(np.uint8)).cuda()
+    scratch = torch.empty(B.soax_remove_scratch_bytes(n), dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        with pytest.raises(B.SoaxError) as ei:
+            B.soax_remove(s.handle, None, kd.data_ptr(), B.SOAX_REMOVE_SWAP_LAST, scratch.data_ptr(), scratch.numel(), side.cuda_stream)
+    assert ei.value.status == B.SOAX_ERR_UNSUPPORTED
+    torch.cuda.synchronize()
+    assert s.n == n and np.array_equal(image(s), base)                # nothing was enqueued
+    # (b)
+    d = Cn.Soax(Cn.R1, 0, capacity=8)
+    recs = torch.from_numpy(np.concatenate([base[:40 * 16], np.zeros(16, np.uint8)])).cuda()
+    d.from_aos_segments(recs, torch.tensor([2, 4], dtype=torch.int32).cuda(), torch.tensor([0, 5], dtype=torch.int32).cuda(), 6)
+    rows = base.reshape(-1, 40)
+    assert np.array_equal(image(d).reshape(-1, 40), rows[[0, 0, 0, 1, 5, 6]])
+    # (c)
+    s.remove_async(kd)                                                # count pending on s
+    B.soax_resize(s.handle, 10)                                       # waits for the pending count, then sets its own
+    assert s.n == 10
+    assert np.array_equal(image(s), oracle.remove_swap_last(base, 40, kd.cpu().numpy())[:400])

@@ -172,3 +172,90 @@ def test_config5_full_size_vs_oracle(gpu):
         assert torch.equal(r2[k], r[k]), k
     assert float(r2["kinetic"].item()) == ke
     assert src.n == n and torch.equal(src.slab, checked)             # same layout, same capacity: the slabs are images of each other
+
+
+# ---- NEXT-3 / NEXT-4 at the sizes bench.py times them (2^24): every row against the oracle ------------------------------------
+# n = 2^24 + 3 is ragged and has 4097 mask tiles, so the one-CTA scan of the tile counts (kill_scan_kernel) walks five chunks
+# of 1024 with its carry; the gather's table has 2 M segments; the mask program and the bulk getElement run at 2^24.
+N_BIG = (1 << 24) + 3
+
+
+@pytest.fixture(scope="module")
+def big(gpu):
+    torch, B, Cn = gpu
+    host = inputs.make_r1(N_BIG, seed=11, threads=os.cpu_count() or 8)
+    base = oracle.r1_soa_to_aos(host)
+    s = Cn.Soax(Cn.R1, N_BIG)
+    s.upload(host)
+    return host, base, s
+
+
+def big_masks(n):
+    rng = np.random.default_rng(24)
+    yield "random 10 %", (rng.random(n) < 0.1).astype(np.uint8)
+    k = np.zeros(n, np.uint8); k[: n // 2] = 1; yield "front half (every hole below m, every mover above)", k
+    k = np.zeros(n, np.uint8); k[n // 2:] = 200; yield "back half (pure truncation)", k
+
+
+def test_remove_full_size_vs_oracle(gpu, big):
+    """soax_remove over 2^24 + 3 particles in SWAP_LAST, STABLE and STABLE | KEEP_FLAGGED against the oracle's forward loop
+    and stable filter, every byte of every surviving record (Q20)."""
+    torch, B, Cn = gpu
+    host, base, s = big
+    n = N_BIG
+    work, d = Cn.Soax(Cn.R1, 0, capacity=n), Cn.Soax(Cn.R1, 0, capacity=n)
+    for what, kill in big_masks(n):
+        kd = torch.from_numpy(kill).cuda()
+        m_exp = int((kill == 0).sum())
+        work.copy_from(s)
+        assert work.remove(kd) == m_exp
+        assert np.array_equal(work.to_aos().cpu().numpy(), oracle.remove_swap_last(base, 40, kill)), what
+        assert s.remove(kd, stable=True, dst=d) == m_exp
+        assert np.array_equal(d.to_aos().cpu().numpy(), oracle.remove_stable(base, 40, kill)), what
+        s.remove_async(kd, stable=True, dst=d, keep_flagged=True)    # the same mask read the other way: the flagged rows stay
+        assert d.n == n - m_exp
+        assert np.array_equal(d.to_aos().cpu().numpy(), oracle.remove_stable(base, 40, (kill == 0).astype(np.uint8))), what
+    assert s.n == n and np.array_equal(s.to_aos().cpu().numpy(), base)  # the source of the stable removals is untouched
+
+
+def test_mask_program_full_size_vs_oracle(gpu, big):
+    """The cell-range condition of the migration step (soax_expr_mask) over 2^24 + 3 particles against oracle.expr.mask."""
+    from oracle import expr as oexpr
+    torch, B, Cn = gpu
+    host, base, s = big
+    cond, sc = "(double(cell(64)) < lo) | (double(cell(64)) >= hi)", {"lo": 70000, "hi": 190000}
+    got = Cn.MaskProgram(Cn.R1, cond, ["lo", "hi"]).mask(s, **sc).cpu().numpy()
+    exp = oexpr.mask(host, cond, sc)
+    assert got.shape == exp.shape and np.array_equal(got, exp) and 0 < int(exp.sum()) < N_BIG
+
+
+def test_get_elements_full_size_vs_oracle(gpu, big):
+    """Bulk getElement of 2^20 random rows (repeats, first and last row included) of the 2^24 + 3 against the oracle."""
+    torch, B, Cn = gpu
+    host, base, s = big
+    rng = np.random.default_rng(5)
+    idx = rng.integers(0, N_BIG, 1 << 20).astype(np.uint32)
+    idx[:4] = [0, N_BIG - 1, N_BIG - 1, 0]
+    got = s.get_elements(torch.from_numpy(idx.view(np.int32)).cuda()).cpu().numpy()
+    assert np.array_equal(got, oracle.get_elements(base, 40, idx))
+
+
+def test_gather_segments_full_size_vs_oracle(gpu, big):
+    """The exchange's merge at the size bench.py times it: 8 runs, 64^3 cells = 2 097 152 segments (many empty or one row
+    long), 2^24 + 3 rows, against the oracle's row loop.  The tables are built from random per-run per-cell counts the way
+    dist.SoaxEngine.merge builds them; the records are the big set's bytes (a gather looks at no field)."""
+    torch, B, Cn = gpu
+    host, base, s = big
+    world, ncell, n = 8, 64 ** 3, N_BIG
+    rng = np.random.default_rng(8)
+    cnt = rng.multinomial(n, np.full(world * ncell, 1.0 / (world * ncell))).reshape(world, ncell).astype(np.int64)
+    sizes = cnt.sum(1)
+    src_start = (np.cumsum(sizes) - sizes)[:, None] + np.cumsum(cnt, 1) - cnt
+    flat = cnt.T.reshape(-1)
+    seg_dst, seg_src = (np.cumsum(flat) - flat), src_start.T.reshape(-1)
+    want = oracle.gather_segments_c(base, 40, seg_dst, seg_src, n)
+    d = Cn.Soax(Cn.R1, 0, capacity=n)
+    recs = torch.empty(n * 40 + 16, dtype=torch.uint8, device="cuda")
+    recs[:n * 40] = torch.from_numpy(base).cuda()
+    d.from_aos_segments(recs, torch.from_numpy(seg_dst.astype(np.int32)).cuda(), torch.from_numpy(seg_src.astype(np.int32)).cuda(), n)
+    assert d.n == n and np.array_equal(d.to_aos().cpu().numpy(), want)
