@@ -180,7 +180,8 @@ double soax_oracle_r1_energy(const void* aos, int64_t n, int32_t kind, double k,
     for (int64_t i = 0; i < n; ++i) {
         R1 p = load1(base, i);
         double v[3] = {(double)p.vel[0], (double)p.vel[1], (double)p.vel[2]};
-        acc.add(energy_term(v, p.pos, kind, k, ctr));
+        double x[3] = {p.pos[0], p.pos[1], p.pos[2]};  // copies: a pointer to the packed (4 mod 8) member would be misaligned
+        acc.add(energy_term(v, x, kind, k, ctr));
     }
     return acc.value();
 }
@@ -231,7 +232,8 @@ int32_t soax_oracle_r1_bin(const void* aos, int64_t n, int32_t G, uint32_t* cell
     std::vector<uint32_t> cl((size_t)n), cnt((size_t)ncell, 0u), off((size_t)ncell, 0u);
     for (int64_t i = 0; i < n; ++i) {
         R1 p = load1(base, i);
-        int64_t c = cell_of(p.pos, G);
+        const double x[3] = {p.pos[0], p.pos[1], p.pos[2]};  // copies: no pointer into the packed record
+        int64_t c = cell_of(x, G);
         if (c < 0 || c >= ncell) return -1;
         cl[(size_t)i] = (uint32_t)c;
         cnt[(size_t)c]++;
