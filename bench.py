@@ -233,18 +233,28 @@ def run_reference(args) -> None:
 
 
 # ------------------------------------------------------------------------------------------------- GPU helpers
+TIMINGS: list = []     # every ev_time_ms call of a run: where it was made, median (the figure reported), best, iterations
+
+
 def ev_time_ms(torch, fn, iters: int, warmup: int = 3) -> float:
-    """average milliseconds of fn() over `iters` calls, CUDA events on the current stream, after warm-up"""
+    """MEDIAN milliseconds of fn() over max(iters, 10) calls, each timed by its own pair of CUDA events on the current
+    stream, after warm-up; the best of them and the call site go to TIMINGS (printed as extras.timing_stats)."""
+    import inspect
+    import statistics
+    iters = max(iters, 10)
     for _ in range(warmup):
         fn()
     torch.cuda.synchronize()
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record()
-    for _ in range(iters):
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(iters + 1)]
+    evs[0].record()
+    for i in range(iters):
         fn()
-    b.record()
+        evs[i + 1].record()
     torch.cuda.synchronize()
-    return a.elapsed_time(b) / iters
+    ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(iters)]
+    fr = inspect.stack()[1]
+    TIMINGS.append({"where": f"{fr.function}:{fr.lineno}", "median_ms": statistics.median(ms), "best_ms": min(ms), "iters": iters})
+    return statistics.median(ms)
 
 
 def device_fill(torch, s, seed: int) -> None:
@@ -289,6 +299,8 @@ def run_extras(torch, B, Cn, s, peak: float, which=("energy", "config3", "config
         _extra_container(torch, B, Cn, s, peak, ex, gbs)
     if "exchange" in which:
         _extra_exchange(torch, B, Cn, s, peak, ex, gbs)
+    ex["timing_stats"] = {"method": "every figure above timed by ev_time_ms is the MEDIAN of >= 10 runs, each between its own pair of "
+                                    "CUDA events; best_ms is the fastest of them", "calls": list(TIMINGS)}
     return ex
 
 
@@ -355,12 +367,84 @@ def _extra_exchange(torch, B, Cn, s, peak, ex, gbs):
         work.remove_async(m1, scratch=rs2)
     ms_swap = ev_time_ms(torch, refresh_and_remove, 10) - ms_copy
     ms_mig = ms_masks + ms_out + ms_swap
+    ids, gone_mask = s.comp_view("id"), m1 != 0
+    refresh_and_remove()
+    verified = bool(same and torch.equal(torch.sort(out.comp_view("id"))[0], torch.sort(fresh.comp_view("id"))[0])   # the merge loses nobody
+                    and gone.n == int(gone_mask.sum().item()) and torch.equal(gone.comp_view("id"), ids[gone_mask])  # leavers, in order
+                    and torch.equal(torch.sort(work.comp_view("id"))[0], torch.sort(ids[~gone_mask])[0]))            # stayers: the rest
     ex["next4_exchange_local_work"] = {
+        "verified": verified,
         "n": n, "runs": world, "merge_segmented_gather_ms": ms_new, "merge_segmented_gather_GBps_80B": gbs(80, n, ms_new),
         "merge_round1_transpose_plus_sort_ms": ms_old, "merge_speedup": ms_old / ms_new, "merge_results_identical": bool(same),
         "migration_local_ms": ms_mig, "migration_mask_ms": ms_masks, "migration_copy_out_leavers_ms": ms_out,
         "migration_overwrite_with_last_ms": ms_swap, "migration_leavers": n_gone, "migration_particles_per_s": n / (ms_mig * 1e-3),
         "note": "device-side pieces of the multi-GPU exchange on one GPU; the collectives themselves are unmeasured on hardware"}
+
+
+def run_exchange_leg(torch, dist, B, Cn, rank: int, world: int, n: int, steps: int = 10) -> dict:
+    """NEXT-4 under `--gpus N` ("transferring [particles] from one processor to another"): EVERY rank
+    runs it.  Config 5 distributed: each rank holds n uniform R1 particles; dist.bin_exchange sorts them by cell on a 64^3 grid,
+    splits the cell range into `world` balanced contiguous pieces from the all-gathered counts, moves the records with ONE
+    all_to_all_single over NCCL and merges the received runs; then `steps` x {one drift step, dist.migrate}.  Times are CUDA
+    events on this stream (they span the host round trip of the plan), max over ranks.  Conservation: the global particle
+    count and the rank-ordered kinetic energy (a drift changes no velocity) must survive."""
+    import statistics
+    from paper_1710_03462_b200 import dist as D
+    G = 64
+    src = Cn.Soax(Cn.R1, n)
+    device_fill(torch, src, 100 + rank)
+    engine = D.SoaxEngine(src, G)
+    e0 = D.energy_sum(src.energy_async(B.SOAX_ENERGY_KINETIC))
+
+    def reduce_max(x: float) -> float:
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def timed(fn):
+        dist.barrier()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        r = fn()
+        b.record()
+        torch.cuda.synchronize()
+        return r, reduce_max(a.elapsed_time(b))
+
+    D.bin_exchange(engine)                                        # warm-up: communicator set-up, program compilation, allocator
+    ex_ms, a2a_ms = [], []
+    for _ in range(3):
+        ((out, _, _), bounds, n_local), ms = timed(lambda: D.bin_exchange(engine))
+        ex_ms.append(ms)
+        ship = engine.last_ship
+        a2a_ms.append(reduce_max(ship["events"][0].elapsed_time(ship["events"][1])))
+    sent = sum(k for q, k in enumerate(ship["n_send"]) if q != rank) * ship["stride"]
+    tot = torch.tensor([n_local, sent], dtype=torch.int64, device="cuda")
+    dist.all_reduce(tot)
+    most = reduce_max(float(n_local))
+    big, mig_ms, moved = out, [], 0
+    for _ in range(steps):
+        def one():
+            big.step(B.SOAX_STEP_DRIFT, DT, nsteps=1)
+            return D.migrate(engine, big, bounds)
+        _, ms = timed(one)
+        mig_ms.append(ms)
+        moved += sum(k for q, k in enumerate(engine.last_ship["n_send"]) if q != rank)
+    cnt = torch.tensor([big.n, moved], dtype=torch.int64, device="cuda")
+    dist.all_reduce(cnt)
+    e1 = D.energy_sum(big.energy_async(B.SOAX_ENERGY_KINETIC))
+    med = statistics.median
+    return {"world": world, "backend": dist.get_backend(), "n_per_rank": n, "grid_dim": G,
+            "bin_exchange_ms": med(ex_ms), "bin_exchange_best_ms": min(ex_ms), "all_to_all_ms": med(a2a_ms),
+            "all_to_all_bytes_all_ranks": int(tot[1]), "all_to_all_GBps_per_gpu": int(tot[1]) / world / (med(a2a_ms) * 1e-3) / 1e9 if med(a2a_ms) > 0 else None,
+            "bin_exchange_particles_per_s": world * n / (med(ex_ms) * 1e-3),
+            "imbalance_max_over_mean": most / (int(tot[0]) / world),
+            "migration_steps": steps, "migration_ms_per_step": med(mig_ms), "migration_best_ms": min(mig_ms),
+            "migration_particles_moved_per_step_all_ranks": int(cnt[1]) / steps,
+            "conserved_count": int(tot[0]) == world * n and int(cnt[0]) == world * n,
+            "kinetic_energy_before": e0, "kinetic_energy_after": e1, "kinetic_rel_err": abs(e1 - e0) / abs(e0),
+            "verified": bool(int(tot[0]) == world * n and int(cnt[0]) == world * n and abs(e1 - e0) <= 1e-10 * abs(e0)),
+            "note": "times are max over ranks; at world = 1 nothing crosses a link (all_to_all of 0 bytes to peers)"}
 
 
 def _extra_container(torch, B, Cn, s, peak, ex, gbs):
@@ -386,7 +470,15 @@ def _extra_container(torch, B, Cn, s, peak, ex, gbs):
     idx = torch.randint(0, n, (1 << 20,), generator=g, device="cuda", dtype=torch.int32)
     out = torch.empty((1 << 20) * 40, dtype=torch.uint8, device="cuda")
     ms_get = ev_time_ms(torch, lambda: s.get_elements(idx, out), 10)
+    # oracle-free invariants on the timed results (the parity tests compare the same calls with the oracle at this size)
+    ids, alive = s.comp_view("id"), kill == 0
+    swap()
+    verified = bool(d.n == m == int(alive.sum().item()) and torch.equal(d.comp_view("id"), ids[alive])          # stable: the unflagged ids, in order
+                    and t.n == m and torch.equal(torch.sort(t.comp_view("id"))[0], torch.sort(ids[alive])[0])   # swap-last: the same set
+                    and torch.equal(t.comp_view("id")[alive[:m]], ids[:m][alive[:m]])                       # ... and no survivor below m moved
+                    and torch.equal(out.view(-1, 40)[:, :4].contiguous().view(torch.int32).reshape(-1), ids[idx.long()]))
     ex["next3_container"] = {
+        "verified": verified,
         "n": n, "kill_fraction": 1 - m / n, "remove_stable_ms": ms_stable,
         "remove_stable_GBps": (2 * n + 80 * m) / ms_stable / 1e6, "remove_stable_frac_of_peak": (2 * n + 80 * m) / ms_stable / 1e6 / peak,
         # sector-granular floor: with 10 % of the rows flagged at random every 32-byte sector of every source array holds a
@@ -865,8 +957,11 @@ def _run_soax(args) -> None:
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the SoAx path has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if world > 1 or args.with_exchange:
+        if world == 1:                                            # --with-exchange on one GPU: an NCCL group of one rank
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", str(29000 + os.getpid() % 2000))
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local), rank=rank, world_size=world)
     B.lib()
     for kv in filter(None, args.tune.split(",")):
         key, val = kv.split("=")
@@ -1025,6 +1120,9 @@ def _run_soax(args) -> None:
         and abs(consumed[-1] - float(e_host[1])) <= 1e-9 * abs(float(e_host[1]))   # same inputs every step: same energy
     del conts, outs
 
+    exchange = None
+    if world > 1 or args.with_exchange:                           # every rank takes part; rank 0 reports it under extras.exchange
+        exchange = run_exchange_leg(torch, dist, B, Cn, rank, world, n)
     if rank == 0:
         peak, peak_src = measured_peak()
         achieved = STEP_BYTES * n / kernel_ms / 1e6              # GB/s: algorithmic bytes per launch / avg launch time
@@ -1066,8 +1164,10 @@ def _run_soax(args) -> None:
                 del pin, out
                 line["extras"] = run_extras(torch, B, Cn, s, peak)
             line["host_seconds_outside_timed_regions"] = time.perf_counter() - t0
+        if exchange is not None:
+            line.setdefault("extras", {})["exchange"] = exchange
         print(json.dumps(line))
-    if world > 1:
+    if world > 1 or args.with_exchange:
         dist.barrier()
         dist.destroy_process_group()
 
@@ -1113,6 +1213,8 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["soax", "reference"], default="soax")
+    ap.add_argument("--with-exchange", action="store_true", help="run the distributed config-5 + migration leg (extras.exchange) at N=1 too, "
+                    "over an NCCL group of one rank; with --gpus N > 1 it always runs")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra per-config measurements (configs 1, 3, 4, 5)")
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5,expr,container: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")

@@ -220,7 +220,17 @@ def _ship(engine: Engine, counts: torch.Tensor, records: torch.Tensor, group, bo
     b, n_send, n_recv = plan_exchange(all_counts, rank, bounds)
     s = engine.stride
     recv = torch.empty(max(sum(n_recv) * s, 16), dtype=torch.uint8, device=records.device)
+    timed = records.is_cuda                                       # measurement aid (bench.py): events around the one all-to-all
+    ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) if timed else None
+    if timed:
+        ev[0].record()
     _all_to_all(recv[:sum(n_recv) * s], records[:sum(n_send) * s], [k * s for k in n_recv], [k * s for k in n_send], group)
+    if timed:
+        ev[1].record()
+    try:
+        engine.last_ship = {"n_send": n_send, "n_recv": n_recv, "events": ev, "stride": s}
+    except AttributeError:
+        pass
     return recv, n_recv, b, all_counts
 
 
