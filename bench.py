@@ -46,8 +46,26 @@ def committed_traffic(key: str = "step_soa_kernel"):
         with open(path) as f:
             d = json.load(f).get(key)
         if d:
-            return d.get("dram_bytes_per_launch"), {k: d.get(k) for k in ("captured_at_commit", "captured_on", "source", "n_particles")}
+            prov = {k: d.get(k) for k in ("captured_at_commit", "captured_on", "source", "n_particles")}
+            ok = commit_in_history(str(d.get("captured_at_commit", "")).split()[0] if d.get("captured_at_commit") else "")
+            if ok is False:                                       # a provenance that cannot be resolved is no provenance
+                prov["rejected"] = "captured_at_commit is not a commit of this repository: traffic withheld"
+                return None, prov
+            prov["commit_checked"] = "resolved in git history" if ok else "not checkable here (no git history on this machine); tests/test_host_abi.py checks it where there is"
+            return d.get("dram_bytes_per_launch"), prov
     return None, None
+
+
+def commit_in_history(rev: str):
+    """True / False if `git cat-file -t rev` can be asked here (a .git directory and a git binary exist), else None: the GPU box
+    receives the tree without its history."""
+    if not rev or not os.path.isdir(os.path.join(ROOT, ".git")):
+        return None if rev else False
+    try:
+        r = subprocess.run(["git", "-C", ROOT, "cat-file", "-t", rev], capture_output=True, text=True, timeout=20)
+    except (OSError, subprocess.TimeoutExpired):
+        return None
+    return r.returncode == 0 and r.stdout.strip() == "commit"
 
 
 # ---------------------------------------------------------------------------------------------- clocks sampling
@@ -708,165 +726,6 @@ def run_tour(torch, B, Cn) -> None:
     print(json.dumps({"tour": "done", "gpu_launches": B.soax_launch_count()}))
 
 
-def run_bin_study(torch, B, Cn, log2n: int = 27) -> None:
-    """Design study behind the counting sort (--bin-study) on the real config-5 input at N = 2^27: digit width x cluster
-    size x cluster barrier x store pacing (soax_tune bin_bits / bin_cluster / bin_csync / bin_pace).  One JSON line per
-    measurement; every variant's permutation is checked against a stable argsort before it is timed."""
-    n = 1 << log2n
-    s5, d5 = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
-    device_fill(torch, s5, 7)
-    i = [(s5.comp_view("pos", c) * 64.0).to(torch.int64) for c in range(3)]
-    ref = torch.sort((i[0] * 64 + i[1]) * 64 + i[2], stable=True)[1].to(torch.int32)
-    del i
-    S = 4096                                                      # bin_pace bit 12: a CTA barrier between a thread's stores
-    rows = [(6, 1, 1, 0, 1), (6, 1, 1, S, 1), (6, 4, 1, S, 1), (9, 1, 1, 0, 1), (9, 1, 1, S, 1), (9, 2, 1, S, 1), (9, 4, 0, 0, 1), (9, 4, 1, 0, 1),
-            (9, 4, 0, S, 1), (9, 4, 1, S, 1), (9, 4, 1, 2 * S, 1), (9, 4, 1, 2 * S, 2), (9, 4, 1, 2 * S, 4), (9, 4, 1, 100, 1), (9, 4, 1, S + 100, 1),
-            (9, 8, 1, 2 * S, 2), (9, 16, 1, 2 * S, 2), (7, 4, 1, 2 * S, 2), (5, 1, 1, 0, 1), (0, 0, 1, -1, 0)]
-    for bits, cl, cs, pace, every in rows:
-        for key, v in (("bin_bits", bits), ("bin_cluster", cl), ("bin_csync", cs), ("bin_pace", pace), ("bin_pace_every", every)):
-            B.soax_tune(key, v)
-        scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
-        r = s5.bin_permute(d5, 64, scratch=scratch)
-        ok = bool(torch.equal(r["perm"], ref))
-        ms0 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, scratch=scratch), 5, 2)
-        ms1 = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True, scratch=scratch), 5, 2)
-        print(json.dumps({"study": "config 5 pipeline at 2^27", "digit_bits": bits or 9, "passes": (18 + (bits or 9) - 1) // (bits or 9),
-                          "cluster": cl or "default(4)", "cluster_barrier": cs, "pace_barrier": "default(cluster)" if pace < 0 else ("none", "cta", "cluster")[pace >> 12],
-                          "pace_sleep_ns": 0 if pace < 0 else pace & 0xfff, "pace_every_n_stores": every or "default(2)", "ms_no_drift": round(ms0, 3), "ms_drift_ke": round(ms1, 3),
-                          "permutation_equals_stable_argsort": ok, "scratch_GB": round(scratch.numel() / 1e9, 3)}), flush=True)
-        del scratch, r
-    for key, v in (("bin_bits", 0), ("bin_cluster", 0), ("bin_csync", 1), ("bin_pace", -1), ("bin_pace_every", 0)):
-        B.soax_tune(key, v)
-    # Control: the SAME default kernel on sets whose tiles fall into fewer bins in the first pass (longer pieces per bin; the
-    # second pass sees all 512 bins as before).  If the first pass speeds up, the scatter is bound by how the memory system takes
-    # short pieces, not by the work of the SMs, which is the same.
-    del ref
-    g = torch.Generator(device="cuda")
-    g.manual_seed(1)
-    tile = torch.arange(n, device="cuda") // 4096
-    scratch = torch.empty(B.soax_scratch_bytes(s5.layout, n, 64), dtype=torch.uint8, device="cuda")
-    for distinct in (512, 128, 64, 16):
-        w = max(distinct // 8, 1)                                 # low digit = (i1 & 7) 64 + i2: 8 values of i1 x w values of i2
-        for c in range(3):
-            s5.comp_view("pos", c).copy_(torch.rand(n, generator=g, device="cuda", dtype=torch.float64))
-        if distinct < 512:
-            for c, mult in ((2, 2654435761), (0, 40503)):
-                base = (tile * mult % 64) // w * w
-                i = base + torch.randint(0, w, (n,), generator=g, device="cuda")
-                s5.comp_view("pos", c).copy_((i.double() + torch.rand(n, generator=g, device="cuda", dtype=torch.float64)) / 64)
-                del base, i
-        ms = ev_time_ms(torch, lambda: s5.bin_permute(d5, 64, scratch=scratch), 5, 2)
-        print(json.dumps({"study": "piece-length control, default kernel, 2^27", "distinct_first_pass_digits_per_tile": distinct,
-                          "elements_per_tile_and_bin_first_pass": 4096 // distinct, "ms_no_drift": round(ms, 3)}), flush=True)
-
-
-def run_scatter_trace(torch, B, Cn, prefix: str, log2n: int = 27) -> None:
-    """Per-phase timeline of the binning scatter (--scatter-trace PREFIX).  Needs a STUDY BUILD of the library:
-        SOAX_NVCC_FLAGS=-DSOAX_SCATTER_TRACE python -m paper_1710_03462_b200.build --force
-    in which thread 0 of every CTA stamps the phases of its tile with %globaltimer.  Runs config 5 once at N = 2^27 (drift + KE),
-    reads the two files the library wrote (one per pass) and prints one JSON line per phase: mean / median / 90th percentile over
-    the 32768 tiles, in nanoseconds.  Rebuild without the flag afterwards."""
-    import numpy as np
-    os.environ["SOAX_TRACE"] = prefix
-    n = 1 << log2n
-    s5, d5 = Cn.Soax(Cn.R1, n), Cn.Soax(Cn.R1, n)
-    device_fill(torch, s5, 7)
-    s5.bin_permute(d5, 64, drift_dt=DT, want_kinetic=True)
-    torch.cuda.synchronize()
-    del os.environ["SOAX_TRACE"]
-    names = {0: "kernel start", 1: "set-up done (barriers, counters zeroed, CTA barrier)", 2: "keys in shared memory", 40: "digit ballots done",
-             41: "per-warp counters updated", 42: "CTA barrier", 43: "bin totals + scan done", 44: "CTA barrier", 45: "inverse permutation written",
-             3: "fence + CTA barrier: stage 1 joins the ring", 4: "unit 0 (keys): sources and destinations computed", 5: "cluster barrier",
-             6: "unit 0 stored", 7: "CTA barrier"}
-    order = [0, 1, 2, 40, 41, 42, 43, 44, 45, 3, 4, 5, 6, 7]
-    for m in range(1, 6):
-        b = 8 + 6 * (m - 1)
-        names.update({b: f"move {m}: begin", b + 1: f"move {m}: unit in shared memory", b + 2: f"move {m}: gathered into registers",
-                      b + 3: f"move {m}: cluster barrier", b + 4: f"move {m}: stored (3 more cluster barriers inside)", b + 5: f"move {m}: CTA barrier"})
-        order += list(range(b, b + 6))
-    for tag, what in (("01", "pass 1 (SoA -> paired, drift applied)"), ("10", "pass 2 (paired -> SoA)")):
-        path = f"{prefix}_{tag}_0.bin"
-        if not os.path.exists(path):
-            print(json.dumps({"scatter_trace": what, "error": f"{path} missing: is the library a -DSOAX_SCATTER_TRACE build?"}))
-            continue
-        t = np.fromfile(path, dtype=np.uint64).reshape(-1, 64).astype(np.int64)
-        t = t[t[:, 0] > 0]
-        total = t[:, order[-1]] - t[:, 0]
-        span = float(t[:, order[-1]].max() - t[:, 0].min())
-        print(json.dumps({"scatter_trace": what, "tiles": int(len(t)), "tile_us_mean": round(float(total.mean()) / 1e3, 2),
-                          "kernel_span_us": round(span / 1e3, 1), "mean_concurrent_ctas": round(float(total.sum()) / span, 1)}))
-        for a, b in zip(order[:-1], order[1:]):
-            d = t[:, b] - t[:, a]
-            print(json.dumps({"pass": tag, "from": names[a], "to": names[b], "ns_mean": round(float(d.mean())), "ns_p50": round(float(np.percentile(d, 50))),
-                              "ns_p90": round(float(np.percentile(d, 90)))}))
-        os.remove(path)
-    for f in (f"{prefix}_01_1.bin", f"{prefix}_10_1.bin"):
-        if os.path.exists(f):
-            os.remove(f)
-
-
-def run_sweeps(torch, B, Cn) -> None:
-    """The launch-shape sweeps DESIGN.md section 6 cites (--sweeps), each one JSON line per point, N = 2^24 R1:
-      step      symplectic-Euler step: particles per thread x threads per CTA x persistent grid
-      xpose     AoS<->SoA transposes: records per stage (256 R) x stages x CTAs per SM
-      streams   a CONTROL for the transposes' plateau: plain copies with 1 input / 7 output streams and 7 / 1, written as
-                expression programs on a run-time layout {double a; double b[7]} (64 B/particle), against soax_copy (7 / 7)"""
-    n = 1 << LOG2N
-    s = Cn.Soax(Cn.R1, n)
-    device_fill(torch, s, 0)
-    kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
-    for ppt in (1, 2, 4):
-        for block in (128, 256, 512):
-            for persist in (0, 2, 4, 8):
-                for k, v in (("step_ppt", ppt), ("step_block", block), ("step_persist", persist)):
-                    B.soax_tune(k, v)
-                ms = ev_time_ms(torch, lambda: s.step(kind, DT, nsteps=20), 3, 1) / 20
-                print(json.dumps({"sweep": "step", "particles_per_thread": ppt, "block": block, "persistent_ctas_per_sm": persist,
-                                  "ms": round(ms, 5), "GBps_72B": round(72 * n / ms / 1e6, 1)}), flush=True)
-    for k, v in (("step_ppt", 4), ("step_block", 256), ("step_persist", 0)):
-        B.soax_tune(k, v)
-    aos = s.to_aos()
-    for r in (1, 2, 4):
-        for ns in (1, 2):
-            for ctas in (1, 2, 4, 8):
-                for k, v in (("xpose_r", r), ("xpose_ns", ns), ("xpose_ctas", ctas)):
-                    B.soax_tune(k, v)
-                try:
-                    a = ev_time_ms(torch, lambda: s.from_aos(aos, n), 10)
-                    b = ev_time_ms(torch, lambda: s.to_aos(aos), 10)
-                except Exception as e:                            # a shape that does not fit shared memory
-                    print(json.dumps({"sweep": "xpose", "records_per_stage": 256 * r, "stages": ns, "ctas_per_sm": ctas, "error": str(e)[:80]}))
-                    continue
-                print(json.dumps({"sweep": "xpose", "records_per_stage": 256 * r, "stages": ns, "ctas_per_sm": ctas,
-                                  "aos_to_soa_ms": round(a, 5), "soa_to_aos_ms": round(b, 5),
-                                  "aos_to_soa_GBps": round(80 * n / a / 1e6, 1), "soa_to_aos_GBps": round(80 * n / b / 1e6, 1)}), flush=True)
-    for k in ("xpose_r", "xpose_ns", "xpose_ctas"):
-        B.soax_tune(k, 0)
-    B.soax_tune("xpose_ring", 0)
-    a = ev_time_ms(torch, lambda: s.from_aos(aos, n), 10)
-    b = ev_time_ms(torch, lambda: s.to_aos(aos), 10)
-    print(json.dumps({"sweep": "xpose", "variant": "one tile per CTA visit (xpose_ring = 0)", "aos_to_soa_GBps": round(80 * n / a / 1e6, 1),
-                      "soa_to_aos_GBps": round(80 * n / b / 1e6, 1)}), flush=True)
-    B.soax_tune("xpose_ring", 1)
-    t = Cn.Soax(Cn.R1, n)
-    ms = ev_time_ms(torch, lambda: t.copy_from(s), 10)
-    print(json.dumps({"sweep": "streams", "copy": "soax_copy: 7 inputs -> 7 outputs (7 cudaMemcpyAsync D2D)", "ms": round(ms, 5),
-                      "GBps_80B": round(80 * n / ms / 1e6, 1)}), flush=True)
-    del t, aos
-    W = (("a", B.SOAX_F64, 1), ("b", B.SOAX_F64, 7))
-    w = Cn.Soax(W, n, dynamic=True)
-    w.slab.zero_()
-    fan_out = Cn.Program(W, "; ".join(f"b[{c}] = a" for c in range(7)), dynamic=True)
-    fan_in = Cn.Program(W, "a = " + " + ".join(f"b[{c}]" for c in range(7)), dynamic=True)
-    one = Cn.Program(W, "b[0] = a", dynamic=True)
-    for name, prog in (("1 input -> 7 outputs", fan_out), ("7 inputs -> 1 output", fan_in)):
-        ms = ev_time_ms(torch, lambda: prog.run(w, nsteps=20), 3, 1) / 20
-        print(json.dumps({"sweep": "streams", "copy": name + " (generated kernel, 8-byte elements, 256-bit accesses)", "ms": round(ms, 5),
-                          "GBps_64B": round(64 * n / ms / 1e6, 1)}), flush=True)
-    ms = ev_time_ms(torch, lambda: one.run(w, nsteps=20), 3, 1) / 20
-    print(json.dumps({"sweep": "streams", "copy": "1 input -> 1 output (generated kernel)", "ms": round(ms, 5), "GBps_16B": round(16 * n / ms / 1e6, 1)}), flush=True)
-
-
 def run_paper_replica(torch, B, Cn, max_log2n: int = 27) -> None:
     """NEXT-1 (--paper-replica): the paper's own experiment on B200 -- Eq. 1, x += dt v in float,
     SoA of six float arrays against AoS of Particle<SIZE> = {float x[3]; float v[3]; float temp[SIZE]} (Listing 4),
@@ -971,15 +830,6 @@ def _run_soax(args) -> None:
     kind = B.SOAX_STEP_SYMPLECTIC_EULER_HARMONIC
     if args.tour:
         run_tour(torch, B, Cn)
-        return
-    if args.bin_study:
-        run_bin_study(torch, B, Cn)
-        return
-    if args.scatter_trace:
-        run_scatter_trace(torch, B, Cn, args.scatter_trace)
-        return
-    if args.sweeps:
-        run_sweeps(torch, B, Cn)
         return
     if args.paper_replica:
         run_paper_replica(torch, B, Cn)
@@ -1219,10 +1069,6 @@ def main() -> None:
     ap.add_argument("--only-extras", default="", help="comma list of energy,config3,config1,config4,config5,expr,container: run just those")
     ap.add_argument("--tune", default="", help="comma list of key=value launch-shape knobs passed to soax_tune (sweeps)")
     ap.add_argument("--paper-replica", action="store_true", help="the paper's own float benchmark (Fig. 8) on B200: SoA vs AoS Particle<SIZE> against N")
-    ap.add_argument("--bin-study", action="store_true", help="design study of the counting-sort scatter (digit width, cluster size, pacing)")
-    ap.add_argument("--sweeps", action="store_true", help="launch-shape sweeps of the step and transpose kernels + the stream-count control")
-    ap.add_argument("--scatter-trace", default="", metavar="PREFIX", help="per-phase timeline of the binning scatter (needs a -DSOAX_SCATTER_TRACE study build)")
-    ap.add_argument("--mem-probes", action="store_true", help="memory-system probes behind the scatter design (half-written sectors in the L2, DRAM rate vs burst size)")
     ap.add_argument("--tour", action="store_true", help="profiling aid: launch every kernel family twice at full size, time nothing")
     ap.add_argument("--spawn-check", action="store_true", help="test aid: exercise the --gpus N launch path alone over gloo (no GPU)")
     args = ap.parse_args()
@@ -1230,10 +1076,6 @@ def main() -> None:
         raise SystemExit(spawn_ranks(args, sys.argv[1:]))
     if args.spawn_check:
         run_spawn_check(args)
-    elif args.mem_probes:                                           # stand-alone executables built from csrc/probes/*.cu
-        import subprocess
-        from paper_1710_03462_b200.build import build_probe
-        raise SystemExit(subprocess.call([build_probe("mem_probes")]) or subprocess.call([build_probe("rank_probe")]))
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -18,7 +18,7 @@ LIB = os.path.join(HERE, "libsoax.so")
 SOURCES = ["api.cu", "step_kernels.cu", "reduce_kernels.cu", "aos_kernels.cu", "bin_kernels.cu", "expr.cu", "container_kernels.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-fmad=false",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-I", INC]
-NVCC_FLAGS += os.environ.get("SOAX_NVCC_FLAGS", "").split()     # study builds only, e.g. -DSOAX_SCATTER_TRACE (bin_kernels.cu)
+NVCC_FLAGS += os.environ.get("SOAX_NVCC_FLAGS", "").split()     # extra flags for a one-off build, e.g. -DSOAX_SCATTER_TRACE (bin_kernels.cu)
 
 
 def _nvcc() -> str:
@@ -74,17 +74,6 @@ def _build_locked(verbose: bool) -> str:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     os.replace(tmp, LIB)
     return LIB
-
-
-def build_probe(name: str = "mem_probes") -> str:
-    """Compile csrc/probes/<name>.cu into a stand-alone executable under build/ (measurement aids, not part of libsoax.so)."""
-    os.makedirs(OBJ, exist_ok=True)
-    src, exe = os.path.join(CSRC, "probes", name + ".cu"), os.path.join(OBJ, name)
-    if not os.path.exists(exe) or os.path.getmtime(exe) < os.path.getmtime(src):
-        r = subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-o", exe, src], capture_output=True, text=True)
-        if r.returncode != 0:
-            raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")
-    return exe
 
 
 if __name__ == "__main__":

@@ -252,3 +252,24 @@ def test_bench_gpus_n_spawns_n_ranks():
     assert r.returncode == 0, r.stdout + r.stderr
     lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
     assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
+
+
+@pytest.mark.gpu
+def test_exchange_leg_world2_over_nccl():
+    """The exchange and the per-step migration with the product engine over the NCCL branch at world size 2 -- device tensors
+    through all_gather_into_tensor and all_to_all_single, one rank per GPU -- as `bench.py --gpus 2` runs it: the global
+    particle count and the rank-ordered kinetic energy survive, records do cross between the ranks, and the split is balanced.
+    Needs two GPUs; skipped on a one-GPU box (where the same engine runs over gloo in the test above, and over an NCCL group of
+    one rank in test_bin_exchange_product_engine_nccl_world1)."""
+    import json
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 GPUs")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "2", "--warmup", "3", "--no-extras"],
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout + r.stderr
+    line = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+    ex = line["extras"]["exchange"]
+    assert line["n_gpus"] == 2 and ex["world"] == 2 and ex["backend"] == "nccl"
+    assert ex["verified"] and ex["conserved_count"] and ex["kinetic_rel_err"] <= 1e-10
+    assert ex["all_to_all_bytes_all_ranks"] > 0 and ex["migration_particles_moved_per_step_all_ranks"] > 0
+    assert ex["imbalance_max_over_mean"] < 1.05
