@@ -199,3 +199,24 @@ def test_maximum_sizes_are_refused_before_any_launch():
         assert e.value.status == B.SOAX_ERR_UNSUPPORTED
     assert B.soax_scratch_bytes(L, (1 << 32) - 1, 64) > 40 * ((1 << 32) - 1)     # the plan itself is computed in 64 bits
     B.soax_free(a), B.soax_free(b)
+
+
+def test_committed_traffic_names_commits_that_exist():
+    """profiles/kernel_traffic.json feeds roofline.traffic in bench.py: every captured_at_commit in it must resolve in this
+    repository's history (checked here, where the history is; the GPU box gets the tree without .git), and bench.py withholds
+    the number when one does not."""
+    import json
+    import subprocess
+    import bench
+    if not os.path.isdir(os.path.join(ROOT, ".git")):
+        pytest.skip("no git history here")
+    with open(os.path.join(ROOT, "profiles", "kernel_traffic.json")) as f:
+        table = json.load(f)
+    assert table
+    for key, d in table.items():
+        rev = d["captured_at_commit"].split()[0]
+        r = subprocess.run(["git", "-C", ROOT, "cat-file", "-t", rev], capture_output=True, text=True)
+        assert r.returncode == 0 and r.stdout.strip() == "commit", (key, rev)
+        traffic, prov = bench.committed_traffic(key)
+        assert traffic == d["dram_bytes_per_launch"] and "rejected" not in prov
+    assert bench.commit_in_history("0123456789abcdef0123456789abcdef01234567") is False
